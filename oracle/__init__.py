@@ -1,0 +1,5 @@
+"""CPU oracle of the forward 3DGS tile rasterizer -- TEST INFRASTRUCTURE, not the product.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this
+package.  It shares no code with paper_2606_16566_b200 (the CUDA path) and neither imports the other.
+"""

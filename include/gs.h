@@ -1,0 +1,114 @@
+/* gs.h -- C ABI of the B200-native forward 3D Gaussian Splatting tile rasterizer (libgs.so).
+ *
+ * What it computes: the forward 3DGS render pipeline of PAPER.md:51-53 (Fig. 2: preprocess -> duplication +
+ * sort -> render) with the render kernel of Local-GS (Sec. III: tile-local hoisting Eq. 1-10, warp-level
+ * culling Eq. 13-21, warp-coherent blending Eq. 22 / Alg. 1).  Everything the paper leaves open (near plane,
+ * dilation, rect rounding, SH convention, termination rule ...) follows the readings listed in DESIGN.md.
+ *
+ * Conventions
+ *   - "dev" pointers are CUDA device pointers owned by the caller (e.g. torch tensors); "host" pointers are
+ *     ordinary host memory read during the call.  The library never allocates or frees caller-visible memory and
+ *     keeps no reference to any pointer after the call returns, except that gs_get_intermediates() returns
+ *     pointers INTO the caller's workspace.
+ *   - Matrices are 16 floats, row-major, column-vector convention (p_cam = V * [p;1]).
+ *   - All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *     gs_render() returns after enqueueing; it performs NO host synchronisation unless timing is enabled.
+ *   - Return value: 0 (GS_OK) or a negative error code; nothing is printed, thrown or exit()ed.
+ *   - Not thread-safe per workspace; distinct workspaces on distinct streams may be used concurrently.
+ */
+#ifndef GS_H
+#define GS_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GS_OK 0
+#define GS_ERR_BAD_ARG (-1)   /* null pointer, P < 0, W/H <= 0, sh_degree not in [0,3], > 2^24 tiles ...         */
+#define GS_ERR_WORKSPACE (-2) /* workspace_bytes < gs_workspace_bytes(P, W, H, max_dup) or misaligned pointer    */
+#define GS_ERR_OVERFLOW (-3)  /* reported by gs_get_intermediates: the frame needed more than max_dup duplicates */
+#define GS_ERR_CUDA (-4)      /* a CUDA runtime call failed; gs_last_cuda_error() returns its cudaError_t        */
+
+#define GS_TILE 16            /* tile edge in pixels                                         */
+
+/* Scratch size (bytes) that gs_render needs for P Gaussians, a W x H image and room for `max_dup` duplicated
+ * (tile, Gaussian) entries ("duplicates the surviving primitives across intersecting tiles").
+ * Returns 0 on bad arguments.  max_dup must be < 2^32. */
+size_t gs_workspace_bytes(int P, int W, int H, uint64_t max_dup);
+
+/* Forward render of one frame.
+ *
+ *  Per-Gaussian inputs: dev, fp32, read-only, reusable across calls
+ *    means3D   [P,3]   world-space centres
+ *    scales    [P,3]   ACTIVATED scales (positive)
+ *    rotations [P,4]   unit quaternions (w,x,y,z); not re-normalised
+ *    opacities [P]     ACTIVATED opacities in (0,1)
+ *    sh_coeffs [P,K,3] K = (sh_degree+1)^2, coefficient-major, RGB innermost
+ *  Camera (host): viewmatrix (world->camera), projmatrix (FULL transform Proj*V), fx, fy in pixels, W, H, bg[3].
+ *  Outputs (dev, fully overwritten):
+ *    out_rgb         [3,H,W] planar fp32:  C + T_final * bg
+ *    out_final_T     [H,W]   fp32 final transmittance
+ *    out_tile_counts [gy*gx] u32, gx=(W+15)/16, gy=(H+15)/16: length of each tile's sorted list
+ *    out_n_contrib   [H,W]   u32 number of Gaussians blended into the pixel, or NULL
+ *  workspace: dev, 256-byte aligned, >= gs_workspace_bytes(P, W, H, max_dup) bytes; max_dup is recovered from
+ *    workspace_bytes (the largest capacity that fits).  If the frame produces more duplicates than fit, the image
+ *    is rendered from the truncated lists and gs_get_intermediates() reports GS_ERR_OVERFLOW.
+ */
+int gs_render(int P, const float* means3D, const float* scales, const float* rotations, const float* opacities,
+              const float* sh_coeffs, int sh_degree, const float* viewmatrix, const float* projmatrix, float fx,
+              float fy, int W, int H, const float* bg, float* out_rgb, float* out_final_T,
+              uint32_t* out_tile_counts, uint32_t* out_n_contrib, void* workspace, size_t workspace_bytes,
+              void* cuda_stream);
+
+/* Pointers into the workspace of the LAST gs_render() call on it (valid until the next call on that workspace).
+ * For parity tests and diagnostics; calling it synchronises the stream of that call. */
+typedef struct gs_intermediates {
+    int32_t P, W, H, grid_x, grid_y, n_tiles;
+    uint32_t n_visible;            /* Gaussians with tiles_touched > 0                                           */
+    uint64_t n_dup;                /* total duplicated entries the frame needs = sum of tiles_touched            */
+    uint64_t max_dup;              /* capacity of this workspace                                                  */
+    const uint32_t* per_gaussian;  /* dev [P,4] u32: {xmin | ymin<<16, xmax | ymax<<16, depth bits, radius};
+                                      rect in tiles, half-open; all zero for a culled Gaussian                   */
+    const float* geom;             /* dev [P,8]: mu_x, mu_y, conic a, b, c, log2(opacity), a*c-b*b, flags(bits);
+                                      defined only where tiles_touched > 0                                       */
+    const float* colour;           /* dev [P,4]: r, g, b, 0 (SH colour clamped at 0); defined where visible      */
+    const uint64_t* depth_sorted;  /* dev [n_visible]: (depth bits << 32 | Gaussian id), ascending, stable       */
+    const uint32_t* dup_offsets;   /* dev [n_visible]: exclusive prefix sum of tiles_touched in depth order      */
+    const uint32_t* tile_ranges;   /* dev [n_tiles+1]: list of tile t is sorted_ids[tile_ranges[t] .. [t+1])     */
+    const uint32_t* sorted_ids;    /* dev [min(n_dup,max_dup)]: Gaussian ids, by (tile, depth bits, id)          */
+} gs_intermediates;
+int gs_get_intermediates(const void* workspace, gs_intermediates* out);
+
+/* Per-stage device times (ms, CUDA events) of the last gs_render() on this workspace made while timing was
+ * enabled with gs_set_timing(1): [0] preprocess, [1] depth sort, [2] tile grid, [3] offset scan, [4] duplicate,
+ * [5] tile sort, [6] render, [7] whole frame.  Enabling timing adds event records and one stream synchronisation
+ * per frame; it is off by default. */
+#define GS_N_TIMINGS 8
+int gs_set_timing(int enable);
+int gs_get_timings(const void* workspace, float ms[GS_N_TIMINGS]);
+
+/* Render-kernel variant (ablation ladder of PAPER.md Table IV):
+ *   0 = baseline column of Alg. 1 (one thread per pixel, direct conic, per-pixel branches)
+ *   1 = + tile-local hoisting (Eq. 7-10)
+ *   2 = + warp-level culling (Eq. 13-21)
+ *   3 = + warp-coherent blending (Eq. 22, branch-free)            -- the paper's full method
+ *   4 = B200 design (default): 2 pixels/thread, packed f32x2, per-warp ballot compaction, prefetched staging
+ * Returns GS_ERR_BAD_ARG for an unknown variant.  Process-wide. */
+int gs_set_render_variant(int variant);
+int gs_get_render_variant(void);
+
+/* Number of kernel launches (ours; memsets not counted) enqueued by the last gs_render() in this process. */
+int gs_last_launch_count(void);
+
+/* Synchronous device->host copy of `bytes` bytes (a plain cudaMemcpy) -- lets a binding without CUDA runtime access
+ * read the arrays gs_get_intermediates() points at. */
+int gs_copy_to_host(void* dst_host, const void* src_dev, size_t bytes);
+
+const char* gs_error_string(int code);
+int gs_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,306 @@
+// api.cu -- the C ABI of include/gs.h: workspace carving, the per-frame launch sequence, inspection and timing.
+// Every step of the path runs in the kernels of preprocess.cu / binning.cu / render*.cu; this file only enqueues.
+#include "../../include/gs.h"
+
+#include <atomic>
+#include <map>
+#include <mutex>
+
+#include "common.cuh"
+
+namespace gs {
+void launch_preprocess(const Frame&, const Pointers&, const float*, const float*, const float*, const float*, const float*,
+                       int, cudaStream_t);
+void launch_depth_sort(const Frame&, const Pointers&, int, cudaStream_t, int*);
+void launch_tile_grid(const Frame&, const Pointers&, uint32_t*, cudaStream_t, int*);
+void launch_scan_offsets(const Frame&, const Pointers&, int, cudaStream_t, int*);
+void launch_duplicate_and_tile_sort(const Frame&, const Pointers&, int, cudaStream_t, int*, cudaEvent_t);
+void launch_render_ladder(int, const Frame&, const Pointers&, float*, float*, uint32_t*, cudaStream_t);
+void launch_render_b200(const Frame&, const Pointers&, float*, float*, uint32_t*, int, cudaStream_t);
+}  // namespace gs
+
+namespace {
+using namespace gs;
+
+constexpr size_t ALIGN = 256;
+size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+    size_t ctrl, diff, st_pre, st_scan, st_depth, st_tile, zero_end;
+    size_t per_g, geom, colour, gkeyA, gkeyB, dup_off, chunk_start, ranges, entA, entB, ids, total;
+    size_t n_depth_tiles, n_tile_tiles;
+    int gx, gy, n_tiles, tile_bits, n_tile_passes;
+};
+
+bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
+    if (P < 0 || W <= 0 || H <= 0 || max_dup >= (1ull << 32)) return false;
+    L.gx = (W + TILE - 1) / TILE;
+    L.gy = (H + TILE - 1) / TILE;
+    const long long nt = (long long)L.gx * L.gy;
+    if (nt > (1ll << 24) || L.gx > 65535 || L.gy > 65535) return false;
+    L.n_tiles = (int)nt;
+    L.tile_bits = 1;
+    while ((1ll << L.tile_bits) < nt) L.tile_bits++;
+    L.n_tile_passes = (L.tile_bits + 7) / 8;
+    const size_t Pz = (size_t)P;
+    L.n_depth_tiles = (Pz + SORT_TILE - 1) / SORT_TILE + 1;
+    L.n_tile_tiles = ((size_t)max_dup + SORT_TILE - 1) / SORT_TILE + 1;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { const size_t at = o; o = up(o + bytes); return at; };
+    L.ctrl = take(sizeof(Ctrl));
+    L.diff = take(sizeof(int) * (size_t)(L.gx + 1) * (L.gy + 1));
+    L.st_pre = take(8 * ((Pz + PRE_THREADS - 1) / PRE_THREADS + 1));
+    L.st_scan = take(8 * ((Pz + SCAN_TILE - 1) / SCAN_TILE + 1));
+    L.st_depth = take(8 * 256 * L.n_depth_tiles * MAX_SORT_PASSES_DEPTH);
+    L.st_tile = take(8 * 256 * L.n_tile_tiles * (size_t)L.n_tile_passes);
+    L.zero_end = o;
+    L.per_g = take(16 * Pz);
+    L.geom = take(32 * Pz);
+    L.colour = take(16 * Pz);
+    L.gkeyA = take(8 * Pz);
+    L.gkeyB = take(8 * Pz);
+    L.dup_off = take(4 * Pz);
+    L.chunk_start = take(4 * (((size_t)max_dup + DUP_TILE - 1) / DUP_TILE + 2));
+    L.ranges = take(4 * ((size_t)L.n_tiles + 1));
+    L.entA = take(8 * (size_t)max_dup);
+    L.entB = take(L.n_tile_passes >= 2 ? 8 * (size_t)max_dup : 0);
+    L.ids = take(4 * (size_t)max_dup + 16);
+    L.total = o;
+    return true;
+}
+
+struct LastCall {
+    Layout L;
+    Frame f;
+    unsigned long long max_dup = 0;
+    cudaStream_t stream = nullptr;
+    bool valid = false, timed = false;
+    cudaEvent_t ev[GS_N_TIMINGS + 2] = {};
+    bool have_events = false;
+};
+
+std::mutex g_mu;
+std::map<const void*, LastCall> g_calls;
+std::atomic<int> g_variant{4}, g_timing{0}, g_launches{0}, g_cuda_err{0};
+int g_n_sm = 0;
+
+int cuda_fail(cudaError_t e) {
+    g_cuda_err.store((int)e);
+    return GS_ERR_CUDA;
+}
+
+Pointers carve(void* ws, const Layout& L) {
+    char* b = static_cast<char*>(ws);
+    Pointers p;
+    p.ctrl = reinterpret_cast<Ctrl*>(b + L.ctrl);
+    p.diff = reinterpret_cast<int*>(b + L.diff);
+    p.st_pre = reinterpret_cast<unsigned long long*>(b + L.st_pre);
+    p.st_scan = reinterpret_cast<unsigned long long*>(b + L.st_scan);
+    p.st_depth = reinterpret_cast<unsigned long long*>(b + L.st_depth);
+    p.st_tile = reinterpret_cast<unsigned long long*>(b + L.st_tile);
+    p.per_g = reinterpret_cast<uint4*>(b + L.per_g);
+    p.geom = reinterpret_cast<float4*>(b + L.geom);
+    p.colour = reinterpret_cast<float4*>(b + L.colour);
+    p.gkeyA = reinterpret_cast<unsigned long long*>(b + L.gkeyA);
+    p.gkeyB = reinterpret_cast<unsigned long long*>(b + L.gkeyB);
+    p.dup_off = reinterpret_cast<uint32_t*>(b + L.dup_off);
+    p.chunk_start = reinterpret_cast<uint32_t*>(b + L.chunk_start);
+    p.ranges = reinterpret_cast<uint32_t*>(b + L.ranges);
+    p.entA = reinterpret_cast<unsigned long long*>(b + L.entA);
+    p.entB = reinterpret_cast<unsigned long long*>(b + L.entB);
+    p.ids = reinterpret_cast<uint32_t*>(b + L.ids);
+    p.n_depth_tiles = L.n_depth_tiles;
+    p.n_tile_tiles = L.n_tile_tiles;
+    return p;
+}
+
+// largest max_dup whose layout fits into `bytes` (layout size is monotone in max_dup); false if even 0 does not fit
+bool fit_max_dup(int P, int W, int H, size_t bytes, unsigned long long& max_dup) {
+    Layout L;
+    if (!make_layout(P, W, H, 0, L) || L.total > bytes) return false;
+    unsigned long long lo = 0, hi = (1ull << 32) - 1;
+    while (lo < hi) {
+        const unsigned long long mid = lo + (hi - lo + 1) / 2;
+        make_layout(P, W, H, mid, L);
+        if (L.total <= bytes) lo = mid; else hi = mid - 1;
+    }
+    max_dup = lo;
+    return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t gs_workspace_bytes(int P, int W, int H, uint64_t max_dup) {
+    Layout L;
+    if (!make_layout(P, W, H, max_dup, L)) return 0;
+    return L.total;
+}
+
+int gs_render(int P, const float* means3D, const float* scales, const float* rotations, const float* opacities,
+              const float* sh_coeffs, int sh_degree, const float* viewmatrix, const float* projmatrix, float fx, float fy,
+              int W, int H, const float* bg, float* out_rgb, float* out_final_T, uint32_t* out_tile_counts,
+              uint32_t* out_n_contrib, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (P < 0 || W <= 0 || H <= 0 || sh_degree < 0 || sh_degree > 3 || !viewmatrix || !projmatrix || !bg || !out_rgb ||
+        !out_final_T || !out_tile_counts || !workspace || !(fx > 0.0f) || !(fy > 0.0f))
+        return GS_ERR_BAD_ARG;
+    if (P > 0 && (!means3D || !scales || !rotations || !opacities || !sh_coeffs)) return GS_ERR_BAD_ARG;
+    if (reinterpret_cast<uintptr_t>(workspace) % ALIGN) return GS_ERR_WORKSPACE;
+    unsigned long long max_dup = 0;
+    Layout L;
+    if (!make_layout(P, W, H, 0, L)) return GS_ERR_BAD_ARG;
+    if (!fit_max_dup(P, W, H, workspace_bytes, max_dup)) return GS_ERR_WORKSPACE;
+    make_layout(P, W, H, max_dup, L);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (g_n_sm == 0) {
+        int dev = 0, n = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return cuda_fail(e);
+        g_n_sm = n;
+    }
+    Frame f;
+    f.P = P; f.W = W; f.H = H; f.gx = L.gx; f.gy = L.gy; f.n_tiles = L.n_tiles;
+    f.deg = sh_degree; f.K = (sh_degree + 1) * (sh_degree + 1);
+    f.tile_bits = L.tile_bits; f.n_tile_passes = L.n_tile_passes;
+    for (int k = 0; k < 16; k++) { f.V[k] = viewmatrix[k]; f.PM[k] = projmatrix[k]; }
+    f.fx = fx; f.fy = fy;
+    // camera centre of the rigid view matrix: campos = -Wv^T t (the north_star signature carries no campos)
+    for (int c = 0; c < 3; c++)
+        f.campos[c] = (float)-((double)viewmatrix[c] * viewmatrix[3] + (double)viewmatrix[4 + c] * viewmatrix[7] +
+                               (double)viewmatrix[8 + c] * viewmatrix[11]);
+    for (int c = 0; c < 3; c++) f.bg[c] = bg[c];
+    f.max_dup = max_dup;
+    const Pointers p = carve(workspace, L);
+
+    const bool timed = g_timing.load() != 0;
+    LastCall* lc;
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        lc = &g_calls[workspace];
+    }
+    if (timed && !lc->have_events) {
+        for (auto& e : lc->ev)
+            if (cudaEventCreate(&e) != cudaSuccess) return cuda_fail(cudaGetLastError());
+        lc->have_events = true;
+    }
+    lc->L = L; lc->f = f; lc->max_dup = max_dup; lc->stream = st; lc->valid = true; lc->timed = timed;
+    auto mark = [&](int k) { if (timed) cudaEventRecord(lc->ev[k], st); };
+
+    int launches = 0;
+    mark(0);
+    cudaError_t e = cudaMemsetAsync(workspace, 0, L.zero_end, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    {   // (1) preprocess + compaction + depth histograms + coverage grid
+        const long long tiles = ((long long)P + PRE_THREADS - 1) / PRE_THREADS;
+        const int grid = (int)(tiles < 1 ? 1 : (tiles < (long long)g_n_sm * 8 ? tiles : (long long)g_n_sm * 8));
+        launch_preprocess(f, p, means3D, scales, rotations, opacities, sh_coeffs, grid, st);
+        launches++;
+    }
+    mark(1);
+    launch_depth_sort(f, p, g_n_sm, st, &launches);          // (3a) LSD passes over the depth bits, pre-duplication
+    mark(2);
+    launch_tile_grid(f, p, out_tile_counts, st, &launches);   // tile counts, ranges, N_dup, tile-digit histograms
+    mark(3);
+    launch_scan_offsets(f, p, g_n_sm, st, &launches);         // (2) prefix-sum offsets
+    mark(4);
+    launch_duplicate_and_tile_sort(f, p, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b)
+    mark(6);
+    const int variant = g_variant.load();                      // (4) render
+    if (variant >= 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, st);
+    else launch_render_ladder(variant, f, p, out_rgb, out_final_T, out_n_contrib, st);
+    launches++;
+    mark(7);
+    g_launches.store(launches);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (timed) {
+        e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    return GS_OK;
+}
+
+int gs_get_intermediates(const void* workspace, gs_intermediates* out) {
+    if (!workspace || !out) return GS_ERR_BAD_ARG;
+    LastCall lc;
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        auto it = g_calls.find(workspace);
+        if (it == g_calls.end() || !it->second.valid) return GS_ERR_BAD_ARG;
+        lc = it->second;
+    }
+    cudaError_t e = cudaStreamSynchronize(lc.stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    Ctrl c;
+    e = cudaMemcpy(&c, static_cast<const char*>(workspace) + lc.L.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(e);
+    const Pointers p = carve(const_cast<void*>(workspace), lc.L);
+    out->P = lc.f.P; out->W = lc.f.W; out->H = lc.f.H; out->grid_x = lc.f.gx; out->grid_y = lc.f.gy;
+    out->n_tiles = lc.f.n_tiles;
+    out->n_visible = (uint32_t)c.n_vis;
+    out->n_dup = c.n_dup;
+    out->max_dup = lc.max_dup;
+    out->per_gaussian = reinterpret_cast<const uint32_t*>(p.per_g);
+    out->geom = reinterpret_cast<const float*>(p.geom);
+    out->colour = reinterpret_cast<const float*>(p.colour);
+    out->depth_sorted = reinterpret_cast<const uint64_t*>(p.gkeyA);
+    out->dup_offsets = p.dup_off;
+    out->tile_ranges = p.ranges;
+    out->sorted_ids = p.ids;
+    return c.overflow ? GS_ERR_OVERFLOW : GS_OK;
+}
+
+int gs_set_timing(int enable) {
+    g_timing.store(enable ? 1 : 0);
+    return GS_OK;
+}
+
+int gs_get_timings(const void* workspace, float ms[GS_N_TIMINGS]) {
+    if (!workspace || !ms) return GS_ERR_BAD_ARG;
+    LastCall lc;
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        auto it = g_calls.find(workspace);
+        if (it == g_calls.end() || !it->second.valid || !it->second.timed) return GS_ERR_BAD_ARG;
+        lc = it->second;
+    }
+    cudaError_t e = cudaEventSynchronize(lc.ev[7]);
+    if (e != cudaSuccess) return cuda_fail(e);
+    // events: 0 start | 1 after preprocess | 2 after depth sort | 3 after tile grid | 4 after offset scan |
+    //         5 after duplicate | 6 after tile sort | 7 after render
+    for (int k = 0; k < 7; k++)
+        if ((e = cudaEventElapsedTime(&ms[k], lc.ev[k], lc.ev[k + 1])) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaEventElapsedTime(&ms[7], lc.ev[0], lc.ev[7])) != cudaSuccess) return cuda_fail(e);
+    return GS_OK;
+}
+
+int gs_copy_to_host(void* dst_host, const void* src_dev, size_t bytes) {
+    if (bytes == 0) return GS_OK;
+    if (!dst_host || !src_dev) return GS_ERR_BAD_ARG;
+    const cudaError_t e = cudaMemcpy(dst_host, src_dev, bytes, cudaMemcpyDeviceToHost);
+    return e == cudaSuccess ? GS_OK : cuda_fail(e);
+}
+
+int gs_set_render_variant(int variant) {
+    if (variant < 0 || variant > 4) return GS_ERR_BAD_ARG;
+    g_variant.store(variant);
+    return GS_OK;
+}
+int gs_get_render_variant(void) { return g_variant.load(); }
+int gs_last_launch_count(void) { return g_launches.load(); }
+int gs_last_cuda_error(void) { return g_cuda_err.load(); }
+
+const char* gs_error_string(int code) {
+    switch (code) {
+        case GS_OK: return "ok";
+        case GS_ERR_BAD_ARG: return "bad argument";
+        case GS_ERR_WORKSPACE: return "workspace too small or misaligned";
+        case GS_ERR_OVERFLOW: return "more duplicated entries than the workspace capacity (max_dup)";
+        case GS_ERR_CUDA: return "CUDA runtime error (see gs_last_cuda_error)";
+        default: return "unknown error";
+    }
+}
+
+}  // extern "C"

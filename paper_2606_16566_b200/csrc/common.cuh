@@ -1,0 +1,132 @@
+// common.cuh -- workspace layout, control block and small device helpers shared by the CUDA translation units.
+// Product code (libgs.so).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gs {
+
+constexpr int TILE = 16;
+constexpr int MAX_SORT_PASSES_DEPTH = 4;   // 32 depth bits, 8-bit digits
+constexpr int MAX_SORT_PASSES_TILE = 3;    // up to 24 tile-id bits
+constexpr int SORT_THREADS = 256;
+constexpr int SORT_ITEMS = 16;
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;  // 4096 elements per block-tile
+constexpr int PRE_THREADS = 256;                      // Gaussians per preprocess tile
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;  // 2048 sorted Gaussians per offset-scan tile
+constexpr int DUP_THREADS = 256;
+constexpr int DUP_ITEMS = 8;
+constexpr int DUP_TILE = DUP_THREADS * DUP_ITEMS;     // 2048 duplicated entries per block
+
+// Control block at the start of the workspace; zeroed (with the tile-difference grid and the look-back status
+// arrays that follow it) by one cudaMemsetAsync per frame.
+struct Ctrl {
+    uint32_t tile_counter[16];          // dynamic tile ids of the chained-scan kernels (forward-progress order)
+    unsigned long long n_vis;           // visible Gaussians (compacted count)
+    unsigned long long overflow;        // 1 if n_dup > max_dup
+    unsigned long long n_dup;           // duplicates the frame needs
+    unsigned long long n_dup_eff;       // duplicates actually produced (0 on overflow)
+    uint32_t depth_hist[MAX_SORT_PASSES_DEPTH][256];  // global digit histograms of the depth bits (atomics)
+    uint32_t tile_hist[MAX_SORT_PASSES_TILE][256];    // global digit histograms of the tile ids (from tile counts)
+};
+enum { TC_PRE = 0, TC_DEPTH0 = 1, TC_SCAN = 5, TC_TILE0 = 6 };
+
+// Look-back status word: [63:62] flag, [61:0] value.
+constexpr unsigned long long ST_EMPTY = 0ull;
+constexpr unsigned long long ST_AGG = 1ull << 62;
+constexpr unsigned long long ST_INC = 2ull << 62;
+constexpr unsigned long long ST_MASK = (1ull << 62) - 1;
+
+struct Frame {              // per-frame constants, passed by value to the kernels
+    int P, W, H, gx, gy, n_tiles, deg, K;
+    int tile_bits, n_tile_passes;
+    float V[16], PM[16];
+    float fx, fy;
+    float campos[3];
+    float bg[3];
+    unsigned long long max_dup;
+};
+
+struct Pointers {           // device pointers carved from the workspace
+    Ctrl* ctrl;
+    int* diff;                              // [(gy+1)*(gx+1)] 2-D difference grid of tile coverage
+    unsigned long long* st_pre;             // [pre tiles]    look-back status: compaction of visible Gaussians
+    unsigned long long* st_scan;            // [scan tiles]   look-back status: duplicate offsets
+    unsigned long long* st_depth;           // [4][depth sort tiles][256]
+    unsigned long long* st_tile;            // [3][tile sort tiles][256]
+    uint4* per_g;                           // [P] {rect01, rect23, depth bits, radius}
+    float4* geom;                           // [P][2]
+    float4* colour;                         // [P]
+    unsigned long long* gkeyA;              // [P] (depth bits << 32 | id), compacted
+    unsigned long long* gkeyB;              // [P] ping-pong
+    uint32_t* dup_off;                      // [P] exclusive prefix of tiles_touched in depth order
+    uint32_t* chunk_start;                  // [ceil(max_dup / DUP_TILE) + 1] depth rank owning entry c * DUP_TILE
+    uint32_t* ranges;                       // [n_tiles + 1]
+    unsigned long long* entA;               // [max_dup] (tile << 32 | id)
+    unsigned long long* entB;               // [max_dup] ping-pong
+    uint32_t* ids;                          // [max_dup] final sorted Gaussian ids
+    size_t n_depth_tiles, n_tile_tiles;     // status array strides (tiles per pass)
+};
+
+__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// Warp-parallel decoupled look-back over single-value status words (called by one full warp).
+// Returns the exclusive prefix of tile `tile` (sum of the aggregates of tiles 0..tile-1) in every lane.
+__device__ __forceinline__ unsigned long long lookback_warp(const unsigned long long* status, int tile) {
+    const int lane = threadIdx.x & 31;
+    unsigned long long excl = 0;
+    int idx = tile - 1;
+    while (idx >= 0) {
+        const int my = idx - lane;
+        unsigned long long s = ST_INC;  // tiles before 0: inclusive prefix 0
+        if (my >= 0) {
+            do { s = ld_status(status + my); } while ((s >> 62) == 0);
+        }
+        const unsigned inc = __ballot_sync(0xffffffffu, (s >> 62) == 2);
+        unsigned long long v = s & ST_MASK;
+        if (inc) {
+            const int first = __ffs(inc) - 1;  // nearest tile with an inclusive prefix
+            if (lane > first) v = 0;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        excl += v;
+        if (inc) break;
+        idx -= 32;
+    }
+    return excl;
+}
+
+// Block-wide exclusive scan of one u32 per thread (blockDim.x == 256); returns the exclusive prefix and the total.
+__device__ __forceinline__ uint32_t block_excl_scan_256(uint32_t v, uint32_t* smem_warp /*[8]*/, uint32_t& total) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) smem_warp[w] = inc;
+    __syncthreads();
+    uint32_t base = 0, tot = 0;
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+        const uint32_t s = smem_warp[i];
+        if (i < w) base += s;
+        tot += s;
+    }
+    total = tot;
+    __syncthreads();
+    return base + inc - v;
+}
+
+}  // namespace gs

@@ -1,0 +1,280 @@
+// preprocess.cu -- per-Gaussian preprocess (DESIGN.md steps C-P0..C-P9), fused with
+//   * order-preserving compaction of the visible Gaussians (single-pass chained scan, decoupled look-back),
+//   * the global digit histograms of the depth bits (for the depth radix sort),
+//   * the 2-D difference grid of tile coverage (from which tile counts and tile ranges follow without ever
+//     reading the duplicated keys).
+//
+// Arithmetic contract: C-P0..C-P8 are evaluated in IEEE binary32 with ONE rounding per written operation, in the
+// canonical order of DESIGN.md -- every operation below is an explicit round-to-nearest intrinsic
+// (__fmul_rn/__fadd_rn/__fsub_rn/__fdiv_rn/__fsqrt_rn are never contracted into FMAs and ignore -use_fast_math),
+// so depth bits, radius, rect and tiles_touched are unique integers any conforming implementation reproduces.
+// C-P9 (SH colour) is free-order fp32 (a toleranced output).
+#include "common.cuh"
+
+namespace gs {
+
+__device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float dvd(float a, float b) { return __fdiv_rn(a, b); }
+__device__ __forceinline__ float sqr(float a) { return __fsqrt_rn(a); }
+// ((m0*x + m1*y) + m2*z) + m3
+__device__ __forceinline__ float affine(const float* m, float x, float y, float z) {
+    return add(add(add(mul(m[0], x), mul(m[1], y)), mul(m[2], z)), m[3]);
+}
+__device__ __forceinline__ float dot3(float a0, float a1, float a2, float b0, float b1, float b2) {
+    return add(add(mul(a0, b0), mul(a1, b1)), mul(a2, b2));
+}
+
+struct Splat {
+    float mux, muy, ca, cb, cc, depth;
+    int radius, xmin, ymin, xmax, ymax;
+};
+
+// C-P0..C-P8.  Returns false when the Gaussian is culled.
+__device__ __forceinline__ bool project(const Frame& f, float px, float py, float pz, float sx, float sy, float sz,
+                                        float qw, float qx, float qy, float qz, Splat& o) {
+    const float* V = f.V;
+    const float* PM = f.PM;
+    const float Wf = (float)f.W, Hf = (float)f.H;
+    // C-P0 camera space; near plane 0.2 (reading S2)
+    const float pc0 = affine(V + 0, px, py, pz), pc1 = affine(V + 4, px, py, pz), pc2 = affine(V + 8, px, py, pz);
+    if (!(pc2 > 0.2f)) return false;
+    // C-P1 clip -> pixel (reading S1)
+    const float h0 = affine(PM + 0, px, py, pz), h1 = affine(PM + 4, px, py, pz), h3 = affine(PM + 12, px, py, pz);
+    const float iw = dvd(1.0f, add(h3, 1e-7f));
+    const float ndcx = mul(h0, iw), ndcy = mul(h1, iw);
+    const float mux = mul(sub(mul(add(ndcx, 1.0f), Wf), 1.0f), 0.5f);
+    const float muy = mul(sub(mul(add(ndcy, 1.0f), Hf), 1.0f), 0.5f);
+    if (!(fabsf(mux) <= 1.0e9f) || !(fabsf(muy) <= 1.0e9f)) return false;
+    // C-P2 rotation (reading S19)
+    const float R00 = sub(1.0f, mul(2.0f, add(mul(qy, qy), mul(qz, qz))));
+    const float R01 = mul(2.0f, sub(mul(qx, qy), mul(qw, qz)));
+    const float R02 = mul(2.0f, add(mul(qx, qz), mul(qw, qy)));
+    const float R10 = mul(2.0f, add(mul(qx, qy), mul(qw, qz)));
+    const float R11 = sub(1.0f, mul(2.0f, add(mul(qx, qx), mul(qz, qz))));
+    const float R12 = mul(2.0f, sub(mul(qy, qz), mul(qw, qx)));
+    const float R20 = mul(2.0f, sub(mul(qx, qz), mul(qw, qy)));
+    const float R21 = mul(2.0f, add(mul(qy, qz), mul(qw, qx)));
+    const float R22 = sub(1.0f, mul(2.0f, add(mul(qx, qx), mul(qy, qy))));
+    // C-P3 Sigma = (R S)(R S)^T
+    const float M00 = mul(R00, sx), M01 = mul(R01, sy), M02 = mul(R02, sz);
+    const float M10 = mul(R10, sx), M11 = mul(R11, sy), M12 = mul(R12, sz);
+    const float M20 = mul(R20, sx), M21 = mul(R21, sy), M22 = mul(R22, sz);
+    const float S00 = dot3(M00, M01, M02, M00, M01, M02);
+    const float S01 = dot3(M00, M01, M02, M10, M11, M12);
+    const float S02 = dot3(M00, M01, M02, M20, M21, M22);
+    const float S11 = dot3(M10, M11, M12, M10, M11, M12);
+    const float S12 = dot3(M10, M11, M12, M20, M21, M22);
+    const float S22 = dot3(M20, M21, M22, M20, M21, M22);
+    // C-P4 Jacobian with the 1.3 guard band (reading S3)
+    const float limx = mul(1.3f, dvd(mul(0.5f, Wf), f.fx));
+    const float limy = mul(1.3f, dvd(mul(0.5f, Hf), f.fy));
+    const float tx = mul(fminf(limx, fmaxf(-limx, dvd(pc0, pc2))), pc2);
+    const float ty = mul(fminf(limy, fmaxf(-limy, dvd(pc1, pc2))), pc2);
+    const float tz = pc2;
+    const float j00 = dvd(f.fx, tz);
+    const float j02 = -dvd(mul(f.fx, tx), mul(tz, tz));
+    const float j11 = dvd(f.fy, tz);
+    const float j12 = -dvd(mul(f.fy, ty), mul(tz, tz));
+    // C-P5 cov2D = T Sigma T^T, T = J W, + 0.3 px dilation (reading S4)
+    const float T00 = add(mul(j00, V[0]), mul(j02, V[8])), T01 = add(mul(j00, V[1]), mul(j02, V[9])),
+                T02 = add(mul(j00, V[2]), mul(j02, V[10]));
+    const float T10 = add(mul(j11, V[4]), mul(j12, V[8])), T11 = add(mul(j11, V[5]), mul(j12, V[9])),
+                T12 = add(mul(j11, V[6]), mul(j12, V[10]));
+    const float U00 = dot3(T00, T01, T02, S00, S01, S02), U01 = dot3(T00, T01, T02, S01, S11, S12),
+                U02 = dot3(T00, T01, T02, S02, S12, S22);
+    const float U10 = dot3(T10, T11, T12, S00, S01, S02), U11 = dot3(T10, T11, T12, S01, S11, S12),
+                U12 = dot3(T10, T11, T12, S02, S12, S22);
+    float c00 = dot3(U00, U01, U02, T00, T01, T02);
+    const float c01 = dot3(U00, U01, U02, T10, T11, T12);
+    float c11 = dot3(U10, U11, U12, T10, T11, T12);
+    c00 = add(c00, 0.3f);
+    c11 = add(c11, 0.3f);
+    // C-P6 conic (Eq. 5); cull if !(det > 0) (reading S7)
+    const float det = sub(mul(c00, c11), mul(c01, c01));
+    if (!(det > 0.0f)) return false;
+    const float inv = dvd(1.0f, det);
+    o.ca = mul(c11, inv);
+    o.cb = -mul(c01, inv);
+    o.cc = mul(c00, inv);
+    // C-P7 3-sigma radius (reading S5)
+    const float mid = mul(0.5f, add(c00, c11));
+    const float sq = sqr(fmaxf(0.1f, sub(mul(mid, mid), det)));
+    const float lam = fmaxf(add(mid, sq), sub(mid, sq));
+    const float rf_ = ceilf(mul(3.0f, sqr(lam)));
+    if (!(rf_ <= 1.0e9f)) return false;
+    const int radius = (int)rf_;
+    // C-P8 tile rect, half-open, clamped to the grid (reading S6)
+    const float rf = (float)radius;
+    const float gxf = (float)f.gx, gyf = (float)f.gy;
+    const int xmin = (int)fminf(gxf, fmaxf(0.0f, floorf(dvd(sub(mux, rf), 16.0f))));
+    const int xmax = (int)fminf(gxf, fmaxf(0.0f, floorf(dvd(add(add(mux, rf), 15.0f), 16.0f))));
+    const int ymin = (int)fminf(gyf, fmaxf(0.0f, floorf(dvd(sub(muy, rf), 16.0f))));
+    const int ymax = (int)fminf(gyf, fmaxf(0.0f, floorf(dvd(add(add(muy, rf), 15.0f), 16.0f))));
+    if ((xmax - xmin) * (ymax - ymin) <= 0) return false;
+    o.mux = mux; o.muy = muy; o.depth = pc2; o.radius = radius;
+    o.xmin = xmin; o.ymin = ymin; o.xmax = xmax; o.ymax = ymax;
+    return true;
+}
+
+// C-P9: colour = max(0, 0.5 + sum_k (-1)^m Y_lm(d) sh[k]), k = l^2 + l + m, d = unit vector camera -> Gaussian
+// ("view-dependent color parameterized by spherical harmonics"; reading S8).
+__device__ __forceinline__ void sh_basis(int deg, float x, float y, float z, float* Y) {
+    Y[0] = 0.28209479177387814f;
+    if (deg < 1) return;
+    Y[1] = -0.4886025119029199f * y;
+    Y[2] = 0.4886025119029199f * z;
+    Y[3] = -0.4886025119029199f * x;
+    if (deg < 2) return;
+    const float xx = x * x, yy = y * y, zz = z * z;
+    Y[4] = 1.0925484305920792f * x * y;
+    Y[5] = -1.0925484305920792f * y * z;
+    Y[6] = 0.31539156525252005f * (2.0f * zz - xx - yy);
+    Y[7] = -1.0925484305920792f * x * z;
+    Y[8] = 0.5462742152960396f * (xx - yy);
+    if (deg < 3) return;
+    Y[9] = -0.5900435899266435f * y * (3.0f * xx - yy);
+    Y[10] = 2.890611442640554f * x * y * z;
+    Y[11] = -0.4570457994644658f * y * (4.0f * zz - xx - yy);
+    Y[12] = 0.3731763325901154f * z * (2.0f * zz - 3.0f * xx - 3.0f * yy);
+    Y[13] = -0.4570457994644658f * x * (4.0f * zz - xx - yy);
+    Y[14] = 1.445305721320277f * z * (xx - yy);
+    Y[15] = -0.5900435899266435f * x * (xx - 3.0f * yy);
+}
+
+__device__ __forceinline__ float3 sh_colour(const Frame& f, const float* __restrict__ sh, int i, float px, float py,
+                                            float pz) {
+    float dx = px - f.campos[0], dy = py - f.campos[1], dz = pz - f.campos[2];
+    const float rn = rsqrtf(dx * dx + dy * dy + dz * dz);
+    dx *= rn; dy *= rn; dz *= rn;
+    float Y[16];
+    sh_basis(f.deg, dx, dy, dz, Y);
+    float r = 0.5f, g = 0.5f, b = 0.5f;
+    if (f.deg == 3) {  // 48 floats = 12 aligned float4 (192 B per Gaussian)
+        const float4* s4 = reinterpret_cast<const float4*>(sh + (size_t)i * 48);
+        float c[48];
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            const float4 v = __ldg(s4 + k);
+            c[4 * k] = v.x; c[4 * k + 1] = v.y; c[4 * k + 2] = v.z; c[4 * k + 3] = v.w;
+        }
+#pragma unroll
+        for (int k = 0; k < 16; k++) {
+            r = fmaf(Y[k], c[3 * k], r); g = fmaf(Y[k], c[3 * k + 1], g); b = fmaf(Y[k], c[3 * k + 2], b);
+        }
+    } else {
+        const float* s = sh + (size_t)i * f.K * 3;
+        for (int k = 0; k < f.K; k++) {
+            r = fmaf(Y[k], __ldg(s + 3 * k), r); g = fmaf(Y[k], __ldg(s + 3 * k + 1), g); b = fmaf(Y[k], __ldg(s + 3 * k + 2), b);
+        }
+    }
+    return make_float3(fmaxf(r, 0.0f), fmaxf(g, 0.0f), fmaxf(b, 0.0f));
+}
+
+// Warp-aggregated atomic add on the difference grid: lanes with equal `cell` elect one leader.
+__device__ __forceinline__ void grid_add(int* diff, bool on, int cell, int val) {
+    const unsigned peers = __match_any_sync(0xffffffffu, on ? cell : -1);
+    if (on && (__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(diff + cell, val * __popc(peers));
+}
+
+__global__ void __launch_bounds__(PRE_THREADS)
+preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ means, const float* __restrict__ scales,
+                  const float* __restrict__ rots, const float* __restrict__ opac, const float* __restrict__ sh) {
+    __shared__ uint32_t s_hist[MAX_SORT_PASSES_DEPTH][256];
+    __shared__ uint32_t s_wcount[PRE_THREADS / 32];
+    __shared__ int s_tile;
+    __shared__ unsigned long long s_base;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    for (int k = tid; k < MAX_SORT_PASSES_DEPTH * 256; k += PRE_THREADS) (&s_hist[0][0])[k] = 0;
+    const int n_tiles = (f.P + PRE_THREADS - 1) / PRE_THREADS;
+    while (true) {
+        __syncthreads();  // s_tile / s_base / s_wcount reuse; also orders the histogram zeroing
+        if (tid == 0) s_tile = (int)atomicAdd(&p.ctrl->tile_counter[TC_PRE], 1u);
+        __syncthreads();
+        const int tile = s_tile;
+        if (tile >= n_tiles) break;
+        const int i = tile * PRE_THREADS + tid;
+        Splat s = {};
+        bool vis = false;
+        float px = 0.f, py = 0.f, pz = 0.f;
+        if (i < f.P) {
+            px = __ldg(means + 3 * (size_t)i); py = __ldg(means + 3 * (size_t)i + 1); pz = __ldg(means + 3 * (size_t)i + 2);
+            const float sx = __ldg(scales + 3 * (size_t)i), sy = __ldg(scales + 3 * (size_t)i + 1), sz = __ldg(scales + 3 * (size_t)i + 2);
+            const float4 q = __ldg(reinterpret_cast<const float4*>(rots) + i);
+            vis = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, s);
+        }
+        // ---- block-level count of visible Gaussians; publish the aggregate early, look back with warp 0 ----
+        const unsigned vb = __ballot_sync(0xffffffffu, vis);
+        if (lane == 0) s_wcount[w] = __popc(vb);
+        __syncthreads();
+        uint32_t wbase = 0, btotal = 0;
+#pragma unroll
+        for (int k = 0; k < PRE_THREADS / 32; k++) {
+            const uint32_t c = s_wcount[k];
+            if (k < w) wbase += c;
+            btotal += c;
+        }
+        if (w == 0) {
+            if (lane == 0) st_status(p.st_pre + tile, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)btotal);
+            unsigned long long excl = 0;
+            if (tile > 0) {
+                excl = lookback_warp(p.st_pre, tile);
+                if (lane == 0) st_status(p.st_pre + tile, ST_INC | (excl + btotal));
+            }
+            if (lane == 0) {
+                s_base = excl;
+                if (tile == n_tiles - 1) p.ctrl->n_vis = excl + btotal;
+            }
+        }
+        // ---- everything that does not need the compact index: per-Gaussian record, colour, grid, histograms ----
+        if (i < f.P) {
+            uint4 pg = make_uint4(0u, 0u, 0u, 0u);
+            if (vis) {
+                pg.x = (uint32_t)s.xmin | ((uint32_t)s.ymin << 16);
+                pg.y = (uint32_t)s.xmax | ((uint32_t)s.ymax << 16);
+                pg.z = __float_as_uint(s.depth);
+                pg.w = (uint32_t)s.radius;
+            }
+            p.per_g[i] = pg;
+        }
+        const int gw = f.gx + 1;
+        grid_add(p.diff, vis, s.ymin * gw + s.xmin, 1);
+        grid_add(p.diff, vis, s.ymin * gw + s.xmax, -1);
+        grid_add(p.diff, vis, s.ymax * gw + s.xmin, -1);
+        grid_add(p.diff, vis, s.ymax * gw + s.xmax, 1);
+        if (vis) {
+            const uint32_t db = __float_as_uint(s.depth);
+            atomicAdd(&s_hist[0][db & 255u], 1u);
+            atomicAdd(&s_hist[1][(db >> 8) & 255u], 1u);
+            atomicAdd(&s_hist[2][(db >> 16) & 255u], 1u);
+            atomicAdd(&s_hist[3][db >> 24], 1u);
+            const float o = __ldg(opac + i);
+            const float3 col = sh_colour(f, sh, i, px, py, pz);
+            // det of the STORED conic, exact products in double (24+24 bits): the form is indefinite iff det <= 0,
+            // and the tight box of the render stage needs det without fp32 cancellation (needle-like splats)
+            const double dd = (double)s.ca * (double)s.cc - (double)s.cb * (double)s.cb;
+            const uint32_t flags = (dd <= 0.0) ? 1u : 0u;
+            p.geom[2 * (size_t)i] = make_float4(s.mux, s.muy, s.ca, s.cb);
+            p.geom[2 * (size_t)i + 1] = make_float4(s.cc, log2f(o), (float)dd, __uint_as_float(flags));
+            p.colour[i] = make_float4(col.x, col.y, col.z, 0.0f);
+        }
+        __syncthreads();  // s_base ready
+        if (vis) {
+            const unsigned long long cidx = s_base + wbase + __popc(vb & ((1u << lane) - 1u));
+            p.gkeyA[cidx] = ((unsigned long long)__float_as_uint(s.depth) << 32) | (unsigned)i;
+        }
+    }
+    __syncthreads();
+    for (int k = tid; k < MAX_SORT_PASSES_DEPTH * 256; k += PRE_THREADS) {
+        const uint32_t c = (&s_hist[0][0])[k];
+        if (c) atomicAdd(&p.ctrl->depth_hist[0][0] + k, c);
+    }
+}
+
+void launch_preprocess(const Frame& f, const Pointers& p, const float* means, const float* scales, const float* rots,
+                       const float* opac, const float* sh, int n_blocks, cudaStream_t st) {
+    preprocess_kernel<<<n_blocks, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh);
+}
+
+}  // namespace gs

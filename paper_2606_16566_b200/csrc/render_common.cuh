@@ -1,0 +1,100 @@
+// render_common.cuh -- device helpers of the render kernels: tile-local hoisting (Eq. 1-10) and the
+// tight box / warp visibility mask (Eq. 13-21).  Product code; shares nothing with oracle/.
+#pragma once
+#include "common.cuh"
+
+namespace gs {
+
+constexpr float LOG2E = 1.4426950408889634f;
+constexpr float LN2 = 0.6931471805599453f;
+constexpr float L2_ALPHA_MIN = -7.994353436858858f;  // log2(1/255): the opacity floor in the log2 domain
+constexpr float ALPHA_MIN = 1.0f / 255.0f;
+constexpr float ALPHA_MAX = 0.99f;
+constexpr float T_MIN = 0.0001f;
+
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Hoist transformation (Eq. 8, reading G2), in the log2 domain:
+//   log2(alpha)(x', y') = A x'^2 + B x'y' + C y'^2 + D x' + E y' + F,   (x', y') relative to the origin (ox, oy),
+//   A = -a k/2, B = -b k, C = -c k/2, D = (a dx + b dy) k, E = (b dx + c dy) k,
+//   F = log2(o) - (a dx^2 + 2 b dx dy + c dy^2) k / 2,   (dx, dy) = mu - origin (Eq. 2),  k = log2(e).
+// Evaluated in double and rounded once: D, E, F are sums of large cancelling terms for far-centred splats
+// (reading S14), and this runs once per (tile, Gaussian), off the per-pixel path.
+struct Hoisted { float A, B, C, D, E, F; };
+__device__ __forceinline__ Hoisted hoist(float mux, float muy, float a, float b, float c, float log2o, float ox, float oy) {
+    const double k = 1.4426950408889634;
+    const double dx = (double)mux - (double)ox, dy = (double)muy - (double)oy;
+    const double da = a, db = b, dc = c;
+    const double gx = da * dx + db * dy, gy = db * dx + dc * dy;
+    Hoisted h;
+    h.A = (float)(-0.5 * k * da);
+    h.B = (float)(-k * db);
+    h.C = (float)(-0.5 * k * dc);
+    h.D = (float)(k * gx);
+    h.E = (float)(k * gy);
+    h.F = (float)((double)log2o - 0.5 * k * (gx * dx + gy * dy));
+    return h;
+}
+
+// Tight box (Eq. 13-19): vertical extent [ymin, ymax] (centre-relative) of the ellipse
+// a x^2 + 2 b x y + c y^2 <= tau restricted to the column x in [x0, x1] (centre-relative, Eq. 14).
+// Returns false when the ellipse misses the column.  det = a c - b^2 > 0 is required.
+__device__ __forceinline__ bool column_span(float a, float b, float c, float det, float tau, float x0, float x1,
+                                            float& ymin, float& ymax) {
+    const float dy = sqrtf(__fdividef(a * tau, det));   // Eq. 16
+    const float ct = c * tau;
+    const float ic = __fdividef(1.0f, c);
+    const float ax0 = a * x0, ax1 = a * x1;
+    // upper branch: peak vertex at x = -b dy / a (division-free test)
+    const float tu = -b * dy;
+    if (tu < ax0 || tu > ax1) {
+        const float xs = (tu < ax0) ? x0 : x1;           // Case A (Eq. 17) / Case B (Eq. 18)
+        const float disc = ct - det * xs * xs;
+        if (disc < 0.0f) return false;
+        ymax = (-b * xs + sqrtf(disc)) * ic;
+    } else {
+        ymax = dy;                                       // Case C
+    }
+    // lower branch: "identical conditional logic with reversed signs for the linear terms"
+    const float tl = b * dy;
+    if (tl < ax0 || tl > ax1) {
+        const float xs = (tl < ax0) ? x0 : x1;
+        const float disc = ct - det * xs * xs;
+        if (disc < 0.0f) return false;
+        ymin = (-b * xs - sqrtf(disc)) * ic;
+    } else {
+        ymin = -dy;
+    }
+    return true;
+}
+
+// Threshold of the alpha >= 1/255 ellipse, tau = 2 ln(255 o), from log2(o), widened so that fp32
+// rounding in column_span can never cull a contributing pixel (any conservative mask is correct; S13).
+__device__ __forceinline__ float tau_widened(float log2o) {
+    const float tau = 2.0f * LN2 * (log2o - L2_ALPHA_MIN);
+    return tau + 0.02f + 1e-5f * fabsf(tau);
+}
+constexpr float SPAN_EPS = 2e-3f;  // widening of the vertical span, pixels
+
+// Rows [r0, r1] (tile-local, clamped to [0, 15]) of the tile column [ox + cx0, ox + cx1] that the ellipse can reach;
+// r0 > r1 when empty.  (mux, muy) - (ox, oy) = centre relative to the tile corner.
+__device__ __forceinline__ void column_rows(float dxc, float dyc, float a, float b, float c, float det, float tau,
+                                            float cx0, float cx1, int& r0, int& r1) {
+    float ymin, ymax;
+    r0 = 1; r1 = 0;
+    if (!(det > 0.0f) || !(a > 0.0f) || !(c > 0.0f)) { r0 = 0; r1 = 15; return; }  // degenerate conic: keep everything
+    if (!column_span(a, b, c, det, tau, cx0 - dxc, cx1 - dxc, ymin, ymax)) return;
+    const float lo = ceilf(dyc + ymin - SPAN_EPS), hi = floorf(dyc + ymax + SPAN_EPS);  // Eq. 19 + ceil/floor
+    if (!(lo <= hi)) {  // NaN-safe: a NaN keeps everything
+        if (lo != lo || hi != hi) { r0 = 0; r1 = 15; }
+        return;
+    }
+    r0 = (int)fmaxf(lo, 0.0f);
+    r1 = (int)fminf(hi, 15.0f);
+}
+
+}  // namespace gs

@@ -1,0 +1,122 @@
+"""Parity protocol between the CUDA path (through the C ABI) and the CPU oracle.
+
+1. bit-exact, whole arrays: tiles_touched, radius, rect, depth bits, N_dup, tile counts, tile ranges, sorted id lists;
+2. n_contrib equal on every pixel whose oracle `fragile` flag is 0 (an alpha within delta of 1/255 or a T' within delta
+   of 1e-4 makes a pixel fragile; delta = 1e-3);
+3. image and final_T: |diff| <= 2e-3 on >= 99.9 % of pixels, <= 2/255 on all, and every pixel above 2e-3 is fragile
+   (BASELINE.json north_star).
+Used by tests/test_gpu_parity.py and __graft_entry__.smoke().  Imports the oracle: test infrastructure only.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from oracle import oracle
+from paper_2606_16566_b200 import binding
+from paper_2606_16566_b200.renderer import Renderer
+
+TOL_MOST = 2e-3        # north_star: within 2e-3 absolute on >= 99.9 % of pixels
+TOL_ALL = 2.0 / 255.0  # and within 2/255 on all pixels
+FRAC_MOST = 0.999
+DELTA = 1e-3           # fragile-pixel delta of the parity protocol
+
+
+def run_gpu(scene, cam_index=0, max_dup=None, variant=None, count_contrib=True, device="cuda:0", renderer=None):
+    cam = scene.cameras[cam_index]
+    if max_dup is None:
+        max_dup = 1 << 20
+    if variant is not None:
+        binding.gs_set_render_variant(variant)
+    r = renderer or Renderer(scene.P, cam.W, cam.H, max_dup, device=device, count_contrib=count_contrib)
+    if renderer is None or r.scene is None:
+        r.upload(scene)
+    r.render(cam)
+    torch.cuda.synchronize()
+    return r
+
+
+def run_gpu_auto(scene, cam_index=0, variant=None, count_contrib=True, device="cuda:0", start_dup=1 << 20):
+    """Render, growing the workspace when the frame needs more duplicates than it holds (GS_ERR_OVERFLOW)."""
+    max_dup = start_dup
+    while True:
+        r = run_gpu(scene, cam_index, max_dup, variant, count_contrib, device)
+        try:
+            it = r.intermediates()
+            return r, it
+        except binding.GsError as e:
+            if e.code != binding.GS_ERR_OVERFLOW:
+                raise
+            max_dup = int(e.n_dup * 1.02) + 4096
+            del r
+            torch.cuda.empty_cache()
+
+
+def compare(r, it, ref, check_lists=True, check_pixels=True):
+    """Returns a report dict; raises AssertionError on any violation.  `ref` is an oracle.render() result (possibly a
+    tile subset), `r` a Renderer after render(), `it` its intermediates."""
+    rep = {}
+    # ---- 1. bit-exact integers -----------------------------------------------------------------------------------
+    assert it.P == ref.P and it.n_tiles == ref.n_tiles
+    for name in ("tiles_touched", "radius", "depth_bits"):
+        a, b = getattr(it, name), getattr(ref, name)
+        bad = np.flatnonzero(a != b)
+        assert bad.size == 0, "%s differs for %d Gaussians, first %s: gpu %s oracle %s" % (
+            name, bad.size, bad[:5], a[bad[:5]], b[bad[:5]])
+    bad = np.flatnonzero((it.rect != ref.rect).any(axis=1))
+    assert bad.size == 0, "rect differs for %d Gaussians, first %s" % (bad.size, bad[:5])
+    assert it.n_dup == ref.n_dup, "N_dup gpu %d oracle %d" % (it.n_dup, ref.n_dup)
+    assert it.n_visible == int((ref.tiles_touched > 0).sum())
+    counts = r.out_tile_counts.cpu().numpy().view(np.uint32)
+    assert np.array_equal(counts, ref.tile_counts), "tile counts differ"
+    ranges = it.tile_ranges.astype(np.uint64)
+    assert ranges[0] == 0 and np.array_equal(np.diff(ranges), ref.tile_counts.astype(np.uint64)), "tile ranges differ"
+    rep.update(P=int(it.P), n_visible=int(it.n_visible), n_dup=int(it.n_dup))
+    if check_lists:
+        n_bad = 0
+        for l, t in enumerate(ref.list_tile):
+            a = it.sorted_ids[int(ranges[t]):int(ranges[t + 1])]
+            b = ref.sorted_ids[int(ref.list_offsets[l]):int(ref.list_offsets[l + 1])]
+            if not np.array_equal(a, b):
+                n_bad += 1
+        assert n_bad == 0, "sorted id lists differ in %d of %d tiles" % (n_bad, len(ref.list_tile))
+        rep["lists_checked"] = int(len(ref.list_tile))
+    if not check_pixels:
+        return rep
+    # ---- pixels of rendered tiles ----------------------------------------------------------------------------------
+    H, W, gx = ref.H, ref.W, ref.grid_x
+    tmask = ref.rendered.reshape(ref.grid_y, gx).astype(bool)
+    pmask = np.repeat(np.repeat(tmask, 16, axis=0), 16, axis=1)[:H, :W]
+    img = r.out_rgb.cpu().numpy()
+    fT = r.out_final_T.cpu().numpy()
+    fragile = ref.fragile != 0
+    # ---- 2. contributor counts -------------------------------------------------------------------------------------
+    if r.out_n_contrib is not None:
+        nc = r.out_n_contrib.cpu().numpy().view(np.uint32)
+        diff = (nc != ref.n_contrib) & pmask
+        hard = diff & ~fragile
+        assert hard.sum() == 0, "n_contrib differs on %d NON-fragile pixels, first %s" % (hard.sum(), np.argwhere(hard)[:5])
+        rep["n_contrib_mismatch_fragile"] = int(diff.sum())
+    # ---- 3. image and final T --------------------------------------------------------------------------------------
+    d_img = np.abs(img - ref.image).max(axis=0)
+    d_T = np.abs(fT - ref.final_T)
+    d = np.maximum(d_img, d_T)
+    d = np.where(pmask, d, 0.0)
+    npx = int(pmask.sum())
+    over = d > TOL_MOST
+    assert not np.isnan(img).any() and not np.isnan(fT).any(), "NaN in the output"
+    assert d.max() <= TOL_ALL, "max |diff| %.3g > 2/255 at %s" % (d.max(), np.unravel_index(d.argmax(), d.shape))
+    assert over.sum() <= (1.0 - FRAC_MOST) * npx, "%d of %d pixels above 2e-3" % (over.sum(), npx)
+    assert (over & ~fragile).sum() == 0, "%d NON-fragile pixels above 2e-3" % (over & ~fragile).sum()
+    rep.update(pixels=npx, fragile_share=float((fragile & pmask).sum()) / max(npx, 1), max_abs_diff=float(d.max()),
+               over_2e3=int(over.sum()), p999_abs_diff=float(np.quantile(d[pmask], 0.999)) if npx else 0.0,
+               mean_abs_diff=float(d[pmask].mean()) if npx else 0.0)
+    return rep
+
+
+def oracle_and_compare(scene, cam_index=0, tile_subset=None, n_threads=8, variant=None, count_contrib=True, flags=0):
+    r, it = run_gpu_auto(scene, cam_index, variant=variant, count_contrib=count_contrib)
+    ref = oracle.render(scene, cam_index, tile_subset=tile_subset, n_threads=n_threads, flags=flags, fragile_delta=DELTA)
+    rep = compare(r, it, ref, check_lists=not (flags & oracle.NO_LISTS),
+                  check_pixels=not (flags & (oracle.NO_LISTS | oracle.NO_RENDER)))
+    return rep, r, it, ref

@@ -1,0 +1,228 @@
+"""GPU parity tests: the CUDA path, called through the C ABI (ctypes), against the CPU oracle on the same seeded inputs.
+
+Protocol and tolerances: tests/parity_util.py (BASELINE.json north_star).  Every test needs a B200: `-m gpu`.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle
+from paper_2606_16566_b200 import binding, scenes
+from paper_2606_16566_b200.renderer import Renderer
+
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(autouse=True)
+def _default_variant():
+    binding.gs_set_render_variant(4)
+    yield
+    binding.gs_set_render_variant(4)
+
+
+def _sample_tiles(ref_counts, gx, gy, n, seed):
+    """Tile subset for full-size configs: the longest lists, the image corners/edges, and random tiles."""
+    rng = np.random.default_rng(seed)
+    order = np.argsort(ref_counts)[::-1]
+    pick = list(order[:3]) + [0, gx - 1, (gy - 1) * gx, gy * gx - 1, (gy // 2) * gx + gx // 2]
+    pick += list(rng.choice(gx * gy, size=n, replace=False))
+    return np.unique(np.array(pick, dtype=np.int32))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# config 1 (tiny) -- every render variant of the ablation ladder, whole image
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [4, 3, 2, 1, 0])
+def test_config1_all_variants(variant):
+    sc = scenes.make_scene(1)
+    rep, r, it, ref = pu.oracle_and_compare(sc, 0, variant=variant)
+    assert rep["n_dup"] == ref.n_dup and rep["lists_checked"] == 64
+    print("config1 variant", variant, rep)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# config 2 (object-centric, the bench workload) -- full size, whole image, several poses
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("pose,variant", [(0, 4), (3, 4), (5, 4), (0, 3), (1, 0)])
+def test_config2_full(pose, variant):
+    sc = scenes.make_scene(2)
+    rep, *_ = pu.oracle_and_compare(sc, pose, variant=variant)
+    print("config2 pose", pose, "variant", variant, rep)
+
+
+def test_config2_bench_configuration_without_counts():
+    """bench.py renders without the optional n_contrib output: same image bit for bit, parity holds."""
+    sc = scenes.make_scene(2)
+    r1, it1 = pu.run_gpu_auto(sc, 2, count_contrib=True)
+    r2, it2 = pu.run_gpu_auto(sc, 2, count_contrib=False)
+    assert torch.equal(r1.out_rgb, r2.out_rgb) and torch.equal(r1.out_final_T, r2.out_final_T)
+    ref = oracle.render(sc, 2, n_threads=8, fragile_delta=pu.DELTA)
+    print(pu.compare(r2, it2, ref))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# reduced configs 3-5: same distributions, fewer Gaussians, ragged image sizes (W, H not multiples of 16)
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,P,W,H,f,pose", [
+    (3, 120_000, 637, 419, 500.0, 0),
+    (3, 120_000, 637, 419, 500.0, 7),
+    (4, 60_000, 963, 541, 750.0, 0),
+    (4, 60_000, 963, 541, 750.0, 5),
+    (5, 400_000, 1283, 727, 1000.0, 0),
+    (5, 400_000, 1283, 727, 1000.0, 3),
+])
+def test_reduced_configs(config, P, W, H, f, pose):
+    sc = scenes.make_scene(config, P=P, W=W, H=H, f=f)
+    rep, *_ = pu.oracle_and_compare(sc, pose)
+    print("config", config, "reduced pose", pose, rep)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# full-size configs 3-5 in the launch configuration bench.py uses: all per-Gaussian integers, N_dup, every tile count
+# and range bit-exact; sorted lists and pixels on a sampled subset of tiles the oracle can compute one by one
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,pose,n_tiles", [(3, 0, 24), (5, 0, 16), (4, 0, 4)])
+def test_full_size_sampled_tiles(config, pose, n_tiles):
+    sc = scenes.make_scene(config, poses=max(pose + 1, 2) if config != 4 else 16)
+    cam = sc.cameras[pose]
+    pre = oracle.render(sc, pose, flags=oracle.NO_LISTS)
+    tiles = _sample_tiles(pre.tile_counts, pre.grid_x, pre.grid_y, n_tiles, seed=config)
+    if config == 4:  # every list has > 1e5 entries: keep the sample small
+        tiles = tiles[:6]
+    r, it = pu.run_gpu_auto(sc, pose, start_dup=int(pre.n_dup) + 4096)
+    ref = oracle.render(sc, pose, tile_subset=tiles, n_threads=8, fragile_delta=pu.DELTA)
+    rep = pu.compare(r, it, ref)
+    print("config", config, "FULL pose", pose, "tiles", len(tiles), rep)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# closed-form fixtures on the GPU (DESIGN.md pins T1-T3 applied to the CUDA path)
+# ------------------------------------------------------------------------------------------------------------------
+def test_closed_form_single_gaussian():
+    W = H = 33
+    sc = scenes.single_gaussian_scene([0.0, 0.0, 4.0], [0.1] * 3, [0.5, -0.5, 0.5, 0.5], 0.7, [0.9, 0.5, 0.1],
+                                      [0.2, 0.3, 0.4], W, H, 40.0, 40.0)
+    r, it = pu.run_gpu_auto(sc)
+    img = r.out_rgb.cpu().numpy()
+    fT = r.out_final_T.cpu().numpy()
+    sig2 = (40.0 * 0.1 / 4.0) ** 2 + 0.3
+    yy, xx = np.mgrid[0:H, 0:W]
+    r2 = (xx - 16.0) ** 2 + (yy - 16.0) ** 2
+    a = 0.7 * np.exp(-r2 / (2 * sig2))
+    a = np.where(a < 1.0 / 255.0, 0.0, np.minimum(a, 0.99))
+    inrect = (xx < 32) & (yy < 32)
+    a = np.where(inrect, a, 0.0)
+    near = np.abs(0.7 * np.exp(-r2 / (2 * sig2)) - 1.0 / 255.0) < 1e-5  # exactly-on-threshold pixels: none here
+    assert not near.any()
+    for ch, (c, b) in enumerate(zip([0.9, 0.5, 0.1], [0.2, 0.3, 0.4])):
+        assert np.abs(img[ch] - (b * (1 - a) + c * a)).max() < 2e-5
+    assert np.abs(fT - (1 - a)).max() < 2e-5
+    assert it.radius[0] == 4 and list(it.rect[0]) == [0, 0, 2, 2] and it.n_dup == 4
+
+
+def test_termination_rule_stack():
+    """>= 7 identical centred Gaussians, o = 0.8, equal depth: n_contrib = 5, final T = 3.2e-4 at the centre (R1)."""
+    W = H = 33
+    n = 9
+    sc = scenes.single_gaussian_scene([[0.0, 0.0, 4.0]] * n, [0.2] * 3, [1.0, 0.0, 0.0, 0.0], 0.8, [0.3, 0.6, 0.9],
+                                      [0.0, 0.0, 0.0], W, H, 40.0, 40.0)
+    rep, r, it, ref = pu.oracle_and_compare(sc)
+    assert int(r.out_n_contrib[16, 16]) == 5
+    assert abs(float(r.out_final_T[16, 16]) - 3.2e-4) < 1e-7
+
+
+def test_equal_depth_tie_break_and_order_independence():
+    W = H = 49
+    means = [[0.0, 0.0, 3.0], [0.05, 0.0, 3.0], [0.0, 0.05, 5.0]]
+    cols = [[1.0, 0.0, 0.0], [0.0, 1.0, 0.0], [0.0, 0.0, 1.0]]
+    sc = scenes.single_gaussian_scene(means, [0.3] * 3, [1.0, 0.0, 0.0, 0.0], [0.6, 0.7, 0.8], cols, [0.1] * 3, W, H, 50.0, 50.0)
+    rep, r, it, ref = pu.oracle_and_compare(sc)
+    # ids 0 and 1 share their depth bits: 0 comes first in every list
+    for t in range(it.n_tiles):
+        ids = list(it.sorted_ids[it.tile_ranges[t]:it.tile_ranges[t + 1]])
+        if 0 in ids and 1 in ids:
+            assert ids.index(0) < ids.index(1)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# edge cases
+# ------------------------------------------------------------------------------------------------------------------
+def test_empty_and_all_culled():
+    W, H = 70, 45
+    bg = np.array([0.25, 0.5, 0.75], np.float32)
+    # (a) P = 0
+    sc = scenes.make_scene(1, P=0, W=W, H=H)
+    sc.bg = bg
+    r, it = pu.run_gpu_auto(sc)
+    assert it.n_dup == 0 and it.n_visible == 0
+    assert torch.equal(r.out_final_T, torch.ones_like(r.out_final_T))
+    assert np.array_equal(r.out_rgb.cpu().numpy(), np.broadcast_to(bg[:, None, None], (3, H, W)))
+    assert int(r.out_tile_counts.sum()) == 0 and int(r.out_n_contrib.sum()) == 0
+    # (b) everything behind the camera
+    sc = scenes.make_scene(1, P=500, W=W, H=H)
+    sc.means3D[:, 2] = -sc.means3D[:, 2]
+    sc.bg = bg
+    rep, r, it, ref = pu.oracle_and_compare(sc)
+    assert it.n_dup == 0 and torch.equal(r.out_final_T, torch.ones_like(r.out_final_T))
+
+
+def test_workspace_overflow_is_reported_and_safe():
+    sc = scenes.make_scene(1)
+    cam = sc.cameras[0]
+    r = pu.run_gpu(sc, 0, max_dup=1000)  # the frame needs 5 436 entries
+    with pytest.raises(binding.GsError) as ei:
+        r.intermediates()
+    assert ei.value.code == binding.GS_ERR_OVERFLOW and ei.value.n_dup == oracle.render(sc, flags=oracle.NO_LISTS).n_dup
+    assert torch.equal(r.out_final_T, torch.ones_like(r.out_final_T))  # every list treated as empty
+    # too small for even max_dup = 0
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda:0")
+    with pytest.raises(binding.GsError) as ei:
+        binding.gs_render(r.scene["means3D"], r.scene["scales"], r.scene["rotations"], r.scene["opacities"], r.scene["sh"], 0,
+                          cam.viewmatrix, cam.projmatrix, cam.fx, cam.fy, cam.W, cam.H, sc.bg, r.out_rgb, r.out_final_T,
+                          r.out_tile_counts, r.out_n_contrib, small)
+    assert ei.value.code == binding.GS_ERR_WORKSPACE
+    with pytest.raises(binding.GsError) as ei:
+        binding.gs_render(r.scene["means3D"], r.scene["scales"], r.scene["rotations"], r.scene["opacities"], r.scene["sh"], 7,
+                          cam.viewmatrix, cam.projmatrix, cam.fx, cam.fy, cam.W, cam.H, sc.bg, r.out_rgb, r.out_final_T,
+                          r.out_tile_counts, r.out_n_contrib, r.workspace)
+    assert ei.value.code == binding.GS_ERR_BAD_ARG
+
+
+def test_deterministic_and_reusable_workspace():
+    sc = scenes.make_scene(2, P=30_000, W=400, H=300, f=500.0)
+    r, it = pu.run_gpu_auto(sc, 0)
+    a = (r.out_rgb.clone(), r.out_final_T.clone(), r.out_n_contrib.clone(), it.sorted_ids.copy())
+    for pose in (1, 0):
+        r.render(sc.cameras[pose])
+    torch.cuda.synchronize()
+    it2 = r.intermediates()
+    assert torch.equal(a[0], r.out_rgb) and torch.equal(a[1], r.out_final_T) and torch.equal(a[2], r.out_n_contrib)
+    assert np.array_equal(a[3], it2.sorted_ids)
+
+
+def test_sh_degrees_and_colour_tolerance():
+    """SH degrees 0..3 through the CUDA preprocess: colours within 1e-5 of the oracle's double evaluation."""
+    for deg in (0, 1, 2, 3):
+        sc = scenes.make_scene(2, P=5_000, W=256, H=192, f=300.0, sh_degree=deg)
+        r, it = pu.run_gpu_auto(sc, 1)
+        full = r.intermediates(copy=("per_gaussian", "geom", "tile_ranges", "sorted_ids"))
+        ref = oracle.render(sc, 1, n_threads=8, fragile_delta=pu.DELTA)
+        vis = ref.tiles_touched > 0
+        assert np.abs(full.colour[vis, :3] - ref.rgb[vis]).max() < 1e-5
+        assert np.array_equal(full.geom[vis, 0:2].view(np.uint32), ref.mu[vis].view(np.uint32))      # mu bit-exact
+        assert np.array_equal(full.geom[vis, 2:5].view(np.uint32), ref.conic[vis].view(np.uint32))  # conic bit-exact
+        pu.compare(r, it, ref)
+
+
+def test_per_stage_timings_and_launch_count():
+    sc = scenes.make_scene(1)
+    binding.gs_set_timing(True)
+    try:
+        r = pu.run_gpu(sc, 0)
+        t = binding.gs_get_timings(r.workspace)
+    finally:
+        binding.gs_set_timing(False)
+    assert set(t) == set(binding.TIMING_NAMES) and all(v >= 0 for v in t.values()) and t["frame"] > 0
+    assert binding.gs_last_launch_count() >= 8

@@ -1,0 +1,385 @@
+#!/usr/bin/env python
+"""bench.py -- frames/sec of the forward 3DGS render (BASELINE.json `metric`) on synthetic scenes, 1 line of JSON.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+A STEP is one pass of the whole hot path (preprocess -> duplication + sort -> render) over every
+camera pose of the configuration: `poses` frames.  Default workload: BASELINE.json configs[1] (object-centric,
+100 000 Gaussians, 800x800, SH degree 3, 8 poses) -- the configuration the metric is quoted on that fits one GPU.
+`value` = frames/s with the scene resident in HBM, device-timed (CUDA events on the launching stream, one pair per
+frame, L2 flushed before every frame, max over ranks).  `e2e` = the same metric through the public API with HOST
+buffers: every step copies the scene host->device from pinned memory, renders every pose and copies every image back.
+N > 1 runs N independent replicas (replicas only; no data-path collective).
+
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on the same workload: one pose per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "frames/sec (fwd render)"
+UNIT = "frames/s"
+FP32_LANES_PER_SM = 128          # FP32 FMA lanes per SM per clock (mb probe: FFMA 3.8-4.0 warp-instr/clk/SM)
+INSTR_PER_PAIR = 14              # FP32-pipe thread-instructions per evaluated (pixel, Gaussian) pair
+L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and clock-event reasons through NVML while the timed region runs."""
+
+    def __init__(self, torch_index: int, period_s: float = 0.005):
+        super().__init__(daemon=True)
+        self.period, self.samples, self.reasons, self.stop_flag = period_s, [], set(), False
+        self.h, self.sm_max, self.nv = None, None, None
+        try:
+            import pynvml as nv
+            import torch
+            nv.nvmlInit()
+            self.nv = nv
+            try:
+                uuid = str(torch.cuda.get_device_properties(torch_index).uuid)
+                self.h = nv.nvmlDeviceGetHandleByUUID(("GPU-" + uuid) if not uuid.startswith("GPU-") else uuid)
+            except Exception:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+                idx = int(vis.split(",")[torch_index]) if vis and vis.split(",")[torch_index].isdigit() else torch_index
+                self.h = nv.nvmlDeviceGetHandleByIndex(idx)
+            self.sm_max = int(nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM))
+        except Exception as e:  # NVML unavailable: report it, never fake numbers
+            self.err = repr(e)
+
+    NAMES = (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4),
+             ("hw_power_brake_slowdown", 0x80), ("sync_boost", 0x10), ("applications_clocks_setting", 0x2))
+
+    def run(self):
+        if self.h is None:
+            return
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for name, bit in self.NAMES:
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def result(self):
+        self.stop_flag = True
+        if self.h is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "error": getattr(self, "err", "nvml unavailable")}
+        self.join(timeout=1.0)
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def _dist():
+    ws = int(os.environ.get("WORLD_SIZE", "1"))
+    return ws, int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0"))
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on the host cores
+# ----------------------------------------------------------------------------------------------------------------
+def run_reference(args):
+    ws, rank, _ = _dist()
+    if rank != 0:
+        return 0
+    from oracle import oracle
+    from paper_2606_16566_b200 import scenes
+    cfg = scenes.config_defaults(args.config)
+    sc = scenes.make_scene(args.config)
+    cores = os.cpu_count() or 1
+    n_pose = len(sc.cameras)
+    k = 0
+    for _ in range(args.warmup):
+        oracle.render(sc, k % n_pose, n_threads=cores)
+        k += 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.render(sc, k % n_pose, n_threads=cores)
+        k += 1
+    dt = time.perf_counter() - t0
+    fps = args.steps / dt
+    sample = "1 frame (one camera pose, cycling over the %d poses) of config %d per step, oracle tile-parallel on %d threads" % (
+        n_pose, args.config, cores)
+    line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64 blend / f32 preprocess (CPU oracle)", "data": "synthetic",
+            "config": _config_dict(args.config, cfg, sc, extra={"frames_per_step": 1}),
+            "cpu_baseline": {"value": fps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": fps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def _config_dict(config, cfg, sc, extra=None):
+    d = {"workload": "BASELINE.json configs[%d]: %s, %d Gaussians, %dx%d, f=%g, SH degree %d, %d poses, 16x16 tiles, seed %d" % (
+        config - 1, cfg["name"], sc.P, cfg["W"], cfg["H"], cfg["f"], sc.sh_degree, len(sc.cameras), config - 1),
+         "gaussians": sc.P, "width": cfg["W"], "height": cfg["H"], "sh_degree": sc.sh_degree, "poses": len(sc.cameras)}
+    if extra:
+        d.update(extra)
+    return d
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# our arm: the CUDA path through the C ABI
+# ----------------------------------------------------------------------------------------------------------------
+def _stage_bytes(P, K_sh, n_vis, n_dup, n_tile_passes):
+    """Algorithmic HBM bytes per frame of the memory-bound stages."""
+    return {
+        "preprocess": P * 40 + n_vis * (4 + 12 * K_sh) + P * 16 + n_vis * 56,
+        "depth_sort": 4 * 16 * n_vis,
+        "offset_scan": n_vis * (8 + 16 + 4),
+        "duplicate": n_vis * 28 + n_dup * 8,
+        "tile_sort": (n_tile_passes - 1) * 16 * n_dup + 12 * n_dup,
+    }
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2606_16566_b200 import binding, scenes
+    from paper_2606_16566_b200.renderer import Renderer
+
+    ws, rank, lrank = _dist()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(lrank)
+    dev = torch.device("cuda", lrank)
+    if ws > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    binding.lib()  # raises if libgs.so is missing and cannot be built
+    peaks = _peaks()
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+
+    cfg = scenes.config_defaults(args.config)
+    sc = scenes.make_scene(args.config)
+    cams = sc.cameras
+    n_pose = len(cams)
+    W, H = cfg["W"], cfg["H"]
+
+    def barrier():
+        if ws > 1:
+            dist.barrier()
+
+    def rank_max(x):
+        if ws == 1:
+            return float(x)
+        t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- size the workspace: largest N_dup over the poses (+5 %) -----------------------------------------------------
+    max_dup, need = 1 << 22, 0
+    r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True)
+    r.upload(sc)
+    per_pose = []
+    for cam in cams:
+        r.render(cam, count_contrib=False)
+        try:
+            it = r.intermediates(copy=())
+            need = max(need, it.n_dup)
+            per_pose.append((it.n_visible, it.n_dup))
+        except binding.GsError as e:
+            if e.code != binding.GS_ERR_OVERFLOW:
+                raise
+            need = max(need, e.n_dup)
+            per_pose.append(None)
+    if need > max_dup or any(p is None for p in per_pose):
+        del r
+        torch.cuda.empty_cache()
+        max_dup = int(need * 1.05) + 4096
+        r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True)
+        r.upload(sc)
+    # ---- statistics pass (untimed): units of the rooflines -------------------------------------------------------------
+    binding.gs_set_stats(True)
+    stats, per_pose = [], []
+    for cam in cams:
+        r.render(cam, count_contrib=True)
+        stats.append(binding.gs_get_stats(r.workspace))
+        it = r.intermediates(copy=())
+        per_pose.append((it.n_visible, it.n_dup))
+    binding.gs_set_stats(False)
+    launches_per_frame = binding.gs_last_launch_count()
+    mean = lambda xs: float(sum(xs)) / max(len(xs), 1)
+    pairs_eval = mean([s["pairs_evaluated"] for s in stats])
+    pairs_blend = mean([s["pairs_blended"] for s in stats])
+    staged = mean([s["entries_staged"] for s in stats])
+    n_vis_m, n_dup_m = mean([p[0] for p in per_pose]), mean([p[1] for p in per_pose])
+
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+
+    def frame(cam, e0=None, e1=None):
+        flush.zero_()                       # L2 flush before every frame (outside the event pair)
+        if e0 is not None:
+            e0.record()
+        r.render(cam, count_contrib=False)
+        if e1 is not None:
+            e1.record()
+
+    # ---- pre-warm (clock ramp) + W warm-up steps -------------------------------------------------------------------------
+    t0 = time.perf_counter()
+    while time.perf_counter() - t0 < 0.5:
+        for cam in cams:
+            frame(cam)
+        torch.cuda.synchronize()
+    for _ in range(args.warmup):
+        for cam in cams:
+            frame(cam)
+    # ---- timed region: exactly K steps ---------------------------------------------------------------------------------------
+    K = args.steps
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K * n_pose)]
+    sampler = ClockSampler(lrank)
+    barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    wall0 = time.perf_counter()
+    launches = 0
+    for s in range(K):
+        for i, cam in enumerate(cams):
+            e0, e1 = evs[s * n_pose + i]
+            frame(cam, e0, e1)
+            launches += launches_per_frame
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.result()
+    barrier()
+    dev_ms = sum(e0.elapsed_time(e1) for e0, e1 in evs)
+    dev_ms = rank_max(dev_ms)
+    ms_per_step = dev_ms / K
+    fps = ws * n_pose * K / (dev_ms * 1e-3)
+
+    # ---- per-stage device times: a second pass with the library's own CUDA events between its kernels -----------
+    binding.gs_set_timing(True)
+    acc = {n: 0.0 for n in binding.TIMING_NAMES}
+    n_t = 0
+    for s in range(min(K, 20)):
+        for cam in cams:
+            flush.zero_()
+            r.render(cam, count_contrib=False)
+            t = binding.gs_get_timings(r.workspace)
+            for n in acc:
+                acc[n] += t[n]
+            n_t += 1
+    binding.gs_set_timing(False)
+    stage_ms = {n: acc[n] / n_t for n in acc}
+
+    # ---- e2e: host buffers in, host images out, every step ----------------------------------------------------------------
+    def e2e_step():
+        h2d = r.upload(sc)
+        for i, cam in enumerate(cams):
+            r.render(cam, count_contrib=False)
+            r.read_image(i, n_pose)
+        torch.cuda.synchronize()
+        return h2d
+    for _ in range(2):
+        h2d_bytes = e2e_step()
+    barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        e2e_step()
+    e2e_s = rank_max(time.perf_counter() - t0)
+    h2d_bytes += n_pose * (16 + 16 + 3) * 4
+    d2h_bytes = n_pose * 3 * H * W * 4
+    e2e_fps = ws * n_pose * K / e2e_s
+
+    # ---- rooflines ---------------------------------------------------------------------------------------------------------------------
+    alu_peak = n_sm * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12       # T thread-instr/s
+    render_s = stage_ms["render"] * 1e-3
+    achieved = pairs_eval * INSTR_PER_PAIR / render_s / 1e12
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get("config%d" % args.config, {}).get("render_dram_bytes_per_launch")
+    roofline = {"kernel": "render_b200_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+                "unit": "T FP32-pipe thread-instr/s", "frac": achieved / alu_peak, "traffic": traffic,
+                "peak_source": "derived: %d SMs x %d FP32 lanes x %.0f MHz (max SM clock)" % (n_sm, FP32_LANES_PER_SM, peaks["sm_max_mhz"]),
+                "units_per_launch": {"pairs_evaluated": pairs_eval, "instr_per_pair": INSTR_PER_PAIR,
+                                     "pairs_blended": pairs_blend, "entries_staged": staged},
+                "ms_per_launch": stage_ms["render"]}
+    n_tile_passes = (max(1, (((W + 15) // 16) * ((H + 15) // 16) - 1).bit_length()) + 7) // 8
+    sb = _stage_bytes(sc.P, (sc.sh_degree + 1) ** 2, n_vis_m, n_dup_m, n_tile_passes)
+    kernels = []
+    for n in ("preprocess", "depth_sort", "tile_grid", "offset_scan", "duplicate", "tile_sort", "render"):
+        k = {"stage": n, "ms": stage_ms[n], "share": stage_ms[n] / max(stage_ms["frame"], 1e-9)}
+        if n in sb:
+            gbs = sb[n] / (stage_ms[n] * 1e-3) / 1e9 if stage_ms[n] > 0 else 0.0
+            k.update(bound="hbm", achieved=gbs, peak=peaks["hbm_gbs"], unit="GB/s", frac=gbs / peaks["hbm_gbs"],
+                     algorithmic_bytes=sb[n])
+        elif n == "render":
+            k.update(bound="alu", frac=roofline["frac"])
+        kernels.append(k)
+
+    cpu_baseline = None
+    if rank == 0 and ws == 1 and not args.no_cpu_baseline:
+        from oracle import oracle
+        cores = os.cpu_count() or 1
+        t0 = time.perf_counter()
+        nf = 0
+        while nf < 2 * n_pose and (time.perf_counter() - t0 < 8.0 or nf == 0):
+            oracle.render(sc, nf % n_pose, n_threads=cores)
+            nf += 1
+        dt = time.perf_counter() - t0
+        cpu_baseline = {"value": nf / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": "%d frames (poses 0..%d cycling) of the same workload, oracle tile-parallel on %d threads, %.1f s" % (
+                            nf, min(nf, n_pose) - 1, cores, dt)}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": args.warmup,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": _config_dict(args.config, cfg, sc, extra={
+                    "frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every frame", "parallelism": "replicas x%d" % ws,
+                    "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "render_variant": binding.gs_get_render_variant()}),
+                "ms_per_frame": ms_per_step / n_pose, "wall_ms_per_step_incl_flush": 1e3 * wall / K,
+                "clocks": clocks,
+                "e2e": {"value": e2e_fps, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes},
+                "gpu_launches": launches, "launches_per_frame": launches_per_frame,
+                "roofline": roofline, "kernels": kernels, "stage_ms_per_frame": stage_ms,
+                "cpu_baseline": cpu_baseline, "peaks": peaks}
+        print(json.dumps(line))
+    if ws > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, choices=(1, 2, 3, 4, 5))
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -98,6 +98,18 @@ int gs_get_timings(const void* workspace, float ms[GS_N_TIMINGS]);
 int gs_set_render_variant(int variant);
 int gs_get_render_variant(void);
 
+/* Render statistics (render variant 4 with out_n_contrib != NULL only; off by default, process-wide).  With
+ * gs_set_stats(1) the render kernel counts what its blend loop did and gs_get_stats() (which synchronises the
+ * stream of the last call on `workspace`) returns
+ *   [0] (warp, Gaussian) slots walked by the blend loop (after the warp cull of PAPER.md Sec. III-C, before Eq. 22 exit)
+ *   [1] (pixel, Gaussian) pairs blended = sum of out_n_contrib
+ *   [2] (tile, Gaussian) entries staged into shared memory (Sec. III-B5)
+ *   [3] (pixel, Gaussian) pairs whose alpha was evaluated = 64 x [0]
+ * These are the units of the render roofline in bench.py. */
+#define GS_N_STATS 4
+int gs_set_stats(int enable);
+int gs_get_stats(const void* workspace, uint64_t out[GS_N_STATS]);
+
 /* Number of kernel launches (ours; memsets not counted) enqueued by the last gs_render() in this process. */
 int gs_last_launch_count(void);
 

@@ -23,7 +23,9 @@ TIMING_NAMES = ("preprocess", "depth_sort", "tile_grid", "offset_scan", "duplica
 
 EXPORTS = ("gs_workspace_bytes", "gs_render", "gs_get_intermediates", "gs_set_timing", "gs_get_timings",
            "gs_set_render_variant", "gs_get_render_variant", "gs_last_launch_count", "gs_error_string",
-           "gs_last_cuda_error", "gs_copy_to_host")
+           "gs_last_cuda_error", "gs_copy_to_host", "gs_set_stats", "gs_get_stats")
+GS_N_STATS = 4
+STATS_NAMES = ("warp_slots_walked", "pairs_blended", "entries_staged", "pairs_evaluated")
 
 
 class _Intermediates(C.Structure):
@@ -72,6 +74,10 @@ def lib():
         L.gs_error_string.restype = C.c_char_p
         L.gs_error_string.argtypes = [C.c_int]
         L.gs_last_cuda_error.restype = C.c_int
+        L.gs_set_stats.restype = C.c_int
+        L.gs_set_stats.argtypes = [C.c_int]
+        L.gs_get_stats.restype = C.c_int
+        L.gs_get_stats.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.gs_copy_to_host.restype = C.c_int
         L.gs_copy_to_host.argtypes = [vp, vp, C.c_size_t]
         _lib = L
@@ -179,6 +185,18 @@ def gs_get_timings(workspace) -> dict:
     if rc != GS_OK:
         raise GsError(rc, "gs_get_timings")
     return dict(zip(TIMING_NAMES, [float(x) for x in ms]))
+
+
+def gs_set_stats(enable: bool) -> None:
+    lib().gs_set_stats(1 if enable else 0)
+
+
+def gs_get_stats(workspace) -> dict:
+    out = (C.c_uint64 * GS_N_STATS)()
+    rc = lib().gs_get_stats(C.c_void_p(workspace.data_ptr()), out)
+    if rc != GS_OK:
+        raise GsError(rc, "gs_get_stats")
+    return dict(zip(STATS_NAMES, [int(x) for x in out]))
 
 
 def gs_set_render_variant(variant: int) -> None:

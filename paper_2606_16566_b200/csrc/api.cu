@@ -16,7 +16,7 @@ void launch_tile_grid(const Frame&, const Pointers&, uint32_t*, cudaStream_t, in
 void launch_scan_offsets(const Frame&, const Pointers&, int, cudaStream_t, int*);
 void launch_duplicate_and_tile_sort(const Frame&, const Pointers&, int, cudaStream_t, int*, cudaEvent_t);
 void launch_render_ladder(int, const Frame&, const Pointers&, float*, float*, uint32_t*, cudaStream_t);
-void launch_render_b200(const Frame&, const Pointers&, float*, float*, uint32_t*, int, cudaStream_t);
+void launch_render_b200(const Frame&, const Pointers&, float*, float*, uint32_t*, int, bool, cudaStream_t);
 }  // namespace gs
 
 namespace {
@@ -81,7 +81,7 @@ struct LastCall {
 
 std::mutex g_mu;
 std::map<const void*, LastCall> g_calls;
-std::atomic<int> g_variant{4}, g_timing{0}, g_launches{0}, g_cuda_err{0};
+std::atomic<int> g_variant{4}, g_timing{0}, g_stats{0}, g_launches{0}, g_cuda_err{0};
 int g_n_sm = 0;
 
 int cuda_fail(cudaError_t e) {
@@ -208,7 +208,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     launch_duplicate_and_tile_sort(f, p, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b)
     mark(6);
     const int variant = g_variant.load();                      // (4) render
-    if (variant >= 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, st);
+    if (variant >= 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
     else launch_render_ladder(variant, f, p, out_rgb, out_final_T, out_n_contrib, st);
     launches++;
     mark(7);
@@ -273,6 +273,32 @@ int gs_get_timings(const void* workspace, float ms[GS_N_TIMINGS]) {
     for (int k = 0; k < 7; k++)
         if ((e = cudaEventElapsedTime(&ms[k], lc.ev[k], lc.ev[k + 1])) != cudaSuccess) return cuda_fail(e);
     if ((e = cudaEventElapsedTime(&ms[7], lc.ev[0], lc.ev[7])) != cudaSuccess) return cuda_fail(e);
+    return GS_OK;
+}
+
+int gs_set_stats(int enable) {
+    g_stats.store(enable ? 1 : 0);
+    return GS_OK;
+}
+
+int gs_get_stats(const void* workspace, uint64_t out[GS_N_STATS]) {
+    if (!workspace || !out) return GS_ERR_BAD_ARG;
+    LastCall lc;
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        auto it = g_calls.find(workspace);
+        if (it == g_calls.end() || !it->second.valid) return GS_ERR_BAD_ARG;
+        lc = it->second;
+    }
+    cudaError_t e = cudaStreamSynchronize(lc.stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    Ctrl c;
+    e = cudaMemcpy(&c, static_cast<const char*>(workspace) + lc.L.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(e);
+    out[0] = c.stats[0];
+    out[1] = c.stats[1];
+    out[2] = c.stats[2];
+    out[3] = c.stats[0] * 64ull;  // every walked (warp, Gaussian) slot evaluates the warp's 8x8 pixels
     return GS_OK;
 }
 

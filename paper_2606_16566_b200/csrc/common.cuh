@@ -30,6 +30,7 @@ struct Ctrl {
     unsigned long long n_dup_eff;       // duplicates actually produced (0 on overflow)
     uint32_t depth_hist[MAX_SORT_PASSES_DEPTH][256];  // global digit histograms of the depth bits (atomics)
     uint32_t tile_hist[MAX_SORT_PASSES_TILE][256];    // global digit histograms of the tile ids (from tile counts)
+    unsigned long long stats[4];        // render statistics (gs_set_stats): warp slots walked, pairs blended, entries staged
 };
 enum { TC_PRE = 0, TC_DEPTH0 = 1, TC_SCAN = 5, TC_TILE0 = 6 };
 

@@ -93,9 +93,9 @@ __device__ __forceinline__ bool blend_step(PixelPair& s, const float4 q0, const 
     return all_done;
 }
 
-template <bool COUNT>
+template <bool COUNT, bool STATS>
 __global__ void __launch_bounds__(QB)
-render_b200_kernel(const Frame f, const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ ids,
+render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ ids,
                    const float4* __restrict__ geom, const float4* __restrict__ colour, float* __restrict__ out_rgb,
                    float* __restrict__ out_T, uint32_t* __restrict__ out_n) {
     __shared__ float4 s_q0[QB];       // A, B, C, F
@@ -130,6 +130,7 @@ render_b200_kernel(const Frame f, const uint32_t* __restrict__ ranges, const uin
     const uint32_t start = ranges[tile], end = ranges[tile + 1];
     const unsigned lt = (1u << lane) - 1u;
     int parity = 0;
+    uint32_t st_walk = 0, st_staged = 0;  // STATS only
     for (uint32_t base = start; base < end; base += QB, parity ^= 1) {
         if (tid == 0) s_flag[parity] = 0;
         if (__syncthreads_and(wdone)) break;  // every warp of the tile is finished
@@ -138,6 +139,7 @@ render_b200_kernel(const Frame f, const uint32_t* __restrict__ ranges, const uin
         float4 g0 = make_float4(0.f, 0.f, 0.f, 0.f), g1 = g0;
         uint32_t id = 0;
         const uint32_t k = base + tid;
+        if (STATS && tid == 0) st_staged += min((uint32_t)QB, end - base);
         if (k < end) {
             id = ids[k];
             g0 = __ldg(geom + 2 * (size_t)id);
@@ -182,15 +184,27 @@ render_b200_kernel(const Frame f, const uint32_t* __restrict__ ranges, const uin
             if (s_flag[parity] == 0) {
                 for (int i = 0; i < cnt; i++) {
                     const int j = list[i];
+                    if (STATS) st_walk++;
                     if (blend_step<COUNT, false>(s, s_q0[j], s_q1[j], s_cb[j], 0.0f)) { wdone = true; break; }
                 }
             } else {
                 for (int i = 0; i < cnt; i++) {
                     const int j = list[i];
+                    if (STATS) st_walk++;
                     if (blend_step<COUNT, true>(s, s_q0[j], s_q1[j], s_cb[j], s_guard[j])) { wdone = true; break; }
                 }
             }
         }
+    }
+    if (STATS) {  // gs_set_stats(1): what the blend loop actually did (bench.py roofline)
+        uint32_t nb = s.n0 + s.n1;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nb += __shfl_xor_sync(0xffffffffu, nb, o);
+        if (lane == 0) {
+            atomicAdd(&ctrl->stats[0], (unsigned long long)st_walk);
+            atomicAdd(&ctrl->stats[1], (unsigned long long)nb);
+        }
+        if (tid == 0) atomicAdd(&ctrl->stats[2], (unsigned long long)st_staged);
     }
     // ---- epilogue: out = C + T bg (reading S16) -------------------------------------------------------------------
     float T0, T1, r0, r1, g0_, g1_, b0_, b1_;
@@ -213,11 +227,15 @@ render_b200_kernel(const Frame f, const uint32_t* __restrict__ ranges, const uin
 }
 
 void launch_render_b200(const Frame& f, const Pointers& p, float* out_rgb, float* out_T, uint32_t* out_n, int n_sm,
-                        cudaStream_t st) {
+                        bool stats, cudaStream_t st) {
     (void)n_sm;
     const dim3 grid(f.gx, f.gy), block(QB);
-    if (out_n) render_b200_kernel<true><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.geom, p.colour, out_rgb, out_T, out_n);
-    else render_b200_kernel<false><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.geom, p.colour, out_rgb, out_T, nullptr);
+    if (stats && out_n)
+        render_b200_kernel<true, true><<<grid, block, 0, st>>>(f, p.ctrl, p.ranges, p.ids, p.geom, p.colour, out_rgb, out_T, out_n);
+    else if (out_n)
+        render_b200_kernel<true, false><<<grid, block, 0, st>>>(f, p.ctrl, p.ranges, p.ids, p.geom, p.colour, out_rgb, out_T, out_n);
+    else
+        render_b200_kernel<false, false><<<grid, block, 0, st>>>(f, p.ctrl, p.ranges, p.ids, p.geom, p.colour, out_rgb, out_T, nullptr);
 }
 
 }  // namespace gs

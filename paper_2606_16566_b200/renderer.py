@@ -10,6 +10,8 @@ import torch
 
 from . import binding
 
+_SCENE_ARRAYS = ("means3D", "scales", "rotations", "opacities", "sh")
+
 
 class Renderer:
     def __init__(self, P: int, W: int, H: int, max_dup: int, device="cuda:0", count_contrib: bool = True):
@@ -24,21 +26,37 @@ class Renderer:
         self.out_tile_counts = torch.empty((self.gy * self.gx,), dtype=torch.int32, device=self.device)
         self.out_n_contrib = torch.empty((H, W), dtype=torch.int32, device=self.device) if count_contrib else None
         self.scene = None
+        self._pinned = None   # host staging of the scene arrays (pinned), allocated on the first upload
+        self._host_rgb = None
 
-    def upload(self, scene) -> None:
-        """Host (numpy) scene -> device tensors (pinned staging, async copies on the current stream)."""
-        def up(a):
-            t = torch.from_numpy(np.ascontiguousarray(a))
-            return t.pin_memory().to(self.device, non_blocking=True)
-        self.scene = dict(means3D=up(scene.means3D), scales=up(scene.scales), rotations=up(scene.rotations),
-                          opacities=up(scene.opacities), sh=up(scene.sh), sh_degree=int(scene.sh_degree),
-                          bg=np.asarray(scene.bg, dtype=np.float32))
+    def upload(self, scene) -> int:
+        """Host (numpy) scene -> device tensors: pinned staging, async copies on the current stream.  The staging and
+        device buffers are allocated on the first call and reused.  Returns the bytes copied host -> device."""
+        if self._pinned is None:
+            self._pinned = {n: torch.from_numpy(np.array(getattr(scene, n), dtype=np.float32, order="C")).pin_memory()
+                            for n in _SCENE_ARRAYS}
+            dev = {n: torch.empty_like(t, device=self.device) for n, t in self._pinned.items()}
+            self.scene = dict(dev, sh_degree=int(scene.sh_degree), bg=np.array(scene.bg, dtype=np.float32))
+        nbytes = 0
+        for n in _SCENE_ARRAYS:
+            self.scene[n].copy_(self._pinned[n], non_blocking=True)
+            nbytes += self._pinned[n].numel() * 4
+        return nbytes
 
-    def render(self, cam, stream=None) -> None:
+    def render(self, cam, stream=None, count_contrib: bool = True) -> None:
         s = self.scene
         binding.gs_render(s["means3D"], s["scales"], s["rotations"], s["opacities"], s["sh"], s["sh_degree"],
                           cam.viewmatrix, cam.projmatrix, cam.fx, cam.fy, cam.W, cam.H, s["bg"], self.out_rgb,
-                          self.out_final_T, self.out_tile_counts, self.out_n_contrib, self.workspace, stream)
+                          self.out_final_T, self.out_tile_counts, self.out_n_contrib if count_contrib else None,
+                          self.workspace, stream)
+
+    def read_image(self, slot: int = 0, n_slots: int = 1) -> torch.Tensor:
+        """Async device -> pinned-host copy of the last frame's RGB image into host slot `slot`; returns the host
+        tensor (valid after the stream is synchronised)."""
+        if self._host_rgb is None or self._host_rgb.shape[0] < n_slots:
+            self._host_rgb = torch.empty((n_slots, 3, self.H, self.W), dtype=torch.float32).pin_memory()
+        self._host_rgb[slot].copy_(self.out_rgb, non_blocking=True)
+        return self._host_rgb[slot]
 
     def intermediates(self, copy=("per_gaussian", "tile_ranges", "sorted_ids")):
         return binding.gs_get_intermediates(self.workspace, copy)

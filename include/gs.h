@@ -70,9 +70,12 @@ typedef struct gs_intermediates {
     uint64_t max_dup;              /* capacity of this workspace                                                  */
     const uint32_t* per_gaussian;  /* dev [P,4] u32: {xmin | ymin<<16, xmax | ymax<<16, depth bits, radius};
                                       rect in tiles, half-open; all zero for a culled Gaussian                   */
-    const float* geom;             /* dev [P,8]: mu_x, mu_y, conic a, b, c, log2(opacity), a*c-b*b, flags(bits);
-                                      defined only where tiles_touched > 0                                       */
-    const float* colour;           /* dev [P,4]: r, g, b, 0 (SH colour clamped at 0); defined where visible      */
+    const float* record;           /* dev [P,16], the 64-byte render record, defined only where tiles_touched > 0:
+                                      [0..1] mu_x, mu_y (pixels)   [2..4] conic a, b, c (Eq. 5)
+                                      [5] log2(opacity)   [6] a*c-b*b   [7] flags (bits; 1 = degenerate conic)
+                                      [8..10] r, g, b (SH colour clamped at 0)
+                                      [11] x*  [12] 1/c  [13] c*tau: per-Gaussian constants of the tight box
+                                      (Eq. 13-18; tau = 2 ln(255 o) widened)   [14..15] 0                        */
     const uint64_t* depth_sorted;  /* dev [n_visible]: (depth bits << 32 | Gaussian id), ascending, stable       */
     const uint32_t* dup_offsets;   /* dev [n_visible]: exclusive prefix sum of tiles_touched in depth order      */
     const uint32_t* tile_ranges;   /* dev [n_tiles+1]: list of tile t is sorted_ids[tile_ranges[t] .. [t+1])     */

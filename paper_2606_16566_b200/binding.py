@@ -31,7 +31,7 @@ STATS_NAMES = ("warp_slots_walked", "pairs_blended", "entries_staged", "pairs_ev
 class _Intermediates(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("P", "W", "H", "grid_x", "grid_y", "n_tiles")] + [
         ("n_visible", C.c_uint32), ("n_dup", C.c_uint64), ("max_dup", C.c_uint64),
-        ("per_gaussian", C.c_void_p), ("geom", C.c_void_p), ("colour", C.c_void_p), ("depth_sorted", C.c_void_p),
+        ("per_gaussian", C.c_void_p), ("record", C.c_void_p), ("depth_sorted", C.c_void_p),
         ("dup_offsets", C.c_void_p), ("tile_ranges", C.c_void_p), ("sorted_ids", C.c_void_p)]
 
 
@@ -163,8 +163,9 @@ def gs_get_intermediates(workspace, copy=("per_gaussian", "tile_ranges", "sorted
         out.radius = pg[:, 3].astype(np.int32)
         out.tiles_touched = ((out.rect[:, 2] - out.rect[:, 0]) * (out.rect[:, 3] - out.rect[:, 1])).astype(np.uint32)
     if "geom" in copy:
-        out.geom = _copy_out(it.geom, 8 * it.P, np.float32, dev).reshape(it.P, 8)
-        out.colour = _copy_out(it.colour, 4 * it.P, np.float32, dev).reshape(it.P, 4)
+        out.record = _copy_out(it.record, 16 * it.P, np.float32, dev).reshape(it.P, 16)
+        out.geom = out.record[:, 0:8]
+        out.colour = out.record[:, 8:12]
     if "depth_sorted" in copy:
         out.depth_sorted = _copy_out(it.depth_sorted, it.n_visible, np.uint64, dev)
         out.dup_offsets = _copy_out(it.dup_offsets, it.n_visible, np.uint32, dev)

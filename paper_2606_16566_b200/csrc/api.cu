@@ -27,7 +27,7 @@ size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
     size_t ctrl, diff, st_pre, st_scan, st_depth, st_tile, zero_end;
-    size_t per_g, geom, colour, gkeyA, gkeyB, dup_off, chunk_start, ranges, entA, entB, ids, total;
+    size_t per_g, rec, gkeyA, gkeyB, dup_off, chunk_start, ranges, entA, entB, ids, total;
     size_t n_depth_tiles, n_tile_tiles;
     int gx, gy, n_tiles, tile_bits, n_tile_passes;
 };
@@ -55,8 +55,7 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     L.st_tile = take(8 * 256 * L.n_tile_tiles * (size_t)L.n_tile_passes);
     L.zero_end = o;
     L.per_g = take(16 * Pz);
-    L.geom = take(32 * Pz);
-    L.colour = take(16 * Pz);
+    L.rec = take(64 * Pz);
     L.gkeyA = take(8 * Pz);
     L.gkeyB = take(8 * Pz);
     L.dup_off = take(4 * Pz);
@@ -99,8 +98,7 @@ Pointers carve(void* ws, const Layout& L) {
     p.st_depth = reinterpret_cast<unsigned long long*>(b + L.st_depth);
     p.st_tile = reinterpret_cast<unsigned long long*>(b + L.st_tile);
     p.per_g = reinterpret_cast<uint4*>(b + L.per_g);
-    p.geom = reinterpret_cast<float4*>(b + L.geom);
-    p.colour = reinterpret_cast<float4*>(b + L.colour);
+    p.rec = reinterpret_cast<float4*>(b + L.rec);
     p.gkeyA = reinterpret_cast<unsigned long long*>(b + L.gkeyA);
     p.gkeyB = reinterpret_cast<unsigned long long*>(b + L.gkeyB);
     p.dup_off = reinterpret_cast<uint32_t*>(b + L.dup_off);
@@ -243,8 +241,7 @@ int gs_get_intermediates(const void* workspace, gs_intermediates* out) {
     out->n_dup = c.n_dup;
     out->max_dup = lc.max_dup;
     out->per_gaussian = reinterpret_cast<const uint32_t*>(p.per_g);
-    out->geom = reinterpret_cast<const float*>(p.geom);
-    out->colour = reinterpret_cast<const float*>(p.colour);
+    out->record = reinterpret_cast<const float*>(p.rec);
     out->depth_sorted = reinterpret_cast<const uint64_t*>(p.gkeyA);
     out->dup_offsets = p.dup_off;
     out->tile_ranges = p.ranges;

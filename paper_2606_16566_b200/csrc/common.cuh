@@ -58,8 +58,7 @@ struct Pointers {           // device pointers carved from the workspace
     unsigned long long* st_depth;           // [4][depth sort tiles][256]
     unsigned long long* st_tile;            // [3][tile sort tiles][256]
     uint4* per_g;                           // [P] {rect01, rect23, depth bits, radius}
-    float4* geom;                           // [P][2]
-    float4* colour;                         // [P]
+    float4* rec;                            // [P][4] 64-byte render record (layout: include/gs.h, gs_intermediates.record)
     unsigned long long* gkeyA;              // [P] (depth bits << 32 | id), compacted
     unsigned long long* gkeyB;              // [P] ping-pong
     uint32_t* dup_off;                      // [P] exclusive prefix of tiles_touched in depth order

@@ -9,7 +9,7 @@
 // (__fmul_rn/__fadd_rn/__fsub_rn/__fdiv_rn/__fsqrt_rn are never contracted into FMAs and ignore -use_fast_math),
 // so depth bits, radius, rect and tiles_touched are unique integers any conforming implementation reproduces.
 // C-P9 (SH colour) is free-order fp32 (a toleranced output).
-#include "common.cuh"
+#include "render_common.cuh"
 
 namespace gs {
 
@@ -254,10 +254,14 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             // det of the STORED conic, exact products in double (24+24 bits): the form is indefinite iff det <= 0,
             // and the tight box of the render stage needs det without fp32 cancellation (needle-like splats)
             const double dd = (double)s.ca * (double)s.cc - (double)s.cb * (double)s.cb;
-            const uint32_t flags = (dd <= 0.0) ? 1u : 0u;
-            p.geom[2 * (size_t)i] = make_float4(s.mux, s.muy, s.ca, s.cb);
-            p.geom[2 * (size_t)i + 1] = make_float4(s.cc, log2f(o), (float)dd, __uint_as_float(flags));
-            p.colour[i] = make_float4(col.x, col.y, col.z, 0.0f);
+            const float l2o = log2f(o);
+            const TightBox tb = tight_box_constants(s.ca, s.cb, s.cc, (float)dd, l2o);
+            const uint32_t flags = (!(dd > 0.0) || tb.degenerate) ? 1u : 0u;
+            float4* rec = p.rec + 4 * (size_t)i;  // 64-byte render record (include/gs.h: gs_intermediates.record)
+            rec[0] = make_float4(s.mux, s.muy, s.ca, s.cb);
+            rec[1] = make_float4(s.cc, l2o, (float)dd, __uint_as_float(flags));
+            rec[2] = make_float4(col.x, col.y, col.z, tb.xstar);
+            rec[3] = make_float4(tb.ic, tb.ct, 0.0f, 0.0f);
         }
         __syncthreads();  // s_base ready
         if (vis) {

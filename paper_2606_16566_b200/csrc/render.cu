@@ -15,7 +15,7 @@ constexpr int RB = 256;  // batch = block size
 template <int VAR>
 __global__ void __launch_bounds__(256)
 render_ladder_kernel(const Frame f, const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ ids,
-                     const float4* __restrict__ geom, const float4* __restrict__ colour, float* __restrict__ out_rgb,
+                     const float4* __restrict__ rec, float* __restrict__ out_rgb,
                      float* __restrict__ out_T, uint32_t* __restrict__ out_n) {
     constexpr bool HOIST = VAR >= 1, CULL = VAR >= 2, COHERENT = VAR >= 3;
     // staged batch: HOIST ? (A,B,C,F) : (mux,muy,a,b) ; HOIST ? (D,E,guard,-) : (c,o,-,-)
@@ -43,8 +43,8 @@ render_ladder_kernel(const Frame f, const uint32_t* __restrict__ ranges, const u
             const uint32_t k = base + tid;
             if (k < end) {
                 const uint32_t id = ids[k];
-                const float4 g0 = __ldg(geom + 2 * (size_t)id), g1 = __ldg(geom + 2 * (size_t)id + 1);
-                s_col[tid] = __ldg(colour + id);
+                const float4 g0 = __ldg(rec + 4 * (size_t)id), g1 = __ldg(rec + 4 * (size_t)id + 1);
+                s_col[tid] = __ldg(rec + 4 * (size_t)id + 2);
                 const bool indefinite = __float_as_uint(g1.w) & 1u;
                 if (HOIST) {
                     const Hoisted h = hoist(g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, (float)Tx, (float)Ty);
@@ -142,10 +142,10 @@ void launch_render_ladder(int variant, const Frame& f, const Pointers& p, float*
                           cudaStream_t st) {
     const dim3 grid(f.gx, f.gy), block(256);
     switch (variant) {
-        case 0: render_ladder_kernel<0><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.geom, p.colour, out_rgb, out_T, out_n); break;
-        case 1: render_ladder_kernel<1><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.geom, p.colour, out_rgb, out_T, out_n); break;
-        case 2: render_ladder_kernel<2><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.geom, p.colour, out_rgb, out_T, out_n); break;
-        default: render_ladder_kernel<3><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.geom, p.colour, out_rgb, out_T, out_n); break;
+        case 0: render_ladder_kernel<0><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n); break;
+        case 1: render_ladder_kernel<1><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n); break;
+        case 2: render_ladder_kernel<2><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n); break;
+        default: render_ladder_kernel<3><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n); break;
     }
 }
 

@@ -25,10 +25,17 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // Evaluated in double and rounded once: D, E, F are sums of large cancelling terms for far-centred splats
 // (reading S14), and this runs once per (tile, Gaussian), off the per-pixel path.
 struct Hoisted { float A, B, C, D, E, F; };
-__device__ __forceinline__ Hoisted hoist(float mux, float muy, float a, float b, float c, float log2o, float ox, float oy) {
+// exact fp32 -> fp64 conversion (plain cvt: under -use_fast_math a C++ cast first flushes denormals with an FMUL)
+__device__ __forceinline__ double f2d(float x) {
+    double d;
+    asm("cvt.f64.f32 %0, %1;" : "=d"(d) : "f"(x));
+    return d;
+}
+__device__ __forceinline__ Hoisted hoist(float mux, float muy, float a, float b, float c, float log2o, float ox, float oy,
+                                         float bias = 0.0f) {
     const double k = 1.4426950408889634;
-    const double dx = (double)mux - (double)ox, dy = (double)muy - (double)oy;
-    const double da = a, db = b, dc = c;
+    const double dx = f2d(mux) - f2d(ox), dy = f2d(muy) - f2d(oy);
+    const double da = f2d(a), db = f2d(b), dc = f2d(c);
     const double gx = da * dx + db * dy, gy = db * dx + dc * dy;
     Hoisted h;
     h.A = (float)(-0.5 * k * da);
@@ -36,7 +43,7 @@ __device__ __forceinline__ Hoisted hoist(float mux, float muy, float a, float b,
     h.C = (float)(-0.5 * k * dc);
     h.D = (float)(k * gx);
     h.E = (float)(k * gy);
-    h.F = (float)((double)log2o - 0.5 * k * (gx * dx + gy * dy));
+    h.F = (float)((f2d(log2o) + (double)bias) - 0.5 * k * (gx * dx + gy * dy));
     return h;
 }
 
@@ -79,6 +86,47 @@ __device__ __forceinline__ float tau_widened(float log2o) {
     return tau + 0.02f + 1e-5f * fabsf(tau);
 }
 constexpr float SPAN_EPS = 2e-3f;  // widening of the vertical span, pixels
+
+// ---- B200 staging: the same tight box (Eq. 13-19), branch-free, with its per-Gaussian part hoisted into preprocess ----
+// Per Gaussian (once per frame, preprocess.cu): the vertex abscissa of the upper boundary x* = -b d_y / a
+// (Eq. 16 + PAPER.md:198), 1/c and c tau.  Per (tile, Gaussian) (render_b200.cu): Cases A/B/C of Eq. 17-18 collapse to
+// x_s = clamp(+-x*, x0, x1) because the upper boundary y(x) = (-b x + sqrt(c tau - det x^2)) / c is concave with its
+// maximum at x* (the lower one convex with its minimum at -x*); the column misses the ellipse iff c tau - det x_s^2 < 0.
+struct TightBox { float xstar, ic, ct; bool degenerate; };
+__device__ __forceinline__ TightBox tight_box_constants(float a, float b, float c, float det, float log2o) {
+    TightBox t;
+    const float tau = tau_widened(log2o);
+    t.degenerate = !(det > 0.0f) || !(a > 0.0f) || !(c > 0.0f);
+    const float dy = sqrtf(a * tau / det);        // Eq. 16
+    t.xstar = -b * dy / a;
+    t.ic = 1.0f / c;
+    t.ct = c * tau;
+    if (!(tau > 0.0f)) { t.xstar = 0.0f; t.ct = -1.0f; }  // o <= 1/255: never visible (reading S13)
+    if (!(fabsf(t.xstar) <= 3.0e38f) || !(fabsf(t.ic) <= 3.0e38f) || !(fabsf(t.ct) <= 3.0e38f)) t.degenerate = true;
+    return t;
+}
+
+// 4-bit quadrant mask of one (tile, Gaussian): bit (col + 2 band) is set when the alpha >= 1/255 ellipse can reach a
+// pixel of the 8x8 quadrant (columns 8 col .. 8 col + 7, rows 8 band .. 8 band + 7) -- Eq. 19-21 with 8-row bands,
+// evaluated for the two 8-pixel sub-columns.  (dxc, dyc) = centre relative to the tile corner.  Conservative by the
+// widening of tau and SPAN_EPS; a row band is hit iff an INTEGER row lies in [ymin, ymax] (PAPER.md:216 ceil/floor).
+__device__ __forceinline__ uint32_t quadrant_mask(float dxc, float dyc, float b, float det, float xstar, float ic, float ct) {
+    uint32_t m = 0;
+#pragma unroll
+    for (int col = 0; col < 2; col++) {
+        const float x0 = 8.0f * col - dxc, x1 = x0 + 7.0f;      // Eq. 14, centre-relative
+        const float xu = fminf(fmaxf(xstar, x0), x1), xl = fminf(fmaxf(-xstar, x0), x1);
+        const float du = fmaf(-det * xu, xu, ct), dl = fmaf(-det * xl, xl, ct);
+        const float ymax = fmaf(fmaf(-b, xu, sqrtf(fmaxf(du, 0.0f))), ic, dyc + SPAN_EPS);   // Eq. 17 / 18 / Case C
+        const float ymin = fmaf(fmaf(-b, xl, -sqrtf(fmaxf(dl, 0.0f))), ic, dyc - SPAN_EPS);
+        // misses (du or dl < 0) are folded into the comparison operands, so the whole test is straight-line selects
+        const float top = (fminf(du, dl) >= 0.0f) ? ymax : -1.0f;
+        const uint32_t h0 = floorf(fminf(top, 7.0f)) >= fmaxf(ymin, 0.0f) ? 1u : 0u;
+        const uint32_t h1 = floorf(fminf(top, 15.0f)) >= fmaxf(ymin, 8.0f) ? 4u : 0u;
+        m |= (h0 | h1) << col;
+    }
+    return m;
+}
 
 // Rows [r0, r1] (tile-local, clamped to [0, 15]) of the tile column [ox + cx0, ox + cx1] that the ellipse can reach;
 // r0 > r1 when empty.  (mux, muy) - (ox, oy) = centre relative to the tile corner.

@@ -116,6 +116,14 @@ int gs_get_stats(const void* workspace, uint64_t out[GS_N_STATS]);
 /* Number of kernel launches (ours; memsets not counted) enqueued by the last gs_render() in this process. */
 int gs_last_launch_count(void);
 
+/* Device self-test of the one undocumented hardware property the radix sort relies on (csrc/binning.cu,
+ * radix_pass_kernel): the lanes of one warp-wide shared-memory atomicAdd that hit the same address are served in
+ * ascending lane order, and a thread's atomics in program order, so the returned values are stable ranks.  Runs
+ * `iters` iterations x 8 atomics per thread over 7 digit distributions on the current device (synchronous; uses 16
+ * bytes of private device scratch).  out[0] = atomics whose returned value differed from the stable rank (must be
+ * 0), out[1] = atomics checked. */
+int gs_selftest_atomic_order(int iters, uint64_t out[2]);
+
 /* Synchronous device->host copy of `bytes` bytes (a plain cudaMemcpy) -- lets a binding without CUDA runtime access
  * read the arrays gs_get_intermediates() points at. */
 int gs_copy_to_host(void* dst_host, const void* src_dev, size_t bytes);

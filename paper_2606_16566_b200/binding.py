@@ -23,7 +23,7 @@ TIMING_NAMES = ("preprocess", "depth_sort", "tile_grid", "offset_scan", "duplica
 
 EXPORTS = ("gs_workspace_bytes", "gs_render", "gs_get_intermediates", "gs_set_timing", "gs_get_timings",
            "gs_set_render_variant", "gs_get_render_variant", "gs_last_launch_count", "gs_error_string",
-           "gs_last_cuda_error", "gs_copy_to_host", "gs_set_stats", "gs_get_stats")
+           "gs_last_cuda_error", "gs_copy_to_host", "gs_set_stats", "gs_get_stats", "gs_selftest_atomic_order")
 GS_N_STATS = 4
 STATS_NAMES = ("warp_slots_walked", "pairs_blended", "entries_staged", "pairs_evaluated")
 
@@ -80,6 +80,8 @@ def lib():
         L.gs_get_stats.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.gs_copy_to_host.restype = C.c_int
         L.gs_copy_to_host.argtypes = [vp, vp, C.c_size_t]
+        L.gs_selftest_atomic_order.restype = C.c_int
+        L.gs_selftest_atomic_order.argtypes = [C.c_int, C.POINTER(C.c_uint64)]
         _lib = L
     return _lib
 
@@ -198,6 +200,14 @@ def gs_get_stats(workspace) -> dict:
     if rc != GS_OK:
         raise GsError(rc, "gs_get_stats")
     return dict(zip(STATS_NAMES, [int(x) for x in out]))
+
+
+def gs_selftest_atomic_order(iters: int = 50) -> dict:
+    out = (C.c_uint64 * 2)()
+    rc = lib().gs_selftest_atomic_order(int(iters), out)
+    if rc != GS_OK:
+        raise GsError(rc, "gs_selftest_atomic_order")
+    return {"violations": int(out[0]), "atomics_checked": int(out[1])}
 
 
 def gs_set_render_variant(variant: int) -> None:

@@ -3,6 +3,7 @@
 #include "../../include/gs.h"
 
 #include <atomic>
+#include <cstdio>
 #include <map>
 #include <mutex>
 
@@ -15,6 +16,7 @@ void launch_depth_sort(const Frame&, const Pointers&, int, cudaStream_t, int*);
 void launch_tile_grid(const Frame&, const Pointers&, uint32_t*, cudaStream_t, int*);
 void launch_scan_offsets(const Frame&, const Pointers&, int, cudaStream_t, int*);
 void launch_duplicate_and_tile_sort(const Frame&, const Pointers&, int, cudaStream_t, int*, cudaEvent_t);
+void launch_atomic_order_selftest(unsigned long long*, int, uint32_t, int, int, cudaStream_t);
 void launch_render_ladder(int, const Frame&, const Pointers&, float*, float*, uint32_t*, cudaStream_t);
 void launch_render_b200(const Frame&, const Pointers&, float*, float*, uint32_t*, int, bool, cudaStream_t);
 }  // namespace gs
@@ -27,7 +29,7 @@ size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
     size_t ctrl, diff, st_pre, st_scan, st_depth, st_tile, zero_end;
-    size_t per_g, rec, gkeyA, gkeyB, dup_off, chunk_start, ranges, entA, entB, ids, total;
+    size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, entA, entB, ids, total;
     size_t n_depth_tiles, n_tile_tiles;
     int gx, gy, n_tiles, tile_bits, n_tile_passes;
 };
@@ -43,14 +45,15 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     while ((1ll << L.tile_bits) < nt) L.tile_bits++;
     L.n_tile_passes = (L.tile_bits + 7) / 8;
     const size_t Pz = (size_t)P;
-    L.n_depth_tiles = (Pz + SORT_TILE - 1) / SORT_TILE + 1;
-    L.n_tile_tiles = ((size_t)max_dup + SORT_TILE - 1) / SORT_TILE + 1;
+    const size_t depth_tile = (size_t)SORT_THREADS * sort_items_for(Pz), ent_tile = (size_t)SORT_THREADS * sort_items_for(max_dup);
+    L.n_depth_tiles = (Pz + depth_tile - 1) / depth_tile + 1;
+    L.n_tile_tiles = ((size_t)max_dup + ent_tile - 1) / ent_tile + 1;
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o = up(o + bytes); return at; };
     L.ctrl = take(sizeof(Ctrl));
     L.diff = take(sizeof(int) * (size_t)(L.gx + 1) * (L.gy + 1));
-    L.st_pre = take(8 * ((Pz + PRE_THREADS - 1) / PRE_THREADS + 1));
-    L.st_scan = take(8 * ((Pz + SCAN_TILE - 1) / SCAN_TILE + 1));
+    L.st_pre = take(8 * ((Pz + 31) / 32 + 1));
+    L.st_scan = take(8 * ((Pz + SCAN_WARP_TILE - 1) / SCAN_WARP_TILE + 1));
     L.st_depth = take(8 * 256 * L.n_depth_tiles * MAX_SORT_PASSES_DEPTH);
     L.st_tile = take(8 * 256 * L.n_tile_tiles * (size_t)L.n_tile_passes);
     L.zero_end = o;
@@ -59,6 +62,7 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     L.gkeyA = take(8 * Pz);
     L.gkeyB = take(8 * Pz);
     L.dup_off = take(4 * Pz);
+    L.rk_rect = take(8 * Pz);
     L.chunk_start = take(4 * (((size_t)max_dup + DUP_TILE - 1) / DUP_TILE + 2));
     L.ranges = take(4 * ((size_t)L.n_tiles + 1));
     L.entA = take(8 * (size_t)max_dup);
@@ -76,6 +80,8 @@ struct LastCall {
     bool valid = false, timed = false;
     cudaEvent_t ev[GS_N_TIMINGS + 2] = {};
     bool have_events = false;
+    cudaStream_t side = nullptr;          // tile-grid kernel runs here, concurrently with the depth sort
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
 std::mutex g_mu;
@@ -102,6 +108,7 @@ Pointers carve(void* ws, const Layout& L) {
     p.gkeyA = reinterpret_cast<unsigned long long*>(b + L.gkeyA);
     p.gkeyB = reinterpret_cast<unsigned long long*>(b + L.gkeyB);
     p.dup_off = reinterpret_cast<uint32_t*>(b + L.dup_off);
+    p.rk_rect = reinterpret_cast<uint2*>(b + L.rk_rect);
     p.chunk_start = reinterpret_cast<uint32_t*>(b + L.chunk_start);
     p.ranges = reinterpret_cast<uint32_t*>(b + L.ranges);
     p.entA = reinterpret_cast<unsigned long long*>(b + L.entA);
@@ -112,18 +119,27 @@ Pointers carve(void* ws, const Layout& L) {
     return p;
 }
 
-// largest max_dup whose layout fits into `bytes` (layout size is monotone in max_dup); false if even 0 does not fit
+// largest max_dup whose layout fits into `bytes`; false if even 0 does not fit.  The layout size is monotone in
+// max_dup inside each tile-size regime of sort_items_for() but drops at the regime boundary (larger sort tiles need
+// fewer look-back status words), so the regimes are searched separately, the upper one first.
 bool fit_max_dup(int P, int W, int H, size_t bytes, unsigned long long& max_dup) {
     Layout L;
     if (!make_layout(P, W, H, 0, L) || L.total > bytes) return false;
-    unsigned long long lo = 0, hi = (1ull << 32) - 1;
-    while (lo < hi) {
-        const unsigned long long mid = lo + (hi - lo + 1) / 2;
-        make_layout(P, W, H, mid, L);
-        if (L.total <= bytes) lo = mid; else hi = mid - 1;
+    const unsigned long long edge = 4ull << 20;  // sort_items_for: capacity <= edge -> small tiles
+    const unsigned long long lo_of[2] = {edge + 1, 0}, hi_of[2] = {(1ull << 32) - 1, edge};
+    for (int r = 0; r < 2; r++) {
+        unsigned long long lo = lo_of[r], hi = hi_of[r];
+        make_layout(P, W, H, lo, L);
+        if (L.total > bytes) continue;
+        while (lo < hi) {
+            const unsigned long long mid = lo + (hi - lo + 1) / 2;
+            make_layout(P, W, H, mid, L);
+            if (L.total <= bytes) lo = mid; else hi = mid - 1;
+        }
+        max_dup = lo;
+        return true;
     }
-    max_dup = lo;
-    return true;
+    return false;
 }
 
 }  // namespace
@@ -183,23 +199,45 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
             if (cudaEventCreate(&e) != cudaSuccess) return cuda_fail(cudaGetLastError());
         lc->have_events = true;
     }
+    if (!lc->side) {
+        if (cudaStreamCreateWithFlags(&lc->side, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&lc->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&lc->ev_join, cudaEventDisableTiming) != cudaSuccess)
+            return cuda_fail(cudaGetLastError());
+    }
     lc->L = L; lc->f = f; lc->max_dup = max_dup; lc->stream = st; lc->valid = true; lc->timed = timed;
+#ifdef GS_DEBUG_SYNC   // development builds only: synchronise and report after every stage (never defined in libgs.so)
+    auto mark = [&](int k) {
+        const cudaError_t de = cudaStreamSynchronize(st);
+        fprintf(stderr, "[gs debug] stage %d done: %s\n", k, cudaGetErrorString(de));
+        if (timed) cudaEventRecord(lc->ev[k], st);
+    };
+#else
     auto mark = [&](int k) { if (timed) cudaEventRecord(lc->ev[k], st); };
+#endif
 
     int launches = 0;
     mark(0);
     cudaError_t e = cudaMemsetAsync(workspace, 0, L.zero_end, st);
     if (e != cudaSuccess) return cuda_fail(e);
     {   // (1) preprocess + compaction + depth histograms + coverage grid
-        const long long tiles = ((long long)P + PRE_THREADS - 1) / PRE_THREADS;
-        const int grid = (int)(tiles < 1 ? 1 : (tiles < (long long)g_n_sm * 8 ? tiles : (long long)g_n_sm * 8));
-        launch_preprocess(f, p, means3D, scales, rotations, opacities, sh_coeffs, grid, st);
+        launch_preprocess(f, p, means3D, scales, rotations, opacities, sh_coeffs, g_n_sm, st);
         launches++;
     }
     mark(1);
+    // The tile grid (counts, ranges, N_dup, tile-digit histograms) depends on the preprocess only: it runs on a side
+    // stream, concurrently with the depth sort (fork / join with two events).  With timing enabled the stages are
+    // serialised on the caller's stream so that every per-stage time is that stage alone.
+    if (!timed) {
+        cudaEventRecord(lc->ev_fork, st);
+        cudaStreamWaitEvent(lc->side, lc->ev_fork, 0);
+        launch_tile_grid(f, p, out_tile_counts, lc->side, &launches);
+        cudaEventRecord(lc->ev_join, lc->side);
+    }
     launch_depth_sort(f, p, g_n_sm, st, &launches);          // (3a) LSD passes over the depth bits, pre-duplication
     mark(2);
-    launch_tile_grid(f, p, out_tile_counts, st, &launches);   // tile counts, ranges, N_dup, tile-digit histograms
+    if (timed) launch_tile_grid(f, p, out_tile_counts, st, &launches);
+    else cudaStreamWaitEvent(st, lc->ev_join, 0);
     mark(3);
     launch_scan_offsets(f, p, g_n_sm, st, &launches);         // (2) prefix-sum offsets
     mark(4);
@@ -296,6 +334,30 @@ int gs_get_stats(const void* workspace, uint64_t out[GS_N_STATS]) {
     out[1] = c.stats[1];
     out[2] = c.stats[2];
     out[3] = c.stats[0] * 64ull;  // every walked (warp, Gaussian) slot evaluates the warp's 8x8 pixels
+    return GS_OK;
+}
+
+int gs_selftest_atomic_order(int iters, uint64_t out[2]) {
+    if (iters <= 0 || !out) return GS_ERR_BAD_ARG;
+    int dev = 0, n_sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    unsigned long long* d = nullptr;   // 16 bytes of private scratch, freed before returning
+    if ((e = cudaMalloc(&d, 16)) != cudaSuccess) return cuda_fail(e);
+    e = cudaMemset(d, 0, 16);
+    const int bins[7] = {1, 2, 3, 7, 16, 64, 256};
+    for (int k = 0; k < 7 && e == cudaSuccess; k++) {
+        launch_atomic_order_selftest(d, iters, 12345u + (uint32_t)bins[k], bins[k], n_sm, nullptr);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    unsigned long long h[2] = {0, 0};
+    if (e == cudaSuccess) e = cudaMemcpy(h, d, 16, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(e);
+    out[0] = h[0];
+    out[1] = h[1];
     return GS_OK;
 }
 

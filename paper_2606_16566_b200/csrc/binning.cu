@@ -19,17 +19,28 @@ namespace gs {
 // ------------------------------------------------------------------------------------------------------------
 // One stable radix pass over u64 elements on digit (key >> shift) & 255.  No payload: the id lives in the low
 // 32 bits of the element.  OUT32: write only the low 32 bits (last tile pass -> sorted_ids).
+//
+// Ranking.  Keys are loaded warp-striped (lane l of warp w holds elements w*32*ITEMS + j*32 + l, j = 0..ITEMS-1), so
+// the input order inside a warp is (round j, lane).  The stable rank of a key among the warp's keys of equal digit
+// is the value returned by ONE shared-memory atomicAdd on the warp's private digit counter: the ITEMS atomics of a
+// thread are issued in program order, and the lanes of one warp-wide ATOMS that hit the same address are served in
+// ascending lane order.  The second property is how sm_100 hardware resolves the conflict, not a documented PTX
+// guarantee: it is asserted on the device by gs_selftest_atomic_order() (tests/test_gpu_parity.py runs it) and
+// every list-parity test would expose a violation.  Why not match.any: measured on B200 it costs ~400 cycles of
+// latency and ~40-70 cycles of issue per warp instruction (emulated), against ~2 cycles for the atomic
+// (profiles/r01_microbench.md) -- the match-based first version of this kernel spent 35 % of its stall samples there.
 // ------------------------------------------------------------------------------------------------------------
-template <bool OUT32>
-__global__ void __launch_bounds__(SORT_THREADS)
+template <int ITEMS, bool OUT32>
+__global__ void __launch_bounds__(SORT_THREADS, (ITEMS >= 16 ? 4 : 6))
 radix_pass_kernel(const unsigned long long* __restrict__ in, unsigned long long* __restrict__ out,
                   uint32_t* __restrict__ out32, const unsigned long long* __restrict__ n_ptr, int shift,
                   const uint32_t* __restrict__ ghist, unsigned long long* __restrict__ status,
                   uint32_t* __restrict__ tile_counter) {
     constexpr int NW = SORT_THREADS / 32;
-    __shared__ unsigned long long s_sorted[SORT_TILE];
-    __shared__ uint32_t s_hist[NW][257];
-    __shared__ uint32_t s_bpos[257];
+    constexpr int TILE_N = SORT_THREADS * ITEMS;
+    __shared__ unsigned long long s_sorted[TILE_N];
+    __shared__ uint32_t s_hist[NW][256];
+    __shared__ uint32_t s_bpos[256];
     __shared__ uint32_t s_gbase[256];
     __shared__ uint32_t s_gpos[256];
     __shared__ uint32_t s_scan[NW];
@@ -40,40 +51,42 @@ radix_pass_kernel(const unsigned long long* __restrict__ in, unsigned long long*
         uint32_t tot;
         s_gbase[tid] = block_excl_scan_256(ghist[tid], s_scan, tot);
     }
-    const unsigned lt_mask = (1u << lane) - 1u;
     while (true) {
         __syncthreads();
         if (tid == 0) s_tile = (int)atomicAdd(tile_counter, 1u);
+#pragma unroll
+        for (int k = 0; k < 8; k++) s_hist[w][k * 32 + lane] = 0;
         __syncthreads();
         const int tile = s_tile;
-        const unsigned long long tile_base = (unsigned long long)tile * SORT_TILE;
+        const unsigned long long tile_base = (unsigned long long)tile * TILE_N;
         if (tile_base >= n) break;
-        const uint32_t tile_n = (uint32_t)min((unsigned long long)SORT_TILE, n - tile_base);
-        // ---- load (warp-striped: lane l of warp w takes w*512 + j*32 + l) ---------------------------------
-        unsigned long long key[SORT_ITEMS];
-        uint32_t rk[SORT_ITEMS];
+        const uint32_t tile_n = (uint32_t)min((unsigned long long)TILE_N, n - tile_base);
+        // ---- load (warp-striped) and rank: one shared atomic per key ---------------------------------------
+        unsigned long long key[ITEMS];
+        uint32_t rk2[ITEMS / 2];  // two 16-bit ranks per register (a warp holds 32 * ITEMS <= 512 keys)
+        const uint32_t wbase = w * (32 * ITEMS) + lane;
+        if (tile_n == TILE_N) {
 #pragma unroll
-        for (int j = 0; j < SORT_ITEMS; j++) {
-            const uint32_t li = w * (32 * SORT_ITEMS) + j * 32 + lane;
-            key[j] = (li < tile_n) ? in[tile_base + li] : ~0ull;
-        }
-        for (int k = lane; k < 257; k += 32) s_hist[w][k] = 0;
-        __syncwarp();
-        // ---- stable rank inside the warp: (round j, lane) order ------------------------------------------
+            for (int j = 0; j < ITEMS; j++) key[j] = __ldcs(in + tile_base + wbase + j * 32);
 #pragma unroll
-        for (int j = 0; j < SORT_ITEMS; j++) {
-            const uint32_t li = w * (32 * SORT_ITEMS) + j * 32 + lane;
-            const uint32_t d = (li < tile_n) ? (uint32_t)((key[j] >> shift) & 255ull) : 256u;
-            const unsigned peers = __match_any_sync(0xffffffffu, d);
-            const int leader = __ffs(peers) - 1;
-            uint32_t old = 0;
-            if (lane == leader) {
-                old = s_hist[w][d];
-                s_hist[w][d] = old + __popc(peers);
+            for (int j = 0; j < ITEMS; j += 2) {
+                const uint32_t ra = atomicAdd(&s_hist[w][(uint32_t)(key[j] >> shift) & 255u], 1u);
+                const uint32_t rb = atomicAdd(&s_hist[w][(uint32_t)(key[j + 1] >> shift) & 255u], 1u);
+                rk2[j / 2] = ra | (rb << 16);
             }
-            old = __shfl_sync(0xffffffffu, old, leader);
-            rk[j] = old + __popc(peers & lt_mask);
-            __syncwarp();
+        } else {
+#pragma unroll
+            for (int j = 0; j < ITEMS; j++) {
+                const uint32_t li = wbase + j * 32;
+                key[j] = (li < tile_n) ? in[tile_base + li] : 0ull;
+            }
+#pragma unroll
+            for (int j = 0; j < ITEMS; j += 2) {
+                uint32_t ra = 0, rb = 0;
+                if (wbase + j * 32 < tile_n) ra = atomicAdd(&s_hist[w][(uint32_t)(key[j] >> shift) & 255u], 1u);
+                if (wbase + (j + 1) * 32 < tile_n) rb = atomicAdd(&s_hist[w][(uint32_t)(key[j + 1] >> shift) & 255u], 1u);
+                rk2[j / 2] = ra | (rb << 16);
+            }
         }
         __syncthreads();
         // ---- per digit: exclusive prefix over warps, block count, publish aggregate ------------------------
@@ -89,29 +102,35 @@ radix_pass_kernel(const unsigned long long* __restrict__ in, unsigned long long*
         uint32_t tot;
         const uint32_t bpos = block_excl_scan_256(cnt, s_scan, tot);  // contains __syncthreads
         s_bpos[tid] = bpos;
-        if (tid == 0) {
-            s_bpos[256] = tot;  // invalid (tail) elements sort behind every digit
-            uint32_t c = 0;     // their per-warp offsets
-            for (int k = 0; k < NW; k++) { const uint32_t t = s_hist[k][256]; s_hist[k][256] = c; c += t; }
-        }
         __syncthreads();
         // ---- block-local reorder through shared memory ---------------------------------------------------
 #pragma unroll
-        for (int j = 0; j < SORT_ITEMS; j++) {
-            const uint32_t li = w * (32 * SORT_ITEMS) + j * 32 + lane;
-            const uint32_t d = (li < tile_n) ? (uint32_t)((key[j] >> shift) & 255ull) : 256u;
-            s_sorted[s_bpos[d] + s_hist[w][d] + rk[j]] = key[j];
+        for (int j = 0; j < ITEMS; j++) {
+            if (wbase + j * 32 < tile_n) {
+                const uint32_t d = (uint32_t)(key[j] >> shift) & 255u;
+                s_sorted[s_bpos[d] + s_hist[w][d] + ((rk2[j / 2] >> (16 * (j & 1))) & 0xffffu)] = key[j];
+            }
         }
-        // ---- decoupled look-back for digit `tid` ---------------------------------------------------------
+        // ---- decoupled look-back for digit `tid`, LB_WINDOW predecessors per round trip --------------------------
+        // (in the first wave every resident tile only has its aggregate published, so the walk back to an inclusive
+        // prefix is hundreds of tiles long: several status words in flight per step divide that latency chain)
         unsigned long long excl = 0;
         if (tile > 0) {
+            constexpr int LB_WINDOW = 4;
             int idx = tile - 1;
-            while (true) {
-                unsigned long long s;
-                do { s = ld_status(status + (size_t)idx * 256 + tid); } while ((s >> 62) == 0);
-                excl += s & ST_MASK;
-                if ((s >> 62) == 2 || idx == 0) break;
-                idx--;
+            bool done = false;
+            while (!done) {
+                unsigned long long sv[LB_WINDOW];
+#pragma unroll
+                for (int k = 0; k < LB_WINDOW; k++)
+                    sv[k] = (idx - k >= 0) ? ld_status(status + (size_t)(idx - k) * 256 + tid) : ST_INC;
+#pragma unroll
+                for (int k = 0; k < LB_WINDOW; k++) {
+                    if (done || (sv[k] >> 62) == 0) break;   // not published yet: poll again from here
+                    excl += sv[k] & ST_MASK;
+                    idx--;
+                    done = (sv[k] >> 62) == 2;
+                }
             }
             st_status(st, ST_INC | (excl + cnt));
         }
@@ -119,11 +138,11 @@ radix_pass_kernel(const unsigned long long* __restrict__ in, unsigned long long*
         __syncthreads();
         // ---- coalesced output: runs of equal digits are contiguous ---------------------------------------
 #pragma unroll
-        for (int j = 0; j < SORT_ITEMS; j++) {
+        for (int j = 0; j < ITEMS; j++) {
             const uint32_t li = j * SORT_THREADS + tid;
             if (li < tile_n) {
                 const unsigned long long k = s_sorted[li];
-                const uint32_t d = (uint32_t)((k >> shift) & 255ull);
+                const uint32_t d = (uint32_t)(k >> shift) & 255u;
                 const uint32_t pos = s_gpos[d] + li;
                 if (OUT32) out32[pos] = (uint32_t)k;
                 else out[pos] = k;
@@ -224,54 +243,81 @@ __device__ __forceinline__ uint32_t rect_tiles(const uint4 pg) {
     return w * h;
 }
 
+// One WARP per 256-rank tile (8 consecutive ranks per lane), chained through the look-back status words; no block
+// barrier.  The rect of every rank is gathered once here and stored in depth order for the duplicate kernel.
 __global__ void __launch_bounds__(SCAN_THREADS)
 scan_offsets_kernel(const Pointers p) {
-    __shared__ uint32_t s_scan[SCAN_THREADS / 32];
-    __shared__ int s_tile;
-    __shared__ unsigned long long s_base;
-    const int tid = threadIdx.x;
+    const int lane = threadIdx.x & 31;
     const unsigned long long n = p.ctrl->n_vis;
-    const bool dead = p.ctrl->overflow != 0;
+    if (p.ctrl->overflow != 0) return;
     while (true) {
-        __syncthreads();
-        if (tid == 0) s_tile = (int)atomicAdd(&p.ctrl->tile_counter[TC_SCAN], 1u);
-        __syncthreads();
-        const int tile = s_tile;
-        const unsigned long long base_r = (unsigned long long)tile * SCAN_TILE;
-        if (base_r >= n || dead) break;
-        uint32_t tt[SCAN_ITEMS];
+        int tile = 0;
+        if (lane == 0) tile = (int)atomicAdd(&p.ctrl->tile_counter[TC_SCAN], 1u);
+        tile = __shfl_sync(0xffffffffu, tile, 0);
+        const unsigned long long base_r = (unsigned long long)tile * SCAN_WARP_TILE + (unsigned long long)lane * SCAN_ITEMS;
+        if ((unsigned long long)tile * SCAN_WARP_TILE >= n) break;
+        uint32_t id[SCAN_ITEMS], tt[SCAN_ITEMS];
+        uint2 rc[SCAN_ITEMS];
+        const bool full = (unsigned long long)(tile + 1) * SCAN_WARP_TILE <= n;  // warp-uniform
+        if (full) {   // 64 contiguous, 64-byte aligned bytes per lane: four 16-byte loads
+            const ulonglong2* src = reinterpret_cast<const ulonglong2*>(p.gkeyA + base_r);
+#pragma unroll
+            for (int k = 0; k < SCAN_ITEMS; k += 2) {
+                const ulonglong2 v = __ldg(src + k / 2);
+                id[k] = (uint32_t)v.x; id[k + 1] = (uint32_t)v.y;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < SCAN_ITEMS; k++) id[k] = (base_r + k < n) ? (uint32_t)p.gkeyA[base_r + k] : 0xffffffffu;
+        }
         uint32_t sum = 0;
 #pragma unroll
         for (int k = 0; k < SCAN_ITEMS; k++) {
-            const unsigned long long r = base_r + (unsigned long long)tid * SCAN_ITEMS + k;
             tt[k] = 0;
-            if (r < n) {
-                const uint32_t id = (uint32_t)p.gkeyA[r];
-                tt[k] = rect_tiles(__ldg(p.per_g + id));
+            rc[k] = make_uint2(0u, 0u);
+            if (id[k] != 0xffffffffu) {
+                const uint4 pg = __ldg(p.per_g + id[k]);
+                rc[k] = make_uint2(pg.x, pg.y);
+                tt[k] = rect_tiles(pg);
             }
             sum += tt[k];
         }
-        uint32_t btotal;
-        const uint32_t texcl = block_excl_scan_256(sum, s_scan, btotal);
-        if (tid < 32) {
-            if (tid == 0) st_status(p.st_scan + tile, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)btotal);
-            unsigned long long excl = 0;
-            if (tile > 0) {
-                excl = lookback_warp(p.st_scan, tile);
-                if (tid == 0) st_status(p.st_scan + tile, ST_INC | (excl + btotal));
-            }
-            if (tid == 0) s_base = excl;
+        uint32_t inc = sum;   // inclusive scan over the lanes
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
         }
-        __syncthreads();
-        unsigned long long off = s_base + texcl;
+        const uint32_t wtotal = __shfl_sync(0xffffffffu, inc, 31);
+        if (lane == 0) st_status(p.st_scan + tile, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)wtotal);
+        unsigned long long excl = 0;
+        if (tile > 0) {
+            excl = lookback_warp(p.st_scan, tile);
+            if (lane == 0) st_status(p.st_scan + tile, ST_INC | (excl + wtotal));
+        }
+        unsigned long long off = excl + inc - sum;
+        if (full) {   // rect in depth order: duplicate_kernel reads it sequentially
+            uint32_t o[SCAN_ITEMS];
+            unsigned long long run = off;
+#pragma unroll
+            for (int k = 0; k < SCAN_ITEMS; k++) { o[k] = (uint32_t)run; run += tt[k]; }
+            uint4* d4 = reinterpret_cast<uint4*>(p.dup_off + base_r);
+            d4[0] = make_uint4(o[0], o[1], o[2], o[3]);
+            d4[1] = make_uint4(o[4], o[5], o[6], o[7]);
+            uint4* r4 = reinterpret_cast<uint4*>(p.rk_rect + base_r);
+#pragma unroll
+            for (int k = 0; k < SCAN_ITEMS; k += 2) r4[k / 2] = make_uint4(rc[k].x, rc[k].y, rc[k + 1].x, rc[k + 1].y);
+        }
 #pragma unroll
         for (int k = 0; k < SCAN_ITEMS; k++) {
-            const unsigned long long r = base_r + (unsigned long long)tid * SCAN_ITEMS + k;
-            if (r < n) {
-                p.dup_off[r] = (uint32_t)off;
+            if (base_r + k < n) {
+                if (!full) {
+                    p.dup_off[base_r + k] = (uint32_t)off;
+                    p.rk_rect[base_r + k] = rc[k];
+                }
                 if (tt[k]) {  // chunk boundaries c*DUP_TILE that fall inside [off, off + tt)
                     const unsigned long long c0 = (off + DUP_TILE - 1) / DUP_TILE, c1 = (off + tt[k] - 1) / DUP_TILE;
-                    for (unsigned long long c = c0; c <= c1; c++) p.chunk_start[c] = (uint32_t)r;
+                    for (unsigned long long c = c0; c <= c1; c++) p.chunk_start[c] = (uint32_t)(base_r + k);
                 }
             }
             off += tt[k];
@@ -287,9 +333,12 @@ scan_offsets_kernel(const Pointers p) {
 __global__ void __launch_bounds__(DUP_THREADS)
 duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict__ ent) {
     __shared__ uint32_t s_off[DUP_TILE + 2];
+    __shared__ uint2 s_rect[DUP_TILE + 2];
+    __shared__ uint32_t s_id[DUP_TILE + 2];
     const int tid = threadIdx.x;
     const unsigned long long n = p.ctrl->n_dup_eff;
     const uint32_t n_vis = (uint32_t)p.ctrl->n_vis;
+    const uint32_t gx = (uint32_t)f.gx;
     for (unsigned long long chunk = blockIdx.x; chunk * DUP_TILE < n; chunk += gridDim.x) {
         const unsigned long long k0 = chunk * DUP_TILE;
         const uint32_t cn = (uint32_t)min((unsigned long long)DUP_TILE, n - k0);
@@ -297,46 +346,54 @@ duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict
         const uint32_t r1 = ((chunk + 1) * DUP_TILE < n) ? p.chunk_start[chunk + 1] : (n_vis - 1);
         const uint32_t nr = r1 - r0 + 1;  // <= DUP_TILE + 1 ranks can start inside one chunk
         __syncthreads();
-        for (uint32_t k = tid; k < nr; k += DUP_THREADS) s_off[k] = p.dup_off[r0 + k];
+        for (uint32_t k = tid; k < nr; k += DUP_THREADS) {  // the chunk's ranks: offsets, rects, ids -- all sequential reads
+            s_off[k] = p.dup_off[r0 + k];
+            s_rect[k] = p.rk_rect[r0 + k];
+            s_id[k] = (uint32_t)p.gkeyA[r0 + k];
+        }
         __syncthreads();
         const uint32_t lk0 = tid * DUP_ITEMS;
         if (lk0 < cn) {
             const uint32_t kk = (uint32_t)k0 + lk0;  // N_dup < 2^32
-            // largest local rank with s_off <= kk
-            uint32_t lo = 0, hi = nr - 1;
+            uint32_t lo = 0, hi = nr - 1;            // largest local rank with s_off <= kk
             while (lo < hi) {
                 const uint32_t mid = (lo + hi + 1) >> 1;
                 if (s_off[mid] <= kk) lo = mid; else hi = mid - 1;
             }
             uint32_t lr = lo;
-            uint32_t id = (uint32_t)p.gkeyA[r0 + lr];
-            uint4 pg = __ldg(p.per_g + id);
-            uint32_t x0 = pg.x & 0xffffu, y0 = pg.x >> 16, wdt = (pg.y & 0xffffu) - x0;
-            uint32_t end = s_off[lr] + rect_tiles(pg);
+            uint2 rc = s_rect[lr];
+            uint32_t id = s_id[lr];
+            uint32_t x0 = rc.x & 0xffffu, x1 = rc.y & 0xffffu, wdt = x1 - x0;
+            uint32_t left = wdt * ((rc.y >> 16) - (rc.x >> 16)) - (kk - s_off[lr]);  // slots of this rank still to emit
+            uint32_t ty, tx;
+            {   // the one division of this thread: row-major position of slot kk inside the rect
+                const uint32_t j = kk - s_off[lr], row = j / wdt;
+                ty = (rc.x >> 16) + row;
+                tx = x0 + (j - row * wdt);
+            }
+            uint32_t tile = ty * gx + tx;
             unsigned long long outv[DUP_ITEMS];
 #pragma unroll
             for (int q = 0; q < DUP_ITEMS; q++) {
-                const uint32_t k = kk + q;
-                if (lk0 + q < cn) {
-                    while (k >= end) {  // advance to the rank owning slot k (every visible rank has >= 1 tile)
-                        lr++;
-                        id = (uint32_t)p.gkeyA[r0 + lr];
-                        pg = __ldg(p.per_g + id);
-                        x0 = pg.x & 0xffffu; y0 = pg.x >> 16; wdt = (pg.y & 0xffffu) - x0;
-                        end = s_off[lr] + rect_tiles(pg);
-                    }
-                    const uint32_t j = k - s_off[lr];
-                    const uint32_t ty = y0 + j / wdt, tx = x0 + j % wdt;
-                    outv[q] = ((unsigned long long)(ty * (uint32_t)f.gx + tx) << 32) | id;
-                } else {
-                    outv[q] = 0;
+                outv[q] = ((unsigned long long)tile << 32) | id;
+                // advance to the next slot: next column, next row of the rect, or the next rank (every visible rank
+                // has >= 1 tile).  Past the end of the chunk the values are never stored.
+                tx++; tile++; left--;
+                if (left == 0) {
+                    lr = min(lr + 1, nr - 1);
+                    rc = s_rect[lr]; id = s_id[lr];
+                    x0 = rc.x & 0xffffu; x1 = rc.y & 0xffffu; wdt = x1 - x0;
+                    left = wdt * ((rc.y >> 16) - (rc.x >> 16));
+                    tx = x0; ty = rc.x >> 16; tile = ty * gx + tx;
+                } else if (tx == x1) {
+                    tx = x0; ty++; tile = ty * gx + tx;
                 }
             }
             unsigned long long* dst = ent + k0 + lk0;
             if (lk0 + DUP_ITEMS <= cn) {
 #pragma unroll
                 for (int q = 0; q < DUP_ITEMS; q += 2)
-                    *reinterpret_cast<ulonglong2*>(dst + q) = make_ulonglong2(outv[q], outv[q + 1]);
+                    __stcs(reinterpret_cast<ulonglong2*>(dst + q), make_ulonglong2(outv[q], outv[q + 1]));
             } else {
                 for (int q = 0; q < DUP_ITEMS && lk0 + q < cn; q++) dst[q] = outv[q];
             }
@@ -349,14 +406,30 @@ duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict
 // ------------------------------------------------------------------------------------------------------------
 static int imin(long long a, long long b) { return (int)(a < b ? a : b); }
 
+// Launch one pass with the tile size chosen from the CAPACITY of the sorted array (sort_items_for, common.cuh): small
+// arrays use 1 024-key tiles (more blocks, shorter critical path), large ones 4 096-key tiles (less look-back traffic).
+template <bool OUT32>
+static void launch_pass(int items, int n_sm, unsigned long long capacity, const unsigned long long* in,
+                        unsigned long long* out, uint32_t* out32, const unsigned long long* n_ptr, int shift,
+                        const uint32_t* ghist, unsigned long long* status, uint32_t* tile_counter, cudaStream_t st) {
+    const long long tile_n = (long long)SORT_THREADS * items;
+    const long long cap_tiles = ((long long)capacity + tile_n - 1) / tile_n;
+    if (items == 16) {
+        const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
+        radix_pass_kernel<16, OUT32><<<grid, SORT_THREADS, 0, st>>>(in, out, out32, n_ptr, shift, ghist, status, tile_counter);
+    } else {
+        const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 6);
+        radix_pass_kernel<4, OUT32><<<grid, SORT_THREADS, 0, st>>>(in, out, out32, n_ptr, shift, ghist, status, tile_counter);
+    }
+}
+
 void launch_depth_sort(const Frame& f, const Pointers& p, int n_sm, cudaStream_t st, int* launches) {
-    const long long cap_tiles = ((long long)f.P + SORT_TILE - 1) / SORT_TILE;
-    const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
     unsigned long long* bufs[2] = {p.gkeyA, p.gkeyB};
+    const int items = sort_items_for((unsigned long long)f.P);
     for (int pass = 0; pass < MAX_SORT_PASSES_DEPTH; pass++) {
-        radix_pass_kernel<false><<<grid, SORT_THREADS, 0, st>>>(
-            bufs[pass & 1], bufs[(pass + 1) & 1], nullptr, &p.ctrl->n_vis, 32 + 8 * pass, p.ctrl->depth_hist[pass],
-            p.st_depth + (size_t)pass * p.n_depth_tiles * 256, &p.ctrl->tile_counter[TC_DEPTH0 + pass]);
+        launch_pass<false>(items, n_sm, (unsigned long long)f.P, bufs[pass & 1], bufs[(pass + 1) & 1], nullptr, &p.ctrl->n_vis,
+                           32 + 8 * pass, p.ctrl->depth_hist[pass], p.st_depth + (size_t)pass * p.n_depth_tiles * 256,
+                           &p.ctrl->tile_counter[TC_DEPTH0 + pass], st);
         (*launches)++;
     }
 }
@@ -367,8 +440,8 @@ void launch_tile_grid(const Frame& f, const Pointers& p, uint32_t* out_tile_coun
 }
 
 void launch_scan_offsets(const Frame& f, const Pointers& p, int n_sm, cudaStream_t st, int* launches) {
-    const long long cap_tiles = ((long long)f.P + SCAN_TILE - 1) / SCAN_TILE;
-    const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 8);
+    const long long cap_blocks = ((long long)f.P + SCAN_WARP_TILE * (SCAN_THREADS / 32) - 1) / (SCAN_WARP_TILE * (SCAN_THREADS / 32));
+    const int grid = imin(cap_blocks > 0 ? cap_blocks : 1, (long long)n_sm * 8);
     scan_offsets_kernel<<<grid, SCAN_THREADS, 0, st>>>(p);
     (*launches)++;
 }
@@ -381,23 +454,65 @@ void launch_duplicate_and_tile_sort(const Frame& f, const Pointers& p, int n_sm,
     duplicate_kernel<<<dgrid, DUP_THREADS, 0, st>>>(f, p, p.entA);
     (*launches)++;
     if (ev_after_duplicate) cudaEventRecord(ev_after_duplicate, st);
-    const long long cap_tiles = ((long long)f.max_dup + SORT_TILE - 1) / SORT_TILE;
-    const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
     unsigned long long* bufs[2] = {p.entA, p.entB};
+    const int items = sort_items_for(f.max_dup);
     for (int pass = 0; pass < f.n_tile_passes; pass++) {
         const bool last = pass == f.n_tile_passes - 1;
         unsigned long long* status = p.st_tile + (size_t)pass * p.n_tile_tiles * 256;
         if (last)
-            radix_pass_kernel<true><<<grid, SORT_THREADS, 0, st>>>(bufs[pass & 1], nullptr, p.ids, &p.ctrl->n_dup_eff,
-                                                                  32 + 8 * pass, p.ctrl->tile_hist[pass], status,
-                                                                  &p.ctrl->tile_counter[TC_TILE0 + pass]);
+            launch_pass<true>(items, n_sm, f.max_dup, bufs[pass & 1], nullptr, p.ids, &p.ctrl->n_dup_eff, 32 + 8 * pass,
+                              p.ctrl->tile_hist[pass], status, &p.ctrl->tile_counter[TC_TILE0 + pass], st);
         else
-            radix_pass_kernel<false><<<grid, SORT_THREADS, 0, st>>>(bufs[pass & 1], bufs[(pass + 1) & 1], nullptr,
-                                                                   &p.ctrl->n_dup_eff, 32 + 8 * pass,
-                                                                   p.ctrl->tile_hist[pass], status,
-                                                                   &p.ctrl->tile_counter[TC_TILE0 + pass]);
+            launch_pass<false>(items, n_sm, f.max_dup, bufs[pass & 1], bufs[(pass + 1) & 1], nullptr, &p.ctrl->n_dup_eff,
+                               32 + 8 * pass, p.ctrl->tile_hist[pass], status, &p.ctrl->tile_counter[TC_TILE0 + pass], st);
         (*launches)++;
     }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Self-test of the hardware property radix_pass_kernel's ranking relies on (see its header): `rounds` back-to-back
+// shared-memory atomicAdd per thread on a warp-private counter array return, for every key, exactly its stable rank
+// in (round, lane) order -- checked against a shuffle-based count, with random digits drawn from `nbins` bins and a
+// divergent subset of lanes every fourth iteration.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+atomic_order_selftest_kernel(unsigned long long* __restrict__ out, int iters, uint32_t seed, int nbins) {
+    __shared__ uint32_t hist[8][256];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint32_t s = seed ^ (blockIdx.x * 0x9E3779B9u) ^ (threadIdx.x * 0x85EBCA6Bu);
+    unsigned long long bad = 0;
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int k = 0; k < 8; k++) hist[w][k * 32 + lane] = 0;
+        __syncwarp();
+        uint32_t d[8], r[8];
+#pragma unroll
+        for (int j = 0; j < 8; j++) { s = s * 1664525u + 1013904223u; d[j] = (s >> 16) % (uint32_t)nbins; }
+        const bool act = (it & 3) != 3 || ((s >> 8) & 1u);
+        if (act) {
+#pragma unroll
+            for (int j = 0; j < 8; j++) r[j] = atomicAdd(&hist[w][d[j]], 1u);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 8; j++) {
+            uint32_t cnt = 0;
+            for (int jj = 0; jj <= j; jj++)
+                for (int l = 0; l < 32; l++) {
+                    const uint32_t od = __shfl_sync(0xffffffffu, d[jj], l);
+                    const int oa = __shfl_sync(0xffffffffu, (int)act, l);
+                    if (oa && od == d[j] && (jj < j || l < lane)) cnt++;
+                }
+            if (act && r[j] != cnt) bad++;
+        }
+        __syncwarp();
+    }
+    if (bad) atomicAdd(out, bad);
+    if (threadIdx.x == 0) atomicAdd(out + 1, (unsigned long long)iters * 8ull * blockDim.x);
+}
+
+void launch_atomic_order_selftest(unsigned long long* out, int iters, uint32_t seed, int nbins, int n_sm, cudaStream_t st) {
+    atomic_order_selftest_kernel<<<n_sm * 4, 256, 0, st>>>(out, iters, seed, nbins);
 }
 
 }  // namespace gs

@@ -10,12 +10,12 @@ constexpr int TILE = 16;
 constexpr int MAX_SORT_PASSES_DEPTH = 4;   // 32 depth bits, 8-bit digits
 constexpr int MAX_SORT_PASSES_TILE = 3;    // up to 24 tile-id bits
 constexpr int SORT_THREADS = 256;
-constexpr int SORT_ITEMS = 16;
-constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;  // 4096 elements per block-tile
+// keys per thread of a radix-pass tile, from the CAPACITY of the array being sorted (host and layout agree on it)
+__host__ __device__ inline int sort_items_for(unsigned long long capacity) { return capacity <= (4ull << 20) ? 4 : 16; }
 constexpr int PRE_THREADS = 256;                      // Gaussians per preprocess tile
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;
-constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;  // 2048 sorted Gaussians per offset-scan tile
+constexpr int SCAN_WARP_TILE = 32 * SCAN_ITEMS;        // 256 depth-sorted Gaussians per offset-scan tile (one warp)
 constexpr int DUP_THREADS = 256;
 constexpr int DUP_ITEMS = 8;
 constexpr int DUP_TILE = DUP_THREADS * DUP_ITEMS;     // 2048 duplicated entries per block
@@ -62,6 +62,7 @@ struct Pointers {           // device pointers carved from the workspace
     unsigned long long* gkeyA;              // [P] (depth bits << 32 | id), compacted
     unsigned long long* gkeyB;              // [P] ping-pong
     uint32_t* dup_off;                      // [P] exclusive prefix of tiles_touched in depth order
+    uint2* rk_rect;                         // [P] tile rect {xmin | ymin<<16, xmax | ymax<<16} in depth order
     uint32_t* chunk_start;                  // [ceil(max_dup / DUP_TILE) + 1] depth rank owning entry c * DUP_TILE
     uint32_t* ranges;                       // [n_tiles + 1]
     unsigned long long* entA;               // [max_dup] (tile << 32 | id)

@@ -119,154 +119,139 @@ __device__ __forceinline__ bool project(const Frame& f, float px, float py, floa
 }
 
 // C-P9: colour = max(0, 0.5 + sum_k (-1)^m Y_lm(d) sh[k]), k = l^2 + l + m, d = unit vector camera -> Gaussian
-// ("view-dependent color parameterized by spherical harmonics"; reading S8).
-__device__ __forceinline__ void sh_basis(int deg, float x, float y, float z, float* Y) {
-    Y[0] = 0.28209479177387814f;
-    if (deg < 1) return;
-    Y[1] = -0.4886025119029199f * y;
-    Y[2] = 0.4886025119029199f * z;
-    Y[3] = -0.4886025119029199f * x;
-    if (deg < 2) return;
-    const float xx = x * x, yy = y * y, zz = z * z;
-    Y[4] = 1.0925484305920792f * x * y;
-    Y[5] = -1.0925484305920792f * y * z;
-    Y[6] = 0.31539156525252005f * (2.0f * zz - xx - yy);
-    Y[7] = -1.0925484305920792f * x * z;
-    Y[8] = 0.5462742152960396f * (xx - yy);
-    if (deg < 3) return;
-    Y[9] = -0.5900435899266435f * y * (3.0f * xx - yy);
-    Y[10] = 2.890611442640554f * x * y * z;
-    Y[11] = -0.4570457994644658f * y * (4.0f * zz - xx - yy);
-    Y[12] = 0.3731763325901154f * z * (2.0f * zz - 3.0f * xx - 3.0f * yy);
-    Y[13] = -0.4570457994644658f * x * (4.0f * zz - xx - yy);
-    Y[14] = 1.445305721320277f * z * (xx - yy);
-    Y[15] = -0.5900435899266435f * x * (xx - 3.0f * yy);
-}
-
+// ("view-dependent color parameterized by spherical harmonics"; reading S8).  DEG is a template parameter
+// so that the basis lives in registers (a runtime degree indexes the array dynamically and spills it to local memory).
+template <int DEG>
 __device__ __forceinline__ float3 sh_colour(const Frame& f, const float* __restrict__ sh, int i, float px, float py,
                                             float pz) {
-    float dx = px - f.campos[0], dy = py - f.campos[1], dz = pz - f.campos[2];
-    const float rn = rsqrtf(dx * dx + dy * dy + dz * dz);
-    dx *= rn; dy *= rn; dz *= rn;
-    float Y[16];
-    sh_basis(f.deg, dx, dy, dz, Y);
-    float r = 0.5f, g = 0.5f, b = 0.5f;
-    if (f.deg == 3) {  // 48 floats = 12 aligned float4 (192 B per Gaussian)
-        const float4* s4 = reinterpret_cast<const float4*>(sh + (size_t)i * 48);
-        float c[48];
+    constexpr int K = (DEG + 1) * (DEG + 1);
+    float x = px - f.campos[0], y = py - f.campos[1], z = pz - f.campos[2];
+    const float rn = rsqrtf(x * x + y * y + z * z);
+    x *= rn; y *= rn; z *= rn;
+    float Y[K];
+    Y[0] = 0.28209479177387814f;
+    if (DEG >= 1) {
+        Y[1] = -0.4886025119029199f * y;
+        Y[2] = 0.4886025119029199f * z;
+        Y[3] = -0.4886025119029199f * x;
+    }
+    if (DEG >= 2) {
+        const float xx = x * x, yy = y * y, zz = z * z;
+        Y[4] = 1.0925484305920792f * x * y;
+        Y[5] = -1.0925484305920792f * y * z;
+        Y[6] = 0.31539156525252005f * (2.0f * zz - xx - yy);
+        Y[7] = -1.0925484305920792f * x * z;
+        Y[8] = 0.5462742152960396f * (xx - yy);
+        if (DEG >= 3) {
+            Y[9] = -0.5900435899266435f * y * (3.0f * xx - yy);
+            Y[10] = 2.890611442640554f * x * y * z;
+            Y[11] = -0.4570457994644658f * y * (4.0f * zz - xx - yy);
+            Y[12] = 0.3731763325901154f * z * (2.0f * zz - 3.0f * xx - 3.0f * yy);
+            Y[13] = -0.4570457994644658f * x * (4.0f * zz - xx - yy);
+            Y[14] = 1.445305721320277f * z * (xx - yy);
+            Y[15] = -0.5900435899266435f * x * (xx - 3.0f * yy);
+        }
+    }
+    float c[3 * K];
+    if (K % 4 == 0) {  // degrees 1 and 3: 12 / 48 floats = 3 / 12 aligned float4 per Gaussian
+        const float4* s4 = reinterpret_cast<const float4*>(sh + (size_t)i * (3 * K));
 #pragma unroll
-        for (int k = 0; k < 12; k++) {
-            const float4 v = __ldg(s4 + k);
+        for (int k = 0; k < 3 * K / 4; k++) {
+            const float4 v = __ldcs(s4 + k);
             c[4 * k] = v.x; c[4 * k + 1] = v.y; c[4 * k + 2] = v.z; c[4 * k + 3] = v.w;
         }
-#pragma unroll
-        for (int k = 0; k < 16; k++) {
-            r = fmaf(Y[k], c[3 * k], r); g = fmaf(Y[k], c[3 * k + 1], g); b = fmaf(Y[k], c[3 * k + 2], b);
-        }
     } else {
-        const float* s = sh + (size_t)i * f.K * 3;
-        for (int k = 0; k < f.K; k++) {
-            r = fmaf(Y[k], __ldg(s + 3 * k), r); g = fmaf(Y[k], __ldg(s + 3 * k + 1), g); b = fmaf(Y[k], __ldg(s + 3 * k + 2), b);
-        }
+        const float* s1 = sh + (size_t)i * (3 * K);
+#pragma unroll
+        for (int k = 0; k < 3 * K; k++) c[k] = __ldcs(s1 + k);
+    }
+    float r = 0.5f, g = 0.5f, b = 0.5f;
+#pragma unroll
+    for (int k = 0; k < K; k++) {
+        r = fmaf(Y[k], c[3 * k], r); g = fmaf(Y[k], c[3 * k + 1], g); b = fmaf(Y[k], c[3 * k + 2], b);
     }
     return make_float3(fmaxf(r, 0.0f), fmaxf(g, 0.0f), fmaxf(b, 0.0f));
 }
 
-// Warp-aggregated atomic add on the difference grid: lanes with equal `cell` elect one leader.
-__device__ __forceinline__ void grid_add(int* diff, bool on, int cell, int val) {
-    const unsigned peers = __match_any_sync(0xffffffffu, on ? cell : -1);
-    if (on && (__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(diff + cell, val * __popc(peers));
-}
-
+// One WARP is the unit of the order-preserving compaction: it takes one 32-Gaussian sub-tile per atomic ticket,
+// publishes the sub-tile's count of visible Gaussians at once, does all the heavy work (SH colour, records, coverage
+// grid, histograms), and only then looks back for its exclusive prefix -- by which time the predecessors have long
+// published.  There is no block barrier inside the loop.  (Several sub-tiles per ticket would serialise the warps:
+// the count of a later sub-tile is only known when its owner reaches it.)
+template <int DEG>
 __global__ void __launch_bounds__(PRE_THREADS)
 preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ means, const float* __restrict__ scales,
                   const float* __restrict__ rots, const float* __restrict__ opac, const float* __restrict__ sh) {
     __shared__ uint32_t s_hist[MAX_SORT_PASSES_DEPTH][256];
-    __shared__ uint32_t s_wcount[PRE_THREADS / 32];
-    __shared__ int s_tile;
-    __shared__ unsigned long long s_base;
-    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
     for (int k = tid; k < MAX_SORT_PASSES_DEPTH * 256; k += PRE_THREADS) (&s_hist[0][0])[k] = 0;
-    const int n_tiles = (f.P + PRE_THREADS - 1) / PRE_THREADS;
+    __syncthreads();
+    const int n_tiles = (f.P + 31) / 32;
+    const int gw = f.gx + 1;
+    const unsigned lt = (1u << lane) - 1u;
     while (true) {
-        __syncthreads();  // s_tile / s_base / s_wcount reuse; also orders the histogram zeroing
-        if (tid == 0) s_tile = (int)atomicAdd(&p.ctrl->tile_counter[TC_PRE], 1u);
-        __syncthreads();
-        const int tile = s_tile;
+        int tile = 0;
+        if (lane == 0) tile = (int)atomicAdd(&p.ctrl->tile_counter[TC_PRE], 1u);
+        tile = __shfl_sync(0xffffffffu, tile, 0);
         if (tile >= n_tiles) break;
-        const int i = tile * PRE_THREADS + tid;
-        Splat s = {};
-        bool vis = false;
-        float px = 0.f, py = 0.f, pz = 0.f;
-        if (i < f.P) {
-            px = __ldg(means + 3 * (size_t)i); py = __ldg(means + 3 * (size_t)i + 1); pz = __ldg(means + 3 * (size_t)i + 2);
-            const float sx = __ldg(scales + 3 * (size_t)i), sy = __ldg(scales + 3 * (size_t)i + 1), sz = __ldg(scales + 3 * (size_t)i + 2);
-            const float4 q = __ldg(reinterpret_cast<const float4*>(rots) + i);
-            vis = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, s);
-        }
-        // ---- block-level count of visible Gaussians; publish the aggregate early, look back with warp 0 ----
-        const unsigned vb = __ballot_sync(0xffffffffu, vis);
-        if (lane == 0) s_wcount[w] = __popc(vb);
-        __syncthreads();
-        uint32_t wbase = 0, btotal = 0;
-#pragma unroll
-        for (int k = 0; k < PRE_THREADS / 32; k++) {
-            const uint32_t c = s_wcount[k];
-            if (k < w) wbase += c;
-            btotal += c;
-        }
-        if (w == 0) {
-            if (lane == 0) st_status(p.st_pre + tile, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)btotal);
-            unsigned long long excl = 0;
-            if (tile > 0) {
-                excl = lookback_warp(p.st_pre, tile);
-                if (lane == 0) st_status(p.st_pre + tile, ST_INC | (excl + btotal));
+        {
+            const int i = tile * 32 + lane;
+            Splat s = {};
+            bool vis = false;
+            float px = 0.f, py = 0.f, pz = 0.f;
+            if (i < f.P) {
+                // plain loads: the three components of a lane share their cache lines with the neighbouring lanes
+                px = __ldg(means + 3 * (size_t)i); py = __ldg(means + 3 * (size_t)i + 1); pz = __ldg(means + 3 * (size_t)i + 2);
+                const float sx = __ldg(scales + 3 * (size_t)i), sy = __ldg(scales + 3 * (size_t)i + 1), sz = __ldg(scales + 3 * (size_t)i + 2);
+                const float4 q = __ldcs(reinterpret_cast<const float4*>(rots) + i);
+                vis = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, s);
             }
-            if (lane == 0) {
-                s_base = excl;
-                if (tile == n_tiles - 1) p.ctrl->n_vis = excl + btotal;
+            const unsigned vb = __ballot_sync(0xffffffffu, vis);
+            const uint32_t cnt = __popc(vb);
+            if (lane == 0) st_status(p.st_pre + tile, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)cnt);
+            // ---- everything that does not need the compact index ----------------------------------------------
+            if (i < f.P) {
+                uint4 pg = make_uint4(0u, 0u, 0u, 0u);
+                if (vis) {
+                    pg.x = (uint32_t)s.xmin | ((uint32_t)s.ymin << 16);
+                    pg.y = (uint32_t)s.xmax | ((uint32_t)s.ymax << 16);
+                    pg.z = __float_as_uint(s.depth);
+                    pg.w = (uint32_t)s.radius;
+                }
+                p.per_g[i] = pg;
             }
-        }
-        // ---- everything that does not need the compact index: per-Gaussian record, colour, grid, histograms ----
-        if (i < f.P) {
-            uint4 pg = make_uint4(0u, 0u, 0u, 0u);
             if (vis) {
-                pg.x = (uint32_t)s.xmin | ((uint32_t)s.ymin << 16);
-                pg.y = (uint32_t)s.xmax | ((uint32_t)s.ymax << 16);
-                pg.z = __float_as_uint(s.depth);
-                pg.w = (uint32_t)s.radius;
+                atomicAdd(p.diff + s.ymin * gw + s.xmin, 1);
+                atomicAdd(p.diff + s.ymin * gw + s.xmax, -1);
+                atomicAdd(p.diff + s.ymax * gw + s.xmin, -1);
+                atomicAdd(p.diff + s.ymax * gw + s.xmax, 1);
+                const uint32_t db = __float_as_uint(s.depth);
+                atomicAdd(&s_hist[0][db & 255u], 1u);
+                atomicAdd(&s_hist[1][(db >> 8) & 255u], 1u);
+                atomicAdd(&s_hist[2][(db >> 16) & 255u], 1u);
+                atomicAdd(&s_hist[3][db >> 24], 1u);
+                const float o = __ldcs(opac + i);
+                const float3 col = sh_colour<DEG>(f, sh, i, px, py, pz);
+                // det of the STORED conic, exact products in double (24+24 bits): the form is indefinite iff det <= 0,
+                // and the tight box of the render stage needs det without fp32 cancellation (needle-like splats)
+                const double dd = (double)s.ca * (double)s.cc - (double)s.cb * (double)s.cb;
+                const float l2o = log2f(o);
+                const TightBox tb = tight_box_constants(s.ca, s.cb, s.cc, (float)dd, l2o);
+                const uint32_t flags = (!(dd > 0.0) || tb.degenerate) ? 1u : 0u;
+                float4* rec = p.rec + 4 * (size_t)i;  // 64-byte render record (include/gs.h: gs_intermediates.record)
+                rec[0] = make_float4(s.mux, s.muy, s.ca, s.cb);
+                rec[1] = make_float4(s.cc, l2o, (float)dd, __uint_as_float(flags));
+                rec[2] = make_float4(col.x, col.y, col.z, tb.xstar);
+                rec[3] = make_float4(tb.ic, tb.ct, 0.0f, 0.0f);
             }
-            p.per_g[i] = pg;
-        }
-        const int gw = f.gx + 1;
-        grid_add(p.diff, vis, s.ymin * gw + s.xmin, 1);
-        grid_add(p.diff, vis, s.ymin * gw + s.xmax, -1);
-        grid_add(p.diff, vis, s.ymax * gw + s.xmin, -1);
-        grid_add(p.diff, vis, s.ymax * gw + s.xmax, 1);
-        if (vis) {
-            const uint32_t db = __float_as_uint(s.depth);
-            atomicAdd(&s_hist[0][db & 255u], 1u);
-            atomicAdd(&s_hist[1][(db >> 8) & 255u], 1u);
-            atomicAdd(&s_hist[2][(db >> 16) & 255u], 1u);
-            atomicAdd(&s_hist[3][db >> 24], 1u);
-            const float o = __ldg(opac + i);
-            const float3 col = sh_colour(f, sh, i, px, py, pz);
-            // det of the STORED conic, exact products in double (24+24 bits): the form is indefinite iff det <= 0,
-            // and the tight box of the render stage needs det without fp32 cancellation (needle-like splats)
-            const double dd = (double)s.ca * (double)s.cc - (double)s.cb * (double)s.cb;
-            const float l2o = log2f(o);
-            const TightBox tb = tight_box_constants(s.ca, s.cb, s.cc, (float)dd, l2o);
-            const uint32_t flags = (!(dd > 0.0) || tb.degenerate) ? 1u : 0u;
-            float4* rec = p.rec + 4 * (size_t)i;  // 64-byte render record (include/gs.h: gs_intermediates.record)
-            rec[0] = make_float4(s.mux, s.muy, s.ca, s.cb);
-            rec[1] = make_float4(s.cc, l2o, (float)dd, __uint_as_float(flags));
-            rec[2] = make_float4(col.x, col.y, col.z, tb.xstar);
-            rec[3] = make_float4(tb.ic, tb.ct, 0.0f, 0.0f);
-        }
-        __syncthreads();  // s_base ready
-        if (vis) {
-            const unsigned long long cidx = s_base + wbase + __popc(vb & ((1u << lane) - 1u));
-            p.gkeyA[cidx] = ((unsigned long long)__float_as_uint(s.depth) << 32) | (unsigned)i;
+            // ---- exclusive prefix: own chunk's running total, else decoupled look-back ("prefix scan") ----
+            const unsigned long long excl = tile > 0 ? lookback_warp(p.st_pre, tile) : 0ull;
+            const unsigned long long run = excl + cnt;
+            if (lane == 0) {
+                st_status(p.st_pre + tile, ST_INC | run);
+                if (tile == n_tiles - 1) p.ctrl->n_vis = run;
+            }
+            if (vis) p.gkeyA[excl + __popc(vb & lt)] = ((unsigned long long)__float_as_uint(s.depth) << 32) | (unsigned)i;
         }
     }
     __syncthreads();
@@ -277,8 +262,15 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
 }
 
 void launch_preprocess(const Frame& f, const Pointers& p, const float* means, const float* scales, const float* rots,
-                       const float* opac, const float* sh, int n_blocks, cudaStream_t st) {
-    preprocess_kernel<<<n_blocks, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh);
+                       const float* opac, const float* sh, int n_sm, cudaStream_t st) {
+    const long long warps = ((long long)f.P + 31) / 32, blocks = (warps + PRE_THREADS / 32 - 1) / (PRE_THREADS / 32);
+    const int grid = (int)(blocks < 1 ? 1 : (blocks < (long long)n_sm * 8 ? blocks : (long long)n_sm * 8));
+    switch (f.deg) {
+        case 0: preprocess_kernel<0><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh); break;
+        case 1: preprocess_kernel<1><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh); break;
+        case 2: preprocess_kernel<2><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh); break;
+        default: preprocess_kernel<3><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh); break;
+    }
 }
 
 }  // namespace gs

@@ -39,7 +39,7 @@ def run_gpu(scene, cam_index=0, max_dup=None, variant=None, count_contrib=True, 
 def run_gpu_auto(scene, cam_index=0, variant=None, count_contrib=True, device="cuda:0", start_dup=1 << 20):
     """Render, growing the workspace when the frame needs more duplicates than it holds (GS_ERR_OVERFLOW)."""
     max_dup = start_dup
-    while True:
+    for attempt in range(4):
         r = run_gpu(scene, cam_index, max_dup, variant, count_contrib, device)
         try:
             it = r.intermediates()
@@ -47,9 +47,11 @@ def run_gpu_auto(scene, cam_index=0, variant=None, count_contrib=True, device="c
         except binding.GsError as e:
             if e.code != binding.GS_ERR_OVERFLOW:
                 raise
+            assert e.n_dup > max_dup, "overflow reported although the workspace was sized for %d >= %d duplicates" % (max_dup, e.n_dup)
             max_dup = int(e.n_dup * 1.02) + 4096
             del r
             torch.cuda.empty_cache()
+    raise AssertionError("workspace still too small after 4 attempts")
 
 
 def compare(r, it, ref, check_lists=True, check_pixels=True):

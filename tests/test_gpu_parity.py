@@ -226,3 +226,11 @@ def test_per_stage_timings_and_launch_count():
         binding.gs_set_timing(False)
     assert set(t) == set(binding.TIMING_NAMES) and all(v >= 0 for v in t.values()) and t["frame"] > 0
     assert binding.gs_last_launch_count() >= 8
+
+
+def test_shared_atomic_rank_order_selftest():
+    """The radix sort ranks keys with one shared-memory atomicAdd each and relies on same-address lanes being served in
+    lane order (csrc/binning.cu header); the device self-test checks that property on this GPU."""
+    r = binding.gs_selftest_atomic_order(40)
+    assert r["atomics_checked"] > 10_000_000
+    assert r["violations"] == 0, r

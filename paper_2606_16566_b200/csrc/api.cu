@@ -31,7 +31,7 @@ struct Layout {
     size_t ctrl, diff, st_pre, st_scan, st_depth, st_tile, zero_end;
     size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, entA, entB, ids, total;
     size_t n_depth_tiles, n_tile_tiles;
-    int gx, gy, n_tiles, tile_bits, n_tile_passes;
+    int gx, gy, n_tiles, tile_bits, n_tile_passes, diff_copies, diff_cells;
 };
 
 bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
@@ -51,7 +51,10 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o = up(o + bytes); return at; };
     L.ctrl = take(sizeof(Ctrl));
-    L.diff = take(sizeof(int) * (size_t)(L.gx + 1) * (L.gy + 1));
+    L.diff_cells = (L.gx + 1) * (L.gy + 1);
+    L.diff_copies = 1;   // replicas of the coverage grid (spreads the hot corner counters of small grids)
+    while (L.diff_copies < 16 && (long long)L.diff_cells * L.diff_copies * 2 <= 65536) L.diff_copies *= 2;
+    L.diff = take(sizeof(int) * (size_t)L.diff_cells * L.diff_copies);
     L.st_pre = take(8 * ((Pz + 31) / 32 + 1));
     L.st_scan = take(8 * ((Pz + SCAN_WARP_TILE - 1) / SCAN_WARP_TILE + 1));
     L.st_depth = take(8 * 256 * L.n_depth_tiles * MAX_SORT_PASSES_DEPTH);
@@ -178,6 +181,8 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     f.P = P; f.W = W; f.H = H; f.gx = L.gx; f.gy = L.gy; f.n_tiles = L.n_tiles;
     f.deg = sh_degree; f.K = (sh_degree + 1) * (sh_degree + 1);
     f.tile_bits = L.tile_bits; f.n_tile_passes = L.n_tile_passes;
+    f.compact = P >= COMPACT_MIN_P ? 1 : 0;
+    f.diff_copies = L.diff_copies; f.diff_cells = L.diff_cells;
     for (int k = 0; k < 16; k++) { f.V[k] = viewmatrix[k]; f.PM[k] = projmatrix[k]; }
     f.fx = fx; f.fy = fy;
     // camera centre of the rigid view matrix: campos = -Wv^T t (the north_star signature carries no campos)

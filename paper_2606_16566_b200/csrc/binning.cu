@@ -170,7 +170,9 @@ tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts 
         int carry = 0;
         for (int x0 = 0; x0 < gw; x0 += 32) {
             const int x = x0 + lane;
-            int v = (x < gw) ? diff[y * gw + x] : 0;
+            int v = 0;
+            if (x < gw)
+                for (int r = 0; r < f.diff_copies; r++) v += diff[(size_t)r * f.diff_cells + y * gw + x];
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 const int t = __shfl_up_sync(0xffffffffu, v, o);
@@ -427,7 +429,7 @@ void launch_depth_sort(const Frame& f, const Pointers& p, int n_sm, cudaStream_t
     unsigned long long* bufs[2] = {p.gkeyA, p.gkeyB};
     const int items = sort_items_for((unsigned long long)f.P);
     for (int pass = 0; pass < MAX_SORT_PASSES_DEPTH; pass++) {
-        launch_pass<false>(items, n_sm, (unsigned long long)f.P, bufs[pass & 1], bufs[(pass + 1) & 1], nullptr, &p.ctrl->n_vis,
+        launch_pass<false>(items, n_sm, (unsigned long long)f.P, bufs[pass & 1], bufs[(pass + 1) & 1], nullptr, &p.ctrl->n_sort,
                            32 + 8 * pass, p.ctrl->depth_hist[pass], p.st_depth + (size_t)pass * p.n_depth_tiles * 256,
                            &p.ctrl->tile_counter[TC_DEPTH0 + pass], st);
         (*launches)++;

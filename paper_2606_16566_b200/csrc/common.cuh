@@ -12,7 +12,8 @@ constexpr int MAX_SORT_PASSES_TILE = 3;    // up to 24 tile-id bits
 constexpr int SORT_THREADS = 256;
 // keys per thread of a radix-pass tile, from the CAPACITY of the array being sorted (host and layout agree on it)
 __host__ __device__ inline int sort_items_for(unsigned long long capacity) { return capacity <= (4ull << 20) ? 4 : 16; }
-constexpr int PRE_THREADS = 256;                      // Gaussians per preprocess tile
+constexpr int PRE_THREADS = 256;                      // threads per preprocess block (one 32-Gaussian sub-tile per warp)
+constexpr int COMPACT_MIN_P = 1 << 20;                // scenes below this size skip the compaction of visible Gaussians
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_WARP_TILE = 32 * SCAN_ITEMS;        // 256 depth-sorted Gaussians per offset-scan tile (one warp)
@@ -24,7 +25,8 @@ constexpr int DUP_TILE = DUP_THREADS * DUP_ITEMS;     // 2048 duplicated entries
 // arrays that follow it) by one cudaMemsetAsync per frame.
 struct Ctrl {
     uint32_t tile_counter[16];          // dynamic tile ids of the chained-scan kernels (forward-progress order)
-    unsigned long long n_vis;           // visible Gaussians (compacted count)
+    unsigned long long n_vis;           // visible Gaussians
+    unsigned long long n_sort;          // keys the depth sort runs over: n_vis (compacted) or P (small scenes)
     unsigned long long overflow;        // 1 if n_dup > max_dup
     unsigned long long n_dup;           // duplicates the frame needs
     unsigned long long n_dup_eff;       // duplicates actually produced (0 on overflow)
@@ -43,6 +45,8 @@ constexpr unsigned long long ST_MASK = (1ull << 62) - 1;
 struct Frame {              // per-frame constants, passed by value to the kernels
     int P, W, H, gx, gy, n_tiles, deg, K;
     int tile_bits, n_tile_passes;
+    int compact;                // 1: preprocess compacts the visible Gaussians (P >= COMPACT_MIN_P)
+    int diff_copies, diff_cells; // replicas of the coverage difference grid (power of two) and cells per replica
     float V[16], PM[16];
     float fx, fy;
     float campos[3];
@@ -52,7 +56,7 @@ struct Frame {              // per-frame constants, passed by value to the kerne
 
 struct Pointers {           // device pointers carved from the workspace
     Ctrl* ctrl;
-    int* diff;                              // [(gy+1)*(gx+1)] 2-D difference grid of tile coverage
+    int* diff;                              // [diff_copies][(gy+1)*(gx+1)] 2-D difference grid of tile coverage
     unsigned long long* st_pre;             // [pre tiles]    look-back status: compaction of visible Gaussians
     unsigned long long* st_scan;            // [scan tiles]   look-back status: duplicate offsets
     unsigned long long* st_depth;           // [4][depth sort tiles][256]

@@ -122,13 +122,10 @@ __device__ __forceinline__ bool project(const Frame& f, float px, float py, floa
 // ("view-dependent color parameterized by spherical harmonics"; reading S8).  DEG is a template parameter
 // so that the basis lives in registers (a runtime degree indexes the array dynamically and spills it to local memory).
 template <int DEG>
-__device__ __forceinline__ float3 sh_colour(const Frame& f, const float* __restrict__ sh, int i, float px, float py,
-                                            float pz) {
-    constexpr int K = (DEG + 1) * (DEG + 1);
+__device__ __forceinline__ void sh_basis(const Frame& f, float px, float py, float pz, float* Y) {
     float x = px - f.campos[0], y = py - f.campos[1], z = pz - f.campos[2];
     const float rn = rsqrtf(x * x + y * y + z * z);
     x *= rn; y *= rn; z *= rn;
-    float Y[K];
     Y[0] = 0.28209479177387814f;
     if (DEG >= 1) {
         Y[1] = -0.4886025119029199f * y;
@@ -152,8 +149,17 @@ __device__ __forceinline__ float3 sh_colour(const Frame& f, const float* __restr
             Y[15] = -0.5900435899266435f * x * (xx - 3.0f * yy);
         }
     }
+}
+
+// The lane reads its own coefficients (3, 12, 27 or 48 floats; 16-byte loads where the count allows).
+template <int DEG>
+__device__ __forceinline__ float3 sh_colour_direct(const Frame& f, const float* __restrict__ sh, int i, float px, float py,
+                                                   float pz) {
+    constexpr int K = (DEG + 1) * (DEG + 1);
+    float Y[K];
+    sh_basis<DEG>(f, px, py, pz, Y);
     float c[3 * K];
-    if (K % 4 == 0) {  // degrees 1 and 3: 12 / 48 floats = 3 / 12 aligned float4 per Gaussian
+    if (K % 4 == 0) {
         const float4* s4 = reinterpret_cast<const float4*>(sh + (size_t)i * (3 * K));
 #pragma unroll
         for (int k = 0; k < 3 * K / 4; k++) {
@@ -173,85 +179,114 @@ __device__ __forceinline__ float3 sh_colour(const Frame& f, const float* __restr
     return make_float3(fmaxf(r, 0.0f), fmaxf(g, 0.0f), fmaxf(b, 0.0f));
 }
 
-// One WARP is the unit of the order-preserving compaction: it takes one 32-Gaussian sub-tile per atomic ticket,
-// publishes the sub-tile's count of visible Gaussians at once, does all the heavy work (SH colour, records, coverage
-// grid, histograms), and only then looks back for its exclusive prefix -- by which time the predecessors have long
-// published.  There is no block barrier inside the loop.  (Several sub-tiles per ticket would serialise the warps:
-// the count of a later sub-tile is only known when its owner reaches it.)
-template <int DEG>
+// One WARP processes one 32-Gaussian sub-tile at a time; there is no block barrier inside the loop.
+//
+// COMPACT = true (large scenes): order-preserving compaction of the visible Gaussians.  The warp takes a sub-tile per
+//   atomic ticket, publishes the sub-tile's count of visible Gaussians at once, does all the heavy work (SH colour,
+//   records, coverage grid, histograms), and only then looks back for its exclusive prefix -- by which time the
+//   predecessors have long published.
+// COMPACT = false (small scenes, one wave of warps): a single wave gives the look-back nothing to overlap with -- the
+//   inclusive prefixes advance 32 sub-tiles per L2 round trip, ~25 us for 100 000 Gaussians -- so nothing is
+//   compacted: every Gaussian writes a key, culled ones the all-ones key that sorts behind every depth, and the depth
+//   sort runs over all P keys.  Sub-tiles are assigned statically; there is no inter-warp dependency at all.
+template <int DEG, bool COMPACT>
 __global__ void __launch_bounds__(PRE_THREADS)
 preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ means, const float* __restrict__ scales,
                   const float* __restrict__ rots, const float* __restrict__ opac, const float* __restrict__ sh) {
     __shared__ uint32_t s_hist[MAX_SORT_PASSES_DEPTH][256];
+    __shared__ uint32_t s_nvis;
     const int tid = threadIdx.x, lane = tid & 31;
     for (int k = tid; k < MAX_SORT_PASSES_DEPTH * 256; k += PRE_THREADS) (&s_hist[0][0])[k] = 0;
+    if (tid == 0) s_nvis = 0;
     __syncthreads();
     const int n_tiles = (f.P + 31) / 32;
     const int gw = f.gx + 1;
     const unsigned lt = (1u << lane) - 1u;
+    const int gwarp = blockIdx.x * (PRE_THREADS / 32) + (tid >> 5), n_warps = gridDim.x * (PRE_THREADS / 32);
+    // coverage grid copy of this warp: the corner counters of a small grid are hot (hundreds of atomics per address,
+    // serialised in L2), so they are spread over diff_copies replicas that tile_grid_kernel adds up
+    int* diff = p.diff + (size_t)(gwarp & (f.diff_copies - 1)) * f.diff_cells;
+    int tile = gwarp;
     while (true) {
-        int tile = 0;
-        if (lane == 0) tile = (int)atomicAdd(&p.ctrl->tile_counter[TC_PRE], 1u);
-        tile = __shfl_sync(0xffffffffu, tile, 0);
+        if (COMPACT) {
+            if (lane == 0) tile = (int)atomicAdd(&p.ctrl->tile_counter[TC_PRE], 1u);
+            tile = __shfl_sync(0xffffffffu, tile, 0);
+        }
         if (tile >= n_tiles) break;
-        {
-            const int i = tile * 32 + lane;
-            Splat s = {};
-            bool vis = false;
-            float px = 0.f, py = 0.f, pz = 0.f;
-            if (i < f.P) {
-                // plain loads: the three components of a lane share their cache lines with the neighbouring lanes
-                px = __ldg(means + 3 * (size_t)i); py = __ldg(means + 3 * (size_t)i + 1); pz = __ldg(means + 3 * (size_t)i + 2);
-                const float sx = __ldg(scales + 3 * (size_t)i), sy = __ldg(scales + 3 * (size_t)i + 1), sz = __ldg(scales + 3 * (size_t)i + 2);
-                const float4 q = __ldcs(reinterpret_cast<const float4*>(rots) + i);
-                vis = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, s);
-            }
-            const unsigned vb = __ballot_sync(0xffffffffu, vis);
-            const uint32_t cnt = __popc(vb);
+        const int i = tile * 32 + lane;
+        Splat s = {};
+        bool vis = false;
+        float px = 0.f, py = 0.f, pz = 0.f;
+        if (i < f.P) {
+            // plain loads: the three components of a lane share their cache lines with the neighbouring lanes
+            px = __ldg(means + 3 * (size_t)i); py = __ldg(means + 3 * (size_t)i + 1); pz = __ldg(means + 3 * (size_t)i + 2);
+            const float sx = __ldg(scales + 3 * (size_t)i), sy = __ldg(scales + 3 * (size_t)i + 1), sz = __ldg(scales + 3 * (size_t)i + 2);
+            const float4 q = __ldcs(reinterpret_cast<const float4*>(rots) + i);
+            vis = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, s);
+        }
+        const unsigned vb = __ballot_sync(0xffffffffu, vis);
+        const uint32_t cnt = __popc(vb);
+        if (COMPACT) {
             if (lane == 0) st_status(p.st_pre + tile, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)cnt);
-            // ---- everything that does not need the compact index ----------------------------------------------
-            if (i < f.P) {
-                uint4 pg = make_uint4(0u, 0u, 0u, 0u);
-                if (vis) {
-                    pg.x = (uint32_t)s.xmin | ((uint32_t)s.ymin << 16);
-                    pg.y = (uint32_t)s.xmax | ((uint32_t)s.ymax << 16);
-                    pg.z = __float_as_uint(s.depth);
-                    pg.w = (uint32_t)s.radius;
-                }
-                p.per_g[i] = pg;
-            }
+        } else if (lane == 0 && cnt) {
+            atomicAdd(&s_nvis, cnt);
+        }
+        // ---- everything that does not need the compact index --------------------------------------------------
+        if (i < f.P) {
+            uint4 pg = make_uint4(0u, 0u, 0u, 0u);
             if (vis) {
-                atomicAdd(p.diff + s.ymin * gw + s.xmin, 1);
-                atomicAdd(p.diff + s.ymin * gw + s.xmax, -1);
-                atomicAdd(p.diff + s.ymax * gw + s.xmin, -1);
-                atomicAdd(p.diff + s.ymax * gw + s.xmax, 1);
+                pg.x = (uint32_t)s.xmin | ((uint32_t)s.ymin << 16);
+                pg.y = (uint32_t)s.xmax | ((uint32_t)s.ymax << 16);
+                pg.z = __float_as_uint(s.depth);
+                pg.w = (uint32_t)s.radius;
+            }
+            p.per_g[i] = pg;
+            if (!COMPACT) {  // a culled Gaussian sorts behind every depth: digit 255 in all four passes
+                const uint32_t db = vis ? __float_as_uint(s.depth) : 0xffffffffu;
+                atomicAdd(&s_hist[0][db & 255u], 1u);
+                atomicAdd(&s_hist[1][(db >> 8) & 255u], 1u);
+                atomicAdd(&s_hist[2][(db >> 16) & 255u], 1u);
+                atomicAdd(&s_hist[3][db >> 24], 1u);
+                p.gkeyA[i] = vis ? (((unsigned long long)db << 32) | (unsigned)i) : ~0ull;
+            }
+        }
+        if (vis) {
+            atomicAdd(diff + s.ymin * gw + s.xmin, 1);
+            atomicAdd(diff + s.ymin * gw + s.xmax, -1);
+            atomicAdd(diff + s.ymax * gw + s.xmin, -1);
+            atomicAdd(diff + s.ymax * gw + s.xmax, 1);
+            if (COMPACT) {
                 const uint32_t db = __float_as_uint(s.depth);
                 atomicAdd(&s_hist[0][db & 255u], 1u);
                 atomicAdd(&s_hist[1][(db >> 8) & 255u], 1u);
                 atomicAdd(&s_hist[2][(db >> 16) & 255u], 1u);
                 atomicAdd(&s_hist[3][db >> 24], 1u);
-                const float o = __ldcs(opac + i);
-                const float3 col = sh_colour<DEG>(f, sh, i, px, py, pz);
-                // det of the STORED conic, exact products in double (24+24 bits): the form is indefinite iff det <= 0,
-                // and the tight box of the render stage needs det without fp32 cancellation (needle-like splats)
-                const double dd = (double)s.ca * (double)s.cc - (double)s.cb * (double)s.cb;
-                const float l2o = log2f(o);
-                const TightBox tb = tight_box_constants(s.ca, s.cb, s.cc, (float)dd, l2o);
-                const uint32_t flags = (!(dd > 0.0) || tb.degenerate) ? 1u : 0u;
-                float4* rec = p.rec + 4 * (size_t)i;  // 64-byte render record (include/gs.h: gs_intermediates.record)
-                rec[0] = make_float4(s.mux, s.muy, s.ca, s.cb);
-                rec[1] = make_float4(s.cc, l2o, (float)dd, __uint_as_float(flags));
-                rec[2] = make_float4(col.x, col.y, col.z, tb.xstar);
-                rec[3] = make_float4(tb.ic, tb.ct, 0.0f, 0.0f);
             }
-            // ---- exclusive prefix: own chunk's running total, else decoupled look-back ("prefix scan") ----
+            const float o = __ldcs(opac + i);
+            const float3 col = sh_colour_direct<DEG>(f, sh, i, px, py, pz);
+            // det of the STORED conic, exact products in double (24+24 bits): the form is indefinite iff det <= 0,
+            // and the tight box of the render stage needs det without fp32 cancellation (needle-like splats)
+            const double dd = (double)s.ca * (double)s.cc - (double)s.cb * (double)s.cb;
+            const float l2o = log2f(o);
+            const TightBox tb = tight_box_constants(s.ca, s.cb, s.cc, (float)dd, l2o);
+            const uint32_t flags = (!(dd > 0.0) || tb.degenerate) ? 1u : 0u;
+            float4* rec = p.rec + 4 * (size_t)i;  // 64-byte render record (include/gs.h: gs_intermediates.record)
+            rec[0] = make_float4(s.mux, s.muy, s.ca, s.cb);
+            rec[1] = make_float4(s.cc, l2o, (float)dd, __uint_as_float(flags));
+            rec[2] = make_float4(col.x, col.y, col.z, tb.xstar);
+            rec[3] = make_float4(tb.ic, tb.ct, 0.0f, 0.0f);
+        }
+        if (COMPACT) {
+            // ---- exclusive prefix by decoupled look-back ("parallel prefix scan") ------------------
             const unsigned long long excl = tile > 0 ? lookback_warp(p.st_pre, tile) : 0ull;
             const unsigned long long run = excl + cnt;
             if (lane == 0) {
                 st_status(p.st_pre + tile, ST_INC | run);
-                if (tile == n_tiles - 1) p.ctrl->n_vis = run;
+                if (tile == n_tiles - 1) { p.ctrl->n_vis = run; p.ctrl->n_sort = run; }
             }
             if (vis) p.gkeyA[excl + __popc(vb & lt)] = ((unsigned long long)__float_as_uint(s.depth) << 32) | (unsigned)i;
+        } else {
+            tile += n_warps;
         }
     }
     __syncthreads();
@@ -259,6 +294,17 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
         const uint32_t c = (&s_hist[0][0])[k];
         if (c) atomicAdd(&p.ctrl->depth_hist[0][0] + k, c);
     }
+    if (!COMPACT && tid == 0) {
+        if (s_nvis) atomicAdd(&p.ctrl->n_vis, (unsigned long long)s_nvis);
+        if (blockIdx.x == 0) p.ctrl->n_sort = (unsigned long long)f.P;
+    }
+}
+
+template <int DEG>
+static void launch_pre(const Frame& f, const Pointers& p, const float* means, const float* scales, const float* rots,
+                       const float* opac, const float* sh, int grid, cudaStream_t st) {
+    if (f.compact) preprocess_kernel<DEG, true><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh);
+    else preprocess_kernel<DEG, false><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh);
 }
 
 void launch_preprocess(const Frame& f, const Pointers& p, const float* means, const float* scales, const float* rots,
@@ -266,10 +312,10 @@ void launch_preprocess(const Frame& f, const Pointers& p, const float* means, co
     const long long warps = ((long long)f.P + 31) / 32, blocks = (warps + PRE_THREADS / 32 - 1) / (PRE_THREADS / 32);
     const int grid = (int)(blocks < 1 ? 1 : (blocks < (long long)n_sm * 8 ? blocks : (long long)n_sm * 8));
     switch (f.deg) {
-        case 0: preprocess_kernel<0><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh); break;
-        case 1: preprocess_kernel<1><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh); break;
-        case 2: preprocess_kernel<2><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh); break;
-        default: preprocess_kernel<3><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh); break;
+        case 0: launch_pre<0>(f, p, means, scales, rots, opac, sh, grid, st); break;
+        case 1: launch_pre<1>(f, p, means, scales, rots, opac, sh, grid, st); break;
+        case 2: launch_pre<2>(f, p, means, scales, rots, opac, sh, grid, st); break;
+        default: launch_pre<3>(f, p, means, scales, rots, opac, sh, grid, st); break;
     }
 }
 

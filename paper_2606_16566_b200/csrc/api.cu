@@ -4,12 +4,14 @@
 
 #include <atomic>
 #include <cstdio>
+#include <cstdlib>
 #include <map>
 #include <mutex>
 
 #include "common.cuh"
 
 namespace gs {
+int g_use_pdl = 1;
 void launch_preprocess(const Frame&, const Pointers&, const float*, const float*, const float*, const float*, const float*,
                        int, cudaStream_t);
 void launch_depth_sort(const Frame&, const Pointers&, int, cudaStream_t, int*);
@@ -128,7 +130,7 @@ Pointers carve(void* ws, const Layout& L) {
 bool fit_max_dup(int P, int W, int H, size_t bytes, unsigned long long& max_dup) {
     Layout L;
     if (!make_layout(P, W, H, 0, L) || L.total > bytes) return false;
-    const unsigned long long edge = 4ull << 20;  // sort_items_for: capacity <= edge -> small tiles
+    const unsigned long long edge = 256ull << 10;  // sort_items_for: capacity <= edge -> small tiles
     const unsigned long long lo_of[2] = {edge + 1, 0}, hi_of[2] = {(1ull << 32) - 1, edge};
     for (int r = 0; r < 2; r++) {
         unsigned long long lo = lo_of[r], hi = hi_of[r];
@@ -221,6 +223,13 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     auto mark = [&](int k) { if (timed) cudaEventRecord(lc->ev[k], st); };
 #endif
 
+    // PDL hides launch latency between the 11 kernels of a small frame; large frames (kernels of 100+ us) gain nothing
+    // and lose a little to early-resident dependents, so they launch plainly.  GS_PDL=0/1 overrides (experiments).
+    {
+        static const char* env = getenv("GS_PDL");
+        g_use_pdl = env ? (env[0] == '1') : (P <= (1 << 21) && max_dup <= (1ull << 25));
+        if (timed) g_use_pdl = 0;
+    }
     int launches = 0;
     mark(0);
     cudaError_t e = cudaMemsetAsync(workspace, 0, L.zero_end, st);

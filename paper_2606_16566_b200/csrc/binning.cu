@@ -31,7 +31,7 @@ namespace gs {
 // (profiles/r01_microbench.md) -- the match-based first version of this kernel spent 35 % of its stall samples there.
 // ------------------------------------------------------------------------------------------------------------
 template <int ITEMS, bool OUT32>
-__global__ void __launch_bounds__(SORT_THREADS, (ITEMS >= 16 ? 4 : 6))
+__global__ void __launch_bounds__(SORT_THREADS, 4)
 radix_pass_kernel(const unsigned long long* __restrict__ in, unsigned long long* __restrict__ out,
                   uint32_t* __restrict__ out32, const unsigned long long* __restrict__ n_ptr, int shift,
                   const uint32_t* __restrict__ ghist, unsigned long long* __restrict__ status,
@@ -45,6 +45,7 @@ radix_pass_kernel(const unsigned long long* __restrict__ in, unsigned long long*
     __shared__ uint32_t s_gpos[256];
     __shared__ uint32_t s_scan[NW];
     __shared__ int s_tile;
+    griddep_sync();
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const unsigned long long n = *n_ptr;
     {   // exclusive scan of the global digit histogram -> first output slot of every digit
@@ -111,14 +112,24 @@ radix_pass_kernel(const unsigned long long* __restrict__ in, unsigned long long*
                 s_sorted[s_bpos[d] + s_hist[w][d] + ((rk2[j / 2] >> (16 * (j & 1))) & 0xffffu)] = key[j];
             }
         }
-        // ---- decoupled look-back for digit `tid`, LB_WINDOW predecessors per round trip --------------------------
-        // (in the first wave every resident tile only has its aggregate published, so the walk back to an inclusive
-        // prefix is hundreds of tiles long: several status words in flight per step divide that latency chain)
+        // ---- decoupled look-back for digit `tid` ------------------------------------------------------------
+        // Steady state (many waves of tiles): the direct predecessor already holds its inclusive prefix -- one load.
+        // First wave (or a sort that fits in one wave): every resident tile only has its aggregate published, and the
+        // inclusive prefixes advance a few tiles per L2 round trip; LB_WINDOW status words in flight per step divide
+        // that latency chain (it was 20-30 % of the stall samples of the depth passes with a window of one).
         unsigned long long excl = 0;
         if (tile > 0) {
-            constexpr int LB_WINDOW = 4;
+            constexpr int LB_WINDOW = 16;
             int idx = tile - 1;
             bool done = false;
+            {
+                const unsigned long long s0 = ld_status(status + (size_t)idx * 256 + tid);
+                if ((s0 >> 62) != 0) {
+                    excl = s0 & ST_MASK;
+                    idx--;
+                    done = (s0 >> 62) == 2 || idx < 0;
+                }
+            }
             while (!done) {
                 unsigned long long sv[LB_WINDOW];
 #pragma unroll
@@ -161,6 +172,7 @@ tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts 
     __shared__ uint32_t s_hist[MAX_SORT_PASSES_TILE][256];
     __shared__ unsigned long long s_part[GRID_THREADS / 32];
     __shared__ unsigned long long s_total;
+    griddep_sync();
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int gw = f.gx + 1, gh = f.gy + 1;
     int* diff = p.diff;
@@ -249,6 +261,7 @@ __device__ __forceinline__ uint32_t rect_tiles(const uint4 pg) {
 // barrier.  The rect of every rank is gathered once here and stored in depth order for the duplicate kernel.
 __global__ void __launch_bounds__(SCAN_THREADS)
 scan_offsets_kernel(const Pointers p) {
+    griddep_sync();
     const int lane = threadIdx.x & 31;
     const unsigned long long n = p.ctrl->n_vis;
     if (p.ctrl->overflow != 0) return;
@@ -337,6 +350,7 @@ duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict
     __shared__ uint32_t s_off[DUP_TILE + 2];
     __shared__ uint2 s_rect[DUP_TILE + 2];
     __shared__ uint32_t s_id[DUP_TILE + 2];
+    griddep_sync();
     const int tid = threadIdx.x;
     const unsigned long long n = p.ctrl->n_dup_eff;
     const uint32_t n_vis = (uint32_t)p.ctrl->n_vis;
@@ -418,10 +432,10 @@ static void launch_pass(int items, int n_sm, unsigned long long capacity, const 
     const long long cap_tiles = ((long long)capacity + tile_n - 1) / tile_n;
     if (items == 16) {
         const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
-        radix_pass_kernel<16, OUT32><<<grid, SORT_THREADS, 0, st>>>(in, out, out32, n_ptr, shift, ghist, status, tile_counter);
+        launch_pdl(radix_pass_kernel<16, OUT32>, dim3(grid), dim3(SORT_THREADS), st, in, out, out32, n_ptr, shift, ghist, status, tile_counter);
     } else {
-        const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 6);
-        radix_pass_kernel<4, OUT32><<<grid, SORT_THREADS, 0, st>>>(in, out, out32, n_ptr, shift, ghist, status, tile_counter);
+        const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
+        launch_pdl(radix_pass_kernel<4, OUT32>, dim3(grid), dim3(SORT_THREADS), st, in, out, out32, n_ptr, shift, ghist, status, tile_counter);
     }
 }
 
@@ -437,14 +451,14 @@ void launch_depth_sort(const Frame& f, const Pointers& p, int n_sm, cudaStream_t
 }
 
 void launch_tile_grid(const Frame& f, const Pointers& p, uint32_t* out_tile_counts, cudaStream_t st, int* launches) {
-    tile_grid_kernel<<<1, GRID_THREADS, 0, st>>>(f, p, out_tile_counts);
+    launch_pdl(tile_grid_kernel, dim3(1), dim3(GRID_THREADS), st, f, p, out_tile_counts);
     (*launches)++;
 }
 
 void launch_scan_offsets(const Frame& f, const Pointers& p, int n_sm, cudaStream_t st, int* launches) {
     const long long cap_blocks = ((long long)f.P + SCAN_WARP_TILE * (SCAN_THREADS / 32) - 1) / (SCAN_WARP_TILE * (SCAN_THREADS / 32));
     const int grid = imin(cap_blocks > 0 ? cap_blocks : 1, (long long)n_sm * 8);
-    scan_offsets_kernel<<<grid, SCAN_THREADS, 0, st>>>(p);
+    launch_pdl(scan_offsets_kernel, dim3(grid), dim3(SCAN_THREADS), st, p);
     (*launches)++;
 }
 
@@ -453,7 +467,7 @@ void launch_duplicate_and_tile_sort(const Frame& f, const Pointers& p, int n_sm,
                                     cudaEvent_t ev_after_duplicate) {
     const long long cap_chunks = ((long long)f.max_dup + DUP_TILE - 1) / DUP_TILE;
     const int dgrid = imin(cap_chunks > 0 ? cap_chunks : 1, (long long)n_sm * 8);
-    duplicate_kernel<<<dgrid, DUP_THREADS, 0, st>>>(f, p, p.entA);
+    launch_pdl(duplicate_kernel, dim3(dgrid), dim3(DUP_THREADS), st, f, p, p.entA);
     (*launches)++;
     if (ev_after_duplicate) cudaEventRecord(ev_after_duplicate, st);
     unsigned long long* bufs[2] = {p.entA, p.entB};

@@ -195,6 +195,7 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
                   const float* __restrict__ rots, const float* __restrict__ opac, const float* __restrict__ sh) {
     __shared__ uint32_t s_hist[MAX_SORT_PASSES_DEPTH][256];
     __shared__ uint32_t s_nvis;
+    griddep_sync();
     const int tid = threadIdx.x, lane = tid & 31;
     for (int k = tid; k < MAX_SORT_PASSES_DEPTH * 256; k += PRE_THREADS) (&s_hist[0][0])[k] = 0;
     if (tid == 0) s_nvis = 0;
@@ -303,8 +304,8 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
 template <int DEG>
 static void launch_pre(const Frame& f, const Pointers& p, const float* means, const float* scales, const float* rots,
                        const float* opac, const float* sh, int grid, cudaStream_t st) {
-    if (f.compact) preprocess_kernel<DEG, true><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh);
-    else preprocess_kernel<DEG, false><<<grid, PRE_THREADS, 0, st>>>(f, p, means, scales, rots, opac, sh);
+    if (f.compact) launch_pdl(preprocess_kernel<DEG, true>, dim3(grid), dim3(PRE_THREADS), st, f, p, means, scales, rots, opac, sh);
+    else launch_pdl(preprocess_kernel<DEG, false>, dim3(grid), dim3(PRE_THREADS), st, f, p, means, scales, rots, opac, sh);
 }
 
 void launch_preprocess(const Frame& f, const Pointers& p, const float* means, const float* scales, const float* rots,

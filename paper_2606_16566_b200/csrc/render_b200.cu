@@ -179,6 +179,7 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint32_t* __res
     __shared__ __align__(16) uint32_t s_ball[2][4][4];          // [buffer][staging warp][quadrant] mask ballots
     __shared__ __align__(16) uint32_t s_indef[2][4];                        // [buffer][staging warp] batch holds an indefinite conic
     __shared__ __align__(16) uint32_t s_list[4][QB + 2];        // per-warp compacted lists of record addresses (padded to even length)
+    griddep_sync();
     const int tid = threadIdx.x, lane = tid & 31;
     // warp index through a warp reduction: ptxas then KNOWS it is warp-uniform (it lives in a uniform register), so
     // every trip count derived from it is uniform and the votes of the blend loop need no divergence guard
@@ -324,11 +325,11 @@ void launch_render_b200(const Frame& f, const Pointers& p, float* out_rgb, float
     (void)n_sm;
     const dim3 grid(f.gx, f.gy), block(QB);
     if (stats && out_n)
-        render_b200_kernel<true, true><<<grid, block, 0, st>>>(f, p.ctrl, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n);
+        launch_pdl(render_b200_kernel<true, true>, grid, block, st, f, p.ctrl, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n);
     else if (out_n)
-        render_b200_kernel<true, false><<<grid, block, 0, st>>>(f, p.ctrl, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n);
+        launch_pdl(render_b200_kernel<true, false>, grid, block, st, f, p.ctrl, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n);
     else
-        render_b200_kernel<false, false><<<grid, block, 0, st>>>(f, p.ctrl, p.ranges, p.ids, p.rec, out_rgb, out_T, nullptr);
+        launch_pdl(render_b200_kernel<false, false>, grid, block, st, f, p.ctrl, p.ranges, p.ids, p.rec, out_rgb, out_T, (uint32_t*)nullptr);
 }
 
 }  // namespace gs

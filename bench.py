@@ -171,6 +171,8 @@ def run_ours(args):
     if ws > 1:
         dist.init_process_group("nccl", device_id=dev)
     binding.lib()  # raises if libgs.so is missing and cannot be built
+    if args.render_variant is not None:
+        binding.gs_set_render_variant(args.render_variant)
     peaks = _peaks()
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
 
@@ -374,6 +376,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=(1, 2, 3, 4, 5))
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

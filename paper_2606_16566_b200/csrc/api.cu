@@ -21,6 +21,7 @@ void launch_duplicate_and_tile_sort(const Frame&, const Pointers&, int, cudaStre
 void launch_atomic_order_selftest(unsigned long long*, int, uint32_t, int, int, cudaStream_t);
 void launch_render_ladder(int, const Frame&, const Pointers&, float*, float*, uint32_t*, cudaStream_t);
 void launch_render_b200(const Frame&, const Pointers&, float*, float*, uint32_t*, int, bool, cudaStream_t);
+void launch_render_ws(const Frame&, const Pointers&, float*, float*, uint32_t*, int, bool, cudaStream_t);
 }  // namespace gs
 
 namespace {
@@ -31,7 +32,7 @@ size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
     size_t ctrl, diff, st_pre, st_scan, st_depth, st_tile, zero_end;
-    size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, entA, entB, ids, total;
+    size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, desc, entA, entB, ids, total;
     size_t n_depth_tiles, n_tile_tiles;
     int gx, gy, n_tiles, tile_bits, n_tile_passes, diff_copies, diff_cells;
 };
@@ -70,6 +71,7 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     L.rk_rect = take(8 * Pz);
     L.chunk_start = take(4 * (((size_t)max_dup + DUP_TILE - 1) / DUP_TILE + 2));
     L.ranges = take(4 * ((size_t)L.n_tiles + 1));
+    L.desc = take(16 * (size_t)L.n_tiles);
     L.entA = take(8 * (size_t)max_dup);
     L.entB = take(L.n_tile_passes >= 2 ? 8 * (size_t)max_dup : 0);
     L.ids = take(4 * (size_t)max_dup + 16);
@@ -116,6 +118,7 @@ Pointers carve(void* ws, const Layout& L) {
     p.rk_rect = reinterpret_cast<uint2*>(b + L.rk_rect);
     p.chunk_start = reinterpret_cast<uint32_t*>(b + L.chunk_start);
     p.ranges = reinterpret_cast<uint32_t*>(b + L.ranges);
+    p.desc = reinterpret_cast<uint4*>(b + L.desc);
     p.entA = reinterpret_cast<unsigned long long*>(b + L.entA);
     p.entB = reinterpret_cast<unsigned long long*>(b + L.entB);
     p.ids = reinterpret_cast<uint32_t*>(b + L.ids);
@@ -258,7 +261,8 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     launch_duplicate_and_tile_sort(f, p, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b)
     mark(6);
     const int variant = g_variant.load();                      // (4) render
-    if (variant >= 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
+    if (variant >= 5) launch_render_ws(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
+    else if (variant == 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
     else launch_render_ladder(variant, f, p, out_rgb, out_final_T, out_n_contrib, st);
     launches++;
     mark(7);
@@ -383,7 +387,7 @@ int gs_copy_to_host(void* dst_host, const void* src_dev, size_t bytes) {
 }
 
 int gs_set_render_variant(int variant) {
-    if (variant < 0 || variant > 4) return GS_ERR_BAD_ARG;
+    if (variant < 0 || variant > 5) return GS_ERR_BAD_ARG;
     g_variant.store(variant);
     return GS_OK;
 }

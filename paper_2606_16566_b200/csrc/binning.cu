@@ -167,16 +167,26 @@ radix_pass_kernel(const unsigned long long* __restrict__ in, unsigned long long*
 // digit histograms of the tile ids for the tile radix passes.  One block (the grid has <= 2^24 cells).
 // ------------------------------------------------------------------------------------------------------------
 constexpr int GRID_THREADS = 1024;
+// 257 buckets of list length: 0, then 8 sub-steps per power of two -- a coarse descending sort key
+constexpr int LPT_BUCKETS = 257;
+__device__ __forceinline__ int lpt_bucket(uint32_t c) {
+    if (c == 0) return 0;
+    const int l = 31 - __clz(c);
+    const uint32_t frac = l >= 3 ? (c >> (l - 3)) & 7u : (c << (3 - l)) & 7u;
+    return 1 + l * 8 + (int)frac;
+}
 __global__ void __launch_bounds__(GRID_THREADS)
 tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts /* out_tile_counts */) {
     __shared__ uint32_t s_hist[MAX_SORT_PASSES_TILE][256];
     __shared__ unsigned long long s_part[GRID_THREADS / 32];
     __shared__ unsigned long long s_total;
+    __shared__ uint32_t s_bucket[LPT_BUCKETS];
     griddep_sync();
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int gw = f.gx + 1, gh = f.gy + 1;
     int* diff = p.diff;
     for (int k = tid; k < MAX_SORT_PASSES_TILE * 256; k += GRID_THREADS) (&s_hist[0][0])[k] = 0;
+    for (int k = tid; k < LPT_BUCKETS; k += GRID_THREADS) s_bucket[k] = 0;
     // row-wise inclusive prefix, one warp per row, in place
     for (int y = w; y < gh; y += GRID_THREADS / 32) {
         int carry = 0;
@@ -210,7 +220,11 @@ tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts 
     const int per = (f.n_tiles + GRID_THREADS - 1) / GRID_THREADS;
     const int t0 = min(f.n_tiles, tid * per), t1 = min(f.n_tiles, t0 + per);
     unsigned long long sum = 0;
-    for (int t = t0; t < t1; t++) sum += counts[t];
+    for (int t = t0; t < t1; t++) {
+        const uint32_t c = counts[t];
+        sum += c;
+        atomicAdd(&s_bucket[lpt_bucket(c)], 1u);
+    }
     unsigned long long inc = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -224,6 +238,10 @@ tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts 
         for (int k = 0; k < GRID_THREADS / 32; k++) { const unsigned long long t = s_part[k]; s_part[k] = c; c += t; }
         s_total = c;
     }
+    if (tid == 32) {   // first descriptor slot of every bucket, LONGEST lists first
+        uint32_t c = 0;
+        for (int k = LPT_BUCKETS - 1; k >= 0; k--) { const uint32_t t = s_bucket[k]; s_bucket[k] = c; c += t; }
+    }
     __syncthreads();
     const unsigned long long total = s_total;
     const bool overflow = total > f.max_dup;
@@ -231,6 +249,11 @@ tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts 
     for (int t = t0; t < t1; t++) {
         const uint32_t c = counts[t];
         p.ranges[t] = overflow ? 0u : (uint32_t)run;
+        {   // tile descriptor in longest-processing-time-first order (the order inside a bucket is arbitrary: it only
+            // changes which persistent render CTA takes the tile, never a result)
+            const uint32_t slot = atomicAdd(&s_bucket[lpt_bucket(c)], 1u);
+            p.desc[slot] = overflow ? make_uint4((uint32_t)t, 0u, 0u, 0u) : make_uint4((uint32_t)t, (uint32_t)run, (uint32_t)(run + c), 0u);
+        }
         run += c;
         if (!overflow && c) {
 #pragma unroll

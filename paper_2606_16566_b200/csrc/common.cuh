@@ -69,6 +69,7 @@ struct Pointers {           // device pointers carved from the workspace
     uint2* rk_rect;                         // [P] tile rect {xmin | ymin<<16, xmax | ymax<<16} in depth order
     uint32_t* chunk_start;                  // [ceil(max_dup / DUP_TILE) + 1] depth rank owning entry c * DUP_TILE
     uint32_t* ranges;                       // [n_tiles + 1]
+    uint4* desc;                            // [n_tiles] {tile, start, end, -}: tiles by descending list length (render schedule)
     unsigned long long* entA;               // [max_dup] (tile << 32 | id)
     unsigned long long* entB;               // [max_dup] ping-pong
     uint32_t* ids;                          // [max_dup] final sorted Gaussian ids

@@ -320,6 +320,395 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint32_t* __res
     }
 }
 
+// ====================================================================================================================
+// Variant 5: the same blend loop, warp-specialised and persistent.
+//
+//   * 192 threads per CTA: 4 CONSUMER warps (one 8x8 quadrant of the current tile each, running blend_list above) and
+//     2 PRODUCER warps that do all the staging (gather, tight box -> quadrant masks, double-precision hoist, per-quadrant
+//     compacted lists).  Staging costs a quarter of the instructions of the kernel and all of its global-memory
+//     latency; on its own warps it overlaps the blend instead of preceding it.
+//   * a ring of NSTAGE stages of 64 list entries in shared memory, handed over with mbarriers (full: 64 producer
+//     arrivals, empty: 4 consumer-warp arrivals) -- no CTA-wide barrier anywhere; a consumer warp is never held back by
+//     a slower quadrant inside a tile, only by the ring depth.
+//   * persistent CTAs walk a STATIC tile schedule in longest-list-first order (tile descriptors written by
+//     tile_grid_kernel): CTA c takes descriptors c, c + G, c + 2G, ...  No tail of a few long tiles at the end of the
+//     launch, and the next tile is known in advance: its descriptor, first ids and first records are prefetched while
+//     the current tile is staged, so a tile switch costs no global round trip.
+//   * termination (Eq. 22): a consumer warp whose 64 pixels are finished reports to a per-tile counter; when all four
+//     have, the producers abandon the tile (at most NSTAGE - 1 staged batches are wasted) and the consumers skip
+//     whatever stale stages of it remain.
+// ====================================================================================================================
+constexpr int WS_SB = 64;            // list entries per stage
+constexpr int WS_NSTAGE = 3;
+constexpr int WS_THREADS = 192;      // 4 consumer warps + 2 producer warps
+constexpr uint32_t WS_FIRST = 1u, WS_LAST = 2u, WS_EXIT = 4u, WS_INDEF = 8u;
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+
+struct WsShared {
+    __align__(16) unsigned char rec[WS_NSTAGE][WS_SB * REC];  // staged, hoisted records
+    __align__(16) unsigned char null_rec[REC];                // F = -huge: alpha = 0 exactly (list padding)
+    __align__(16) uint32_t list[WS_NSTAGE][4][WS_SB + 2];     // per stage, per quadrant: record addresses, in list order
+    __align__(16) uint4 hdr[WS_NSTAGE];                       // {flags, tile, tile sequence number, 4 x 8-bit list lengths}
+    __align__(8) unsigned long long full[WS_NSTAGE], empty[WS_NSTAGE];
+    uint32_t qid[2 * WS_SB];                                  // producers: queue of Gaussian ids that reach the tile
+    uint32_t xchg[2][2][8];                                   // [iteration parity][producer warp]: ballot counts
+    uint32_t abort_flag[2];                                   // [iteration parity]
+    uint32_t done[8];                                         // consumer warps finished with tile sequence number & 7
+};
+
+// out = C + T bg (reading S16), final T, optional counts, for the two pixels of this thread
+template <bool COUNT>
+__device__ __forceinline__ void ws_write_pixels(const Frame& f, const PixelPair& s, int px, int py, bool in0, bool in1,
+                                                float* __restrict__ out_rgb, float* __restrict__ out_T,
+                                                uint32_t* __restrict__ out_n) {
+    float T0, T1, c0r, c1r, c0g, c1g, c0b, c1b;
+    {   // fold the repairs of the stopped pixels in: T = T - thr where thr < 0, C = C + dC
+        float h0, h1, d0, d1;
+        unpk(s.T, T0, T1); unpk(s.thr, h0, h1);
+        T0 = (h0 < 0.0f ? T0 - h0 : T0) * K_INV;
+        T1 = (h1 < 0.0f ? T1 - h1 : T1) * K_INV;
+        unpk(s.Cr, c0r, c1r); unpk(s.dCr, d0, d1); c0r += d0; c1r += d1;
+        unpk(s.Cg, c0g, c1g); unpk(s.dCg, d0, d1); c0g += d0; c1g += d1;
+        unpk(s.Cb, c0b, c1b); unpk(s.dCb, d0, d1); c0b += d0; c1b += d1;
+    }
+    const size_t npix = (size_t)f.W * f.H, pix = (size_t)py * f.W + px;
+    if (in1 && !(f.W & 1)) {  // both pixels inside, 8-byte aligned pair
+        __stcs(reinterpret_cast<float2*>(out_rgb + pix), make_float2(fmaf(T0, f.bg[0], c0r), fmaf(T1, f.bg[0], c1r)));
+        __stcs(reinterpret_cast<float2*>(out_rgb + npix + pix), make_float2(fmaf(T0, f.bg[1], c0g), fmaf(T1, f.bg[1], c1g)));
+        __stcs(reinterpret_cast<float2*>(out_rgb + 2 * npix + pix), make_float2(fmaf(T0, f.bg[2], c0b), fmaf(T1, f.bg[2], c1b)));
+        __stcs(reinterpret_cast<float2*>(out_T + pix), make_float2(T0, T1));
+        if (COUNT) __stcs(reinterpret_cast<uint2*>(out_n + pix), make_uint2(s.n0, s.n1));
+    } else {
+        if (in0) {
+            out_rgb[pix] = fmaf(T0, f.bg[0], c0r);
+            out_rgb[npix + pix] = fmaf(T0, f.bg[1], c0g);
+            out_rgb[2 * npix + pix] = fmaf(T0, f.bg[2], c0b);
+            out_T[pix] = T0;
+            if (COUNT) out_n[pix] = s.n0;
+        }
+        if (in1) {
+            out_rgb[pix + 1] = fmaf(T1, f.bg[0], c1r);
+            out_rgb[npix + pix + 1] = fmaf(T1, f.bg[1], c1g);
+            out_rgb[2 * npix + pix + 1] = fmaf(T1, f.bg[2], c1b);
+            out_T[pix + 1] = T1;
+            if (COUNT) out_n[pix + 1] = s.n1;
+        }
+    }
+}
+
+// Consumer warp w = quadrant (w & 1, w >> 1) of whatever tile the stage headers announce.
+template <bool COUNT, bool STATS>
+__device__ __forceinline__ void ws_consumer(const Frame& f, WsShared& sm, Ctrl* __restrict__ ctrl, float* __restrict__ out_rgb,
+                                            float* __restrict__ out_T, uint32_t* __restrict__ out_n, const int w,
+                                            const int lane) {
+    const uint32_t full0 = (uint32_t)__cvta_generic_to_shared(&sm.full[0]);
+    const uint32_t empty0 = (uint32_t)__cvta_generic_to_shared(&sm.empty[0]);
+    const uint32_t list0 = (uint32_t)__cvta_generic_to_shared(&sm.list[0][w][0]);
+    const int lx = 8 * (w & 1) + 2 * (lane & 3), ly = 8 * (w >> 1) + (lane >> 2);
+    const float x0 = (float)lx - 7.5f, x1 = x0 + 1.0f, y = (float)ly - 7.5f;  // tile-centre origin (Eq. 1)
+    PixelPair s;
+    s.bxy = pk(x0 * y, x1 * y);
+    s.by2 = pk(y * y, y * y);
+    s.bx = pk(x0, x1);
+    s.by = pk(y, y);
+    s.bx2 = s.T = s.Cr = s.Cg = s.Cb = s.dCr = s.dCg = s.dCb = s.thr = pk(0.0f, 0.0f);
+    s.n0 = s.n1 = 0;
+    bool wdone = true, written = true, in0 = false, in1 = false;
+    int px = 0, py = 0;
+    uint32_t seq = 0;
+    unsigned long long st_walk = 0, st_blend = 0;  // STATS only
+    for (uint32_t g = 0;; g++) {
+        const uint32_t slot = g % WS_NSTAGE;
+        mbar_wait(full0 + 8 * slot, (g / WS_NSTAGE) & 1u);
+        const uint4 h = sm.hdr[slot];
+        if (h.x & WS_EXIT) break;
+        if (h.x & WS_FIRST) {   // a new tile: reset the pixel state
+            const int ty = (int)h.y / f.gx, tx = (int)h.y - ty * f.gx;
+            px = tx * TILE + lx; py = ty * TILE + ly;
+            in0 = px < f.W && py < f.H; in1 = (px + 1) < f.W && py < f.H;
+            s.bx2 = pk(in0 ? x0 * x0 : POISON, in1 ? x1 * x1 : POISON);
+            s.T = pk(K_SCALE, K_SCALE);
+            s.Cr = s.Cg = s.Cb = s.dCr = s.dCg = s.dCb = pk(0.0f, 0.0f);
+            s.thr = pk(TMIN_S, TMIN_S);
+            s.n0 = s.n1 = 0;
+            seq = h.z;
+            written = false;
+            wdone = __all_sync(0xffffffffu, !in0 && !in1);
+            if (wdone && lane == 0) atomicAdd(&sm.done[seq & 7u], 1u);
+        }
+        if (!wdone) {
+            const uint32_t cnt = (h.w >> (8 * w)) & 255u;
+            uint32_t lp = list0 + slot * (uint32_t)(4 * (WS_SB + 2) * 4);
+            const uint32_t lp0 = lp;
+            uint32_t lend = lp + 4 * cnt;
+            if (h.x & WS_INDEF) blend_list<COUNT, true>(s, lp, lend);
+            else blend_list<COUNT, false>(s, lp, lend);
+            wdone = lend == 0;
+            if (STATS) st_walk += min((lp - lp0) / 4, cnt);
+            if (wdone && lane == 0) atomicAdd(&sm.done[seq & 7u], 1u);
+        }
+        if (!written && (wdone || (h.x & WS_LAST))) {
+            ws_write_pixels<COUNT>(f, s, px, py, in0, in1, out_rgb, out_T, out_n);
+            if (STATS) st_blend += s.n0 + s.n1;
+            written = true;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty0 + 8 * slot);
+    }
+    if (STATS) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) st_blend += __shfl_xor_sync(0xffffffffu, st_blend, o);
+        if (lane == 0) {
+            atomicAdd(&ctrl->stats[0], st_walk);
+            atomicAdd(&ctrl->stats[1], st_blend);
+        }
+    }
+}
+
+// The two producer warps (pt = 0..63), in lockstep through named barrier 1.
+//
+// Phase 1, per RAW batch of 64 list entries of the tile (one per thread; records prefetched one batch ahead, ids two):
+//   the tight box of the entry against the WHOLE tile (tile_reach, ~40 instructions).  On the dense scenes 50-85 % of
+//   the entries a 3-sigma rect brings into a list reach no pixel of the tile; they end here.  Survivors are appended,
+//   in list order, to a queue of Gaussian ids.
+// Phase 2, whenever 64 survivors are queued (or the list ends): one STAGE -- records re-read (L1), 4-bit quadrant
+//   masks (Eq. 13-21), per-quadrant compacted lists, double-precision hoist (Eq. 8) -- handed to the consumers.
+// So a stage holds 64 LIVE entries however sparse the list is, and the expensive part of staging runs on dense lanes.
+template <bool STATS>
+__device__ __forceinline__ void ws_producer(const Frame& f, WsShared& sm, Ctrl* __restrict__ ctrl, const uint4* __restrict__ desc,
+                                            const uint32_t* __restrict__ ids, const float4* __restrict__ rec, const int pt) {
+    const int lane = pt & 31, pw = pt >> 5;
+    const unsigned lt = (1u << lane) - 1u;
+    const uint32_t full0 = (uint32_t)__cvta_generic_to_shared(&sm.full[0]);
+    const uint32_t empty0 = (uint32_t)__cvta_generic_to_shared(&sm.empty[0]);
+    const uint32_t null_addr = (uint32_t)__cvta_generic_to_shared(&sm.null_rec[0]);
+    const int G = gridDim.x;
+    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    // ---- current tile: descriptor, records of the raw batch to test next, ids of the batch after -------------------
+    int kn = blockIdx.x;
+    uint4 dc = desc[kn];
+    bool have = true;                       // false once the schedule of this CTA is exhausted
+    uint32_t tile = dc.x, base = dc.y, end = dc.z;
+    float4 r0 = z4, r1 = z4, r2 = z4, r3 = z4;
+    uint32_t idc = 0, idn = 0;
+    if (base + pt < end) {
+        idc = ids[base + pt];
+        const float4* q = rec + 4 * (size_t)idc;
+        r0 = __ldg(q); r1 = __ldg(q + 1); r2 = __ldg(q + 2); r3 = __ldg(q + 3);
+    }
+    if (base + WS_SB + pt < end) idn = ids[base + WS_SB + pt];
+    // ---- next tile: descriptor now, first ids and first records during the batches of the current tile ------------
+    kn += G;
+    bool have_n = kn < f.n_tiles;
+    uint4 dn = have_n ? desc[kn] : make_uint4(0u, 0u, 0u, 0u);
+    int nstate = 0;                         // 0: nothing requested, 1: ids requested, 2: records requested
+    uint32_t nid = 0;
+    float4 n0 = z4, n1 = z4, n2 = z4, n3 = z4;
+    uint32_t seq = 0, g = 0, it = 0;
+    uint32_t qhead = 0, qn = 0;             // survivor queue (circular, 2 * WS_SB ids), identical in all 64 threads
+    bool emitted = false;                   // a stage of the current tile has been handed over
+    unsigned long long st_staged = 0;       // STATS only
+
+    auto next_tile = [&]() {   // switch to the next tile of the schedule (completing its prefetch when the tile was short)
+        have = have_n;
+        qn = 0;
+        emitted = false;
+        if (!have) return;
+        if (nstate == 0 && dn.y + pt < dn.z) nid = ids[dn.y + pt];
+        if (nstate <= 1) {
+            n0 = n1 = n2 = n3 = z4;
+            if (dn.y + pt < dn.z) {
+                const float4* q = rec + 4 * (size_t)nid;
+                n0 = __ldg(q); n1 = __ldg(q + 1); n2 = __ldg(q + 2); n3 = __ldg(q + 3);
+            }
+        }
+        tile = dn.x; base = dn.y; end = dn.z;
+        r0 = n0; r1 = n1; r2 = n2; r3 = n3;
+        idc = nid;
+        idn = (base + WS_SB + pt < end) ? ids[base + WS_SB + pt] : 0u;
+        seq++;
+        if (pt == 0) sm.done[seq & 7u] = 0;   // published to the consumers with the FIRST stage of this tile
+        kn += G;
+        have_n = kn < f.n_tiles;
+        if (have_n) dn = desc[kn];
+        nstate = 0;
+    };
+
+    while (true) {
+        if (!have) {   // schedule exhausted: tell the consumers
+            const uint32_t slot = g % WS_NSTAGE;
+            if (g >= WS_NSTAGE) mbar_wait(empty0 + 8 * slot, ((g / WS_NSTAGE) - 1u) & 1u);
+            if (pt == 0) sm.hdr[slot] = make_uint4(WS_EXIT, 0u, 0u, 0u);
+            mbar_arrive(full0 + 8 * slot);
+            break;
+        }
+        const int ty = (int)tile / f.gx, tx = (int)tile - ty * f.gx;
+        const float Txf = (float)(tx * TILE), Tyf = (float)(ty * TILE);
+        // ---- phase 1: which entries of the raw batch can reach the tile at all ------------------------------------
+        bool alive = false;
+        if (base + pt < end)
+            alive = tile_reach(r0.x - Txf, r0.y - Tyf, r0.w, r1.z, r2.w, r3.x, r3.y) || (__float_as_uint(r1.w) & 1u);
+        const unsigned ba = __ballot_sync(0xffffffffu, alive);
+        uint32_t par = it & 1u;
+        it++;
+        if (lane == 0) sm.xchg[par][pw][0] = __popc(ba);
+        if (pt == 0) sm.abort_flag[par] = *reinterpret_cast<volatile uint32_t*>(&sm.done[seq & 7u]) >= 4u ? 1u : 0u;
+        asm volatile("bar.sync 1, 64;" ::: "memory");   // the two producer warps only
+        if (sm.abort_flag[par]) {   // every pixel of the tile is finished (Eq. 22): abandon it
+            next_tile();
+            continue;
+        }
+        {
+            const uint32_t a0 = sm.xchg[par][0][0], a1 = sm.xchg[par][1][0];
+            if (alive) sm.qid[(qhead + qn + (pw ? a0 : 0u) + __popc(ba & lt)) & (2 * WS_SB - 1)] = idc;
+            qn += a0 + a1;
+        }
+        if (STATS && pt == 0) st_staged += min((uint32_t)WS_SB, end - base);
+        const bool raw_last = base + WS_SB >= end;
+        if (!raw_last) {   // advance the raw pipeline: records of the next batch, ids of the one after
+            base += WS_SB;
+            idc = idn;
+            r0 = r1 = r2 = r3 = z4;
+            if (base + pt < end) {
+                const float4* q = rec + 4 * (size_t)idc;
+                r0 = __ldg(q); r1 = __ldg(q + 1); r2 = __ldg(q + 2); r3 = __ldg(q + 3);
+            }
+            if (base + WS_SB + pt < end) idn = ids[base + WS_SB + pt];
+            if (have_n) {   // one step of the next tile's prefetch
+                if (nstate == 0) {
+                    if (dn.y + pt < dn.z) nid = ids[dn.y + pt];
+                    nstate = 1;
+                } else if (nstate == 1) {
+                    n0 = n1 = n2 = n3 = z4;
+                    if (dn.y + pt < dn.z) {
+                        const float4* q = rec + 4 * (size_t)nid;
+                        n0 = __ldg(q); n1 = __ldg(q + 1); n2 = __ldg(q + 2); n3 = __ldg(q + 3);
+                    }
+                    nstate = 2;
+                }
+            }
+        }
+        // ---- phase 2: hand over full stages (and the partial one when the list ends) --------------------------------
+        bool aborted = false, last_done = false;   // the list's final stage (possibly empty) always carries LAST
+        while (qn >= (uint32_t)WS_SB || (raw_last && !last_done)) {
+            const uint32_t n = min(qn, (uint32_t)WS_SB);
+            const bool last = raw_last && qn == n;
+            const uint32_t slot = g % WS_NSTAGE;
+            if (g >= WS_NSTAGE) mbar_wait(empty0 + 8 * slot, ((g / WS_NSTAGE) - 1u) & 1u);
+            asm volatile("bar.sync 1, 64;" ::: "memory");   // the queue writes of phase 1 are visible
+            float4 s0 = z4, s1 = z4, s2 = z4, s3 = z4;
+            uint32_t m = 0;
+            bool indefinite = false;
+            if (pt < n) {
+                const float4* q = rec + 4 * (size_t)sm.qid[(qhead + pt) & (2 * WS_SB - 1)];
+                s0 = __ldg(q); s1 = __ldg(q + 1); s2 = __ldg(q + 2); s3 = __ldg(q + 3);
+                m = quadrant_mask(s0.x - Txf, s0.y - Tyf, s0.w, s1.z, s2.w, s3.x, s3.y);
+                if (__float_as_uint(s1.w) & 1u) { m = 15u; indefinite = true; }  // degenerate conic: keep everything
+            }
+            const unsigned b0 = __ballot_sync(0xffffffffu, m & 1u), b1 = __ballot_sync(0xffffffffu, m & 2u),
+                           b2 = __ballot_sync(0xffffffffu, m & 4u), b3 = __ballot_sync(0xffffffffu, m & 8u);
+            const unsigned bi = __ballot_sync(0xffffffffu, indefinite);
+            par = it & 1u;
+            it++;
+            if (lane == 0) {
+                *reinterpret_cast<uint4*>(&sm.xchg[par][pw][0]) = make_uint4(__popc(b0), __popc(b1), __popc(b2), __popc(b3));
+                sm.xchg[par][pw][4] = bi ? 1u : 0u;
+            }
+            if (pt == 0) sm.abort_flag[par] = *reinterpret_cast<volatile uint32_t*>(&sm.done[seq & 7u]) >= 4u ? 1u : 0u;
+            asm volatile("bar.sync 1, 64;" ::: "memory");
+            if (sm.abort_flag[par]) { aborted = true; break; }
+            const uint4 c0 = *reinterpret_cast<const uint4*>(&sm.xchg[par][0][0]), c1 = *reinterpret_cast<const uint4*>(&sm.xchg[par][1][0]);
+            const bool any_indef = (sm.xchg[par][0][4] | sm.xchg[par][1][4]) != 0u;
+            // per-quadrant compacted lists of record addresses, in list order (warp 0's entries first)
+            const uint32_t rec_addr = (uint32_t)__cvta_generic_to_shared(&sm.rec[slot][pt * REC]);
+            uint32_t* L0 = &sm.list[slot][0][0];
+            constexpr int LS = WS_SB + 2;
+            if (m & 1u) L0[0 * LS + (pw ? c0.x : 0u) + __popc(b0 & lt)] = rec_addr;
+            if (m & 2u) L0[1 * LS + (pw ? c0.y : 0u) + __popc(b1 & lt)] = rec_addr;
+            if (m & 4u) L0[2 * LS + (pw ? c0.z : 0u) + __popc(b2 & lt)] = rec_addr;
+            if (m & 8u) L0[3 * LS + (pw ? c0.w : 0u) + __popc(b3 & lt)] = rec_addr;
+            const uint32_t t0 = c0.x + c1.x, t1 = c0.y + c1.y, t2 = c0.z + c1.z, t3 = c0.w + c1.w;
+            if (pt < 4) {   // pad every list to an even length with the null record (alpha = 0)
+                const uint32_t tq = pt == 0 ? t0 : (pt == 1 ? t1 : (pt == 2 ? t2 : t3));
+                L0[pt * LS + tq] = null_addr;
+            }
+            if (m) {  // hoist (Eq. 8) in double about the tile centre (reading S14)
+                const Hoisted h = hoist(s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, Txf + 7.5f, Tyf + 7.5f, L_BIAS);
+                float4* d = reinterpret_cast<float4*>(&sm.rec[slot][pt * REC]);
+                d[0] = make_float4(h.A, h.B, h.C, h.F);
+                d[1] = make_float4(h.D, h.E, s2.x, s2.y);
+                d[2] = make_float4(s2.z, indefinite ? s1.y + L_BIAS : 3.0e38f, 0.0f, 0.0f);
+            }
+            if (pt == 0)
+                sm.hdr[slot] = make_uint4((emitted ? 0u : WS_FIRST) | (last ? WS_LAST : 0u) | (any_indef ? WS_INDEF : 0u), tile, seq,
+                                          t0 | (t1 << 8) | (t2 << 16) | (t3 << 24));
+            mbar_arrive(full0 + 8 * slot);   // release: records, lists and header of this thread are visible to the waiters
+            g++;
+            emitted = true;
+            last_done = last;
+            qhead = (qhead + n) & (2 * WS_SB - 1);
+            qn -= n;
+        }
+        if (aborted || raw_last) next_tile();
+    }
+    if (STATS && pt == 0) atomicAdd(&ctrl->stats[2], st_staged);
+}
+
+template <bool COUNT, bool STATS>
+__global__ void __launch_bounds__(WS_THREADS, 4)
+render_ws_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restrict__ desc, const uint32_t* __restrict__ ids,
+                 const float4* __restrict__ rec, float* __restrict__ out_rgb, float* __restrict__ out_T,
+                 uint32_t* __restrict__ out_n) {
+    __shared__ WsShared sm;
+    griddep_sync();
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        for (int k = 0; k < WS_NSTAGE; k++) {
+            mbar_init((uint32_t)__cvta_generic_to_shared(&sm.full[k]), WS_SB);
+            mbar_init((uint32_t)__cvta_generic_to_shared(&sm.empty[k]), 4);
+        }
+    }
+    if (tid < 8) sm.done[tid] = 0;
+    if (tid >= 32 && tid < 35) {   // null record: F = -huge -> alpha = 0 exactly; colours 0; guard never trips
+        float4* d = reinterpret_cast<float4*>(&sm.null_rec[0]) + (tid - 32);
+        *d = make_float4(0.0f, tid == 34 ? 3.0e38f : 0.0f, 0.0f, tid == 32 ? -1.0e30f : 0.0f);
+    }
+    __syncthreads();
+    // warp index through a warp reduction: ptxas then knows it is warp-uniform
+    const int w = __reduce_max_sync(0xffffffffu, tid >> 5);
+    if (w < 4) ws_consumer<COUNT, STATS>(f, sm, ctrl, out_rgb, out_T, out_n, w, tid & 31);
+    else ws_producer<STATS>(f, sm, ctrl, desc, ids, rec, tid - 128);
+}
+
+void launch_render_ws(const Frame& f, const Pointers& p, float* out_rgb, float* out_T, uint32_t* out_n, int n_sm, bool stats,
+                      cudaStream_t st) {
+    const int g = f.n_tiles < n_sm * 4 ? f.n_tiles : n_sm * 4;
+    const dim3 grid(g), block(WS_THREADS);
+    if (stats && out_n)
+        launch_pdl(render_ws_kernel<true, true>, grid, block, st, f, p.ctrl, p.desc, p.ids, p.rec, out_rgb, out_T, out_n);
+    else if (out_n)
+        launch_pdl(render_ws_kernel<true, false>, grid, block, st, f, p.ctrl, p.desc, p.ids, p.rec, out_rgb, out_T, out_n);
+    else
+        launch_pdl(render_ws_kernel<false, false>, grid, block, st, f, p.ctrl, p.desc, p.ids, p.rec, out_rgb, out_T, (uint32_t*)nullptr);
+}
+
 void launch_render_b200(const Frame& f, const Pointers& p, float* out_rgb, float* out_T, uint32_t* out_n, int n_sm,
                         bool stats, cudaStream_t st) {
     (void)n_sm;

@@ -172,7 +172,7 @@ __device__ __forceinline__ void blend_list(PixelPair& s, uint32_t& lp, uint32_t&
 
 template <bool COUNT, bool STATS>
 __global__ void __launch_bounds__(QB, 6)
-render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ ids,
+render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restrict__ desc, const uint32_t* __restrict__ ids,
                    const float4* __restrict__ rec, float* __restrict__ out_rgb, float* __restrict__ out_T,
                    uint32_t* __restrict__ out_n) {
     __shared__ __align__(16) unsigned char s_rec[2][(QB + 1) * REC];  // staged, hoisted records (double-buffered) + a null record
@@ -184,8 +184,12 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint32_t* __res
     // warp index through a warp reduction: ptxas then KNOWS it is warp-uniform (it lives in a uniform register), so
     // every trip count derived from it is uniform and the votes of the blend loop need no divergence guard
     const int w = __reduce_max_sync(0xffffffffu, tid >> 5);
-    const int tile = blockIdx.y * f.gx + blockIdx.x;
-    const int Tx = blockIdx.x * TILE, Ty = blockIdx.y * TILE;
+    // blocks are dispatched in index order: descriptor b follows the render schedule of tile_grid_kernel (classes of
+    // list length, longest first, raster order inside), so the long tiles start first and the launch has no tail
+    const uint4 dsc = desc[blockIdx.x];
+    const int tile = (int)dsc.x;
+    const int tyi = tile / f.gx, txi = tile - tyi * f.gx;
+    const int Tx = txi * TILE, Ty = tyi * TILE;
     // warp w = quadrant (w&1, w>>1); lane -> row lane>>2, column pair lane&3
     const int lx = 8 * (w & 1) + 2 * (lane & 3), ly = 8 * (w >> 1) + (lane >> 2);
     const int px = Tx + lx, py = Ty + ly;
@@ -210,7 +214,7 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint32_t* __res
         if ((tid >> 1) == 2) d->y = 3.0e38f;
     }
     bool wdone = __all_sync(0xffffffffu, !in0 && !in1);
-    const uint32_t start = ranges[tile], end = ranges[tile + 1];
+    const uint32_t start = dsc.y, end = dsc.z;
     const unsigned lt = (1u << lane) - 1u;
     uint32_t st_walk = 0, st_staged = 0;  // STATS only
     // ---- software pipeline prologue: records of batch 0, ids of batch 1 ------------------------------------------
@@ -235,8 +239,9 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint32_t* __res
         const unsigned b0 = __ballot_sync(0xffffffffu, m & 1u), b1 = __ballot_sync(0xffffffffu, m & 2u),
                        b2 = __ballot_sync(0xffffffffu, m & 4u), b3 = __ballot_sync(0xffffffffu, m & 8u);
         const unsigned bi = __ballot_sync(0xffffffffu, indefinite);
-        if (lane == 0) *reinterpret_cast<uint4*>(&s_ball[buf][w][0]) = make_uint4(b0, b1, b2, b3);
-        if (lane == 4) s_indef[buf][w] = bi;
+        // every lane stores the same words (one wavefront, no branch on the lane index)
+        *reinterpret_cast<uint4*>(&s_ball[buf][w][0]) = make_uint4(b0, b1, b2, b3);
+        s_indef[buf][w] = bi;
         if (m) {  // only entries that reach some warp are hoisted
             const Hoisted h = hoist(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, ox, oy, L_BIAS);
             float4* d = reinterpret_cast<float4*>(&s_rec[buf][tid * REC]);
@@ -263,7 +268,7 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint32_t* __res
         if ((bb.y >> lane) & 1u) list[c0 + __popc(bb.y & lt)] = rec_addr + (32 + lane) * REC;
         if ((bb.z >> lane) & 1u) list[c1 + __popc(bb.z & lt)] = rec_addr + (64 + lane) * REC;
         if ((bb.w >> lane) & 1u) list[c2 + __popc(bb.w & lt)] = rec_addr + (96 + lane) * REC;
-        if (lane == 0) list[cnt] = rec_addr + QB * REC;  // pad to an even length with the null record (alpha = 0)
+        list[cnt] = rec_addr + QB * REC;  // pad to an even length with the null record (alpha = 0); same word from every lane
         __syncwarp();
         // ---- blend: this warp walks ITS list only, two entries per iteration ---------------------------------------
         uint32_t lp = (uint32_t)__cvta_generic_to_shared(list);
@@ -712,13 +717,13 @@ void launch_render_ws(const Frame& f, const Pointers& p, float* out_rgb, float* 
 void launch_render_b200(const Frame& f, const Pointers& p, float* out_rgb, float* out_T, uint32_t* out_n, int n_sm,
                         bool stats, cudaStream_t st) {
     (void)n_sm;
-    const dim3 grid(f.gx, f.gy), block(QB);
+    const dim3 grid(f.n_tiles), block(QB);
     if (stats && out_n)
-        launch_pdl(render_b200_kernel<true, true>, grid, block, st, f, p.ctrl, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n);
+        launch_pdl(render_b200_kernel<true, true>, grid, block, st, f, p.ctrl, p.desc, p.ids, p.rec, out_rgb, out_T, out_n);
     else if (out_n)
-        launch_pdl(render_b200_kernel<true, false>, grid, block, st, f, p.ctrl, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n);
+        launch_pdl(render_b200_kernel<true, false>, grid, block, st, f, p.ctrl, p.desc, p.ids, p.rec, out_rgb, out_T, out_n);
     else
-        launch_pdl(render_b200_kernel<false, false>, grid, block, st, f, p.ctrl, p.ranges, p.ids, p.rec, out_rgb, out_T, (uint32_t*)nullptr);
+        launch_pdl(render_b200_kernel<false, false>, grid, block, st, f, p.ctrl, p.desc, p.ids, p.rec, out_rgb, out_T, (uint32_t*)nullptr);
 }
 
 }  // namespace gs

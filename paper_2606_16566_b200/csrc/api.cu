@@ -48,7 +48,7 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     while ((1ll << L.tile_bits) < nt) L.tile_bits++;
     L.n_tile_passes = (L.tile_bits + 7) / 8;
     const size_t Pz = (size_t)P;
-    const size_t depth_tile = (size_t)SORT_THREADS * sort_items_for(Pz), ent_tile = (size_t)SORT_THREADS * sort_items_for(max_dup);
+    const size_t depth_tile = (size_t)SORT_THREADS * sort_items_for(Pz), ent_tile = (size_t)SORT_THREADS * dup_items_for(max_dup);  // the smaller of the tile passes' tiles
     L.n_depth_tiles = (Pz + depth_tile - 1) / depth_tile + 1;
     L.n_tile_tiles = ((size_t)max_dup + ent_tile - 1) / ent_tile + 1;
     size_t o = 0;
@@ -73,7 +73,7 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     L.ranges = take(4 * ((size_t)L.n_tiles + 1));
     L.desc = take(16 * (size_t)L.n_tiles);
     L.entA = take(8 * (size_t)max_dup);
-    L.entB = take(L.n_tile_passes >= 2 ? 8 * (size_t)max_dup : 0);
+    L.entB = take((L.n_tile_passes >= 3 || max_dup > FUSED_DUP_MAX) ? 8 * (size_t)max_dup : 0);
     L.ids = take(4 * (size_t)max_dup + 16);
     L.total = o;
     return true;

@@ -12,6 +12,8 @@
 //
 // Kernels: radix_pass_kernel (one-sweep: block-local ranking + chained decoupled look-back per digit),
 //          tile_grid_kernel, scan_offsets_kernel (chained scan), duplicate_kernel (load-balanced by output chunk).
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace gs {
@@ -30,135 +32,161 @@ namespace gs {
 // latency and ~40-70 cycles of issue per warp instruction (emulated), against ~2 cycles for the atomic
 // (profiles/r01_microbench.md) -- the match-based first version of this kernel spent 35 % of its stall samples there.
 // ------------------------------------------------------------------------------------------------------------
-template <int ITEMS, bool OUT32>
-__global__ void __launch_bounds__(SORT_THREADS, 4)
-radix_pass_kernel(const unsigned long long* __restrict__ in, unsigned long long* __restrict__ out,
-                  uint32_t* __restrict__ out32, const unsigned long long* __restrict__ n_ptr, int shift,
-                  const uint32_t* __restrict__ ghist, unsigned long long* __restrict__ status,
-                  uint32_t* __restrict__ tile_counter) {
+template <int ITEMS, typename K>
+struct SortSmem {
+    K sorted[SORT_THREADS * ITEMS];
+    uint32_t hist[SORT_THREADS / 32][256];
+    uint32_t bpos[256], gbase[256], gpos[256];
+    uint32_t scan[SORT_THREADS / 32];
+    int tile;
+};
+
+// One tile of a pass, shared by the plain pass kernel and the fused duplicate + first-pass kernel.  key[] holds the
+// tile's keys warp-striped (element w*32*ITEMS + j*32 + lane in key[j]); sm.hist is zeroed and sm.gbase holds the
+// exclusive scan of the global digit histogram.  digit(key) -> 0..255; store(pos, key) writes one output element.
+template <int ITEMS, typename K, typename DigitF, typename StoreF>
+__device__ __forceinline__ void radix_tile(SortSmem<ITEMS, K>& sm, K (&key)[ITEMS], const int tile, const uint32_t tile_n,
+                                           unsigned long long* __restrict__ status, DigitF digit, StoreF store) {
     constexpr int NW = SORT_THREADS / 32;
     constexpr int TILE_N = SORT_THREADS * ITEMS;
-    __shared__ unsigned long long s_sorted[TILE_N];
-    __shared__ uint32_t s_hist[NW][256];
-    __shared__ uint32_t s_bpos[256];
-    __shared__ uint32_t s_gbase[256];
-    __shared__ uint32_t s_gpos[256];
-    __shared__ uint32_t s_scan[NW];
-    __shared__ int s_tile;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const uint32_t wbase = w * (32 * ITEMS) + lane;
+    uint32_t rk2[ITEMS / 2];  // two 16-bit ranks per register (a warp holds 32 * ITEMS <= 512 keys)
+    if (tile_n == TILE_N) {
+#pragma unroll
+        for (int j = 0; j < ITEMS; j += 2) {
+            const uint32_t ra = atomicAdd(&sm.hist[w][digit(key[j])], 1u);
+            const uint32_t rb = atomicAdd(&sm.hist[w][digit(key[j + 1])], 1u);
+            rk2[j / 2] = ra | (rb << 16);
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < ITEMS; j += 2) {
+            uint32_t ra = 0, rb = 0;
+            if (wbase + j * 32 < tile_n) ra = atomicAdd(&sm.hist[w][digit(key[j])], 1u);
+            if (wbase + (j + 1) * 32 < tile_n) rb = atomicAdd(&sm.hist[w][digit(key[j + 1])], 1u);
+            rk2[j / 2] = ra | (rb << 16);
+        }
+    }
+    __syncthreads();
+    // ---- per digit: exclusive prefix over warps, block count, publish aggregate ------------------------------
+    uint32_t cnt = 0;
+#pragma unroll
+    for (int k = 0; k < NW; k++) {
+        const uint32_t t = sm.hist[k][tid];
+        sm.hist[k][tid] = cnt;
+        cnt += t;
+    }
+    unsigned long long* st = status + (size_t)tile * 256 + tid;
+    st_status(st, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)cnt);
+    uint32_t tot;
+    const uint32_t bpos = block_excl_scan_256(cnt, sm.scan, tot);  // contains __syncthreads
+    sm.bpos[tid] = bpos;
+    __syncthreads();
+    // ---- block-local reorder through shared memory ---------------------------------------------------------
+#pragma unroll
+    for (int j = 0; j < ITEMS; j++) {
+        if (wbase + j * 32 < tile_n) {
+            const uint32_t d = digit(key[j]);
+            sm.sorted[sm.bpos[d] + sm.hist[w][d] + ((rk2[j / 2] >> (16 * (j & 1))) & 0xffffu)] = key[j];
+        }
+    }
+    // ---- decoupled look-back for digit `tid` ------------------------------------------------------------------
+    // Steady state (many waves of tiles): the direct predecessor already holds its inclusive prefix -- one load.
+    // First wave (or a sort that fits in one wave): every resident tile only has its aggregate published, and the
+    // inclusive prefixes advance a few tiles per L2 round trip; LB_WINDOW status words in flight per step divide
+    // that latency chain.
+    unsigned long long excl = 0;
+    if (tile > 0) {
+        constexpr int LB_WINDOW = 16;
+        int idx = tile - 1;
+        bool done = false;
+        {
+            const unsigned long long s0 = ld_status(status + (size_t)idx * 256 + tid);
+            if ((s0 >> 62) != 0) {
+                excl = s0 & ST_MASK;
+                idx--;
+                done = (s0 >> 62) == 2 || idx < 0;
+            }
+        }
+        while (!done) {
+            unsigned long long sv[LB_WINDOW];
+#pragma unroll
+            for (int k = 0; k < LB_WINDOW; k++)
+                sv[k] = (idx - k >= 0) ? ld_status(status + (size_t)(idx - k) * 256 + tid) : ST_INC;
+#pragma unroll
+            for (int k = 0; k < LB_WINDOW; k++) {
+                if (done || (sv[k] >> 62) == 0) break;   // not published yet: poll again from here
+                excl += sv[k] & ST_MASK;
+                idx--;
+                done = (sv[k] >> 62) == 2;
+            }
+        }
+        st_status(st, ST_INC | (excl + cnt));
+    }
+    sm.gpos[tid] = sm.gbase[tid] + (uint32_t)excl - bpos;
+    __syncthreads();
+    // ---- coalesced output: runs of equal digits are contiguous ---------------------------------------------
+#pragma unroll
+    for (int j = 0; j < ITEMS; j++) {
+        const uint32_t li = j * SORT_THREADS + tid;
+        if (li < tile_n) {
+            const K k = sm.sorted[li];
+            store(sm.gpos[digit(k)] + li, k);
+        }
+    }
+}
+
+// MODE 0: u64 keys in and out, digit (key >> shift) & 255.
+// MODE 1: u64 keys in, only the low 32 bits (the Gaussian id) out -- the last pass of the 64-bit path.
+// MODE 2: packed 32-bit entries (tile >> 8) << 24 | id in, digit = entry >> 24, id out -- the last of two tile passes.
+// MODE 3: u64 entries (tile << 32 | id) in, packed 32-bit entries out -- the first of two tile passes, P <= 2^24.
+template <int ITEMS, int MODE>
+__global__ void __launch_bounds__(SORT_THREADS, 4)
+radix_pass_kernel(const void* __restrict__ in_v, void* __restrict__ out_v, const unsigned long long* __restrict__ n_ptr,
+                  int shift, const uint32_t* __restrict__ ghist, unsigned long long* __restrict__ status,
+                  uint32_t* __restrict__ tile_counter) {
+    using K = typename std::conditional<MODE == 2, uint32_t, unsigned long long>::type;
+    constexpr int TILE_N = SORT_THREADS * ITEMS;
+    __shared__ SortSmem<ITEMS, K> sm;
     griddep_sync();
+    const K* __restrict__ in = static_cast<const K*>(in_v);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const unsigned long long n = *n_ptr;
     {   // exclusive scan of the global digit histogram -> first output slot of every digit
         uint32_t tot;
-        s_gbase[tid] = block_excl_scan_256(ghist[tid], s_scan, tot);
+        sm.gbase[tid] = block_excl_scan_256(ghist[tid], sm.scan, tot);
     }
+    auto digit = [shift](K k) -> uint32_t {
+        if (MODE == 2) return (uint32_t)(k >> 24);
+        return (uint32_t)(k >> shift) & 255u;
+    };
+    auto store = [out_v](uint32_t pos, K k) {
+        if (MODE == 0) static_cast<unsigned long long*>(out_v)[pos] = k;
+        else if (MODE == 1) static_cast<uint32_t*>(out_v)[pos] = (uint32_t)k;
+        else if (MODE == 2) static_cast<uint32_t*>(out_v)[pos] = (uint32_t)k & 0xffffffu;
+        else static_cast<uint32_t*>(out_v)[pos] = ((uint32_t)((unsigned long long)k >> 40) << 24) | ((uint32_t)k & 0xffffffu);
+    };
     while (true) {
         __syncthreads();
-        if (tid == 0) s_tile = (int)atomicAdd(tile_counter, 1u);
+        if (tid == 0) sm.tile = (int)atomicAdd(tile_counter, 1u);
 #pragma unroll
-        for (int k = 0; k < 8; k++) s_hist[w][k * 32 + lane] = 0;
+        for (int k = 0; k < 8; k++) sm.hist[w][k * 32 + lane] = 0;
         __syncthreads();
-        const int tile = s_tile;
+        const int tile = sm.tile;
         const unsigned long long tile_base = (unsigned long long)tile * TILE_N;
         if (tile_base >= n) break;
         const uint32_t tile_n = (uint32_t)min((unsigned long long)TILE_N, n - tile_base);
-        // ---- load (warp-striped) and rank: one shared atomic per key ---------------------------------------
-        unsigned long long key[ITEMS];
-        uint32_t rk2[ITEMS / 2];  // two 16-bit ranks per register (a warp holds 32 * ITEMS <= 512 keys)
+        K key[ITEMS];
         const uint32_t wbase = w * (32 * ITEMS) + lane;
         if (tile_n == TILE_N) {
 #pragma unroll
             for (int j = 0; j < ITEMS; j++) key[j] = __ldcs(in + tile_base + wbase + j * 32);
-#pragma unroll
-            for (int j = 0; j < ITEMS; j += 2) {
-                const uint32_t ra = atomicAdd(&s_hist[w][(uint32_t)(key[j] >> shift) & 255u], 1u);
-                const uint32_t rb = atomicAdd(&s_hist[w][(uint32_t)(key[j + 1] >> shift) & 255u], 1u);
-                rk2[j / 2] = ra | (rb << 16);
-            }
         } else {
 #pragma unroll
-            for (int j = 0; j < ITEMS; j++) {
-                const uint32_t li = wbase + j * 32;
-                key[j] = (li < tile_n) ? in[tile_base + li] : 0ull;
-            }
-#pragma unroll
-            for (int j = 0; j < ITEMS; j += 2) {
-                uint32_t ra = 0, rb = 0;
-                if (wbase + j * 32 < tile_n) ra = atomicAdd(&s_hist[w][(uint32_t)(key[j] >> shift) & 255u], 1u);
-                if (wbase + (j + 1) * 32 < tile_n) rb = atomicAdd(&s_hist[w][(uint32_t)(key[j + 1] >> shift) & 255u], 1u);
-                rk2[j / 2] = ra | (rb << 16);
-            }
+            for (int j = 0; j < ITEMS; j++) key[j] = (wbase + j * 32 < tile_n) ? in[tile_base + wbase + j * 32] : (K)0;
         }
-        __syncthreads();
-        // ---- per digit: exclusive prefix over warps, block count, publish aggregate ------------------------
-        uint32_t cnt = 0;
-#pragma unroll
-        for (int k = 0; k < NW; k++) {
-            const uint32_t t = s_hist[k][tid];
-            s_hist[k][tid] = cnt;
-            cnt += t;
-        }
-        unsigned long long* st = status + (size_t)tile * 256 + tid;
-        st_status(st, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)cnt);
-        uint32_t tot;
-        const uint32_t bpos = block_excl_scan_256(cnt, s_scan, tot);  // contains __syncthreads
-        s_bpos[tid] = bpos;
-        __syncthreads();
-        // ---- block-local reorder through shared memory ---------------------------------------------------
-#pragma unroll
-        for (int j = 0; j < ITEMS; j++) {
-            if (wbase + j * 32 < tile_n) {
-                const uint32_t d = (uint32_t)(key[j] >> shift) & 255u;
-                s_sorted[s_bpos[d] + s_hist[w][d] + ((rk2[j / 2] >> (16 * (j & 1))) & 0xffffu)] = key[j];
-            }
-        }
-        // ---- decoupled look-back for digit `tid` ------------------------------------------------------------
-        // Steady state (many waves of tiles): the direct predecessor already holds its inclusive prefix -- one load.
-        // First wave (or a sort that fits in one wave): every resident tile only has its aggregate published, and the
-        // inclusive prefixes advance a few tiles per L2 round trip; LB_WINDOW status words in flight per step divide
-        // that latency chain (it was 20-30 % of the stall samples of the depth passes with a window of one).
-        unsigned long long excl = 0;
-        if (tile > 0) {
-            constexpr int LB_WINDOW = 16;
-            int idx = tile - 1;
-            bool done = false;
-            {
-                const unsigned long long s0 = ld_status(status + (size_t)idx * 256 + tid);
-                if ((s0 >> 62) != 0) {
-                    excl = s0 & ST_MASK;
-                    idx--;
-                    done = (s0 >> 62) == 2 || idx < 0;
-                }
-            }
-            while (!done) {
-                unsigned long long sv[LB_WINDOW];
-#pragma unroll
-                for (int k = 0; k < LB_WINDOW; k++)
-                    sv[k] = (idx - k >= 0) ? ld_status(status + (size_t)(idx - k) * 256 + tid) : ST_INC;
-#pragma unroll
-                for (int k = 0; k < LB_WINDOW; k++) {
-                    if (done || (sv[k] >> 62) == 0) break;   // not published yet: poll again from here
-                    excl += sv[k] & ST_MASK;
-                    idx--;
-                    done = (sv[k] >> 62) == 2;
-                }
-            }
-            st_status(st, ST_INC | (excl + cnt));
-        }
-        s_gpos[tid] = s_gbase[tid] + (uint32_t)excl - bpos;
-        __syncthreads();
-        // ---- coalesced output: runs of equal digits are contiguous ---------------------------------------
-#pragma unroll
-        for (int j = 0; j < ITEMS; j++) {
-            const uint32_t li = j * SORT_THREADS + tid;
-            if (li < tile_n) {
-                const unsigned long long k = s_sorted[li];
-                const uint32_t d = (uint32_t)(k >> shift) & 255u;
-                const uint32_t pos = s_gpos[d] + li;
-                if (OUT32) out32[pos] = (uint32_t)k;
-                else out[pos] = k;
-            }
-        }
+        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, digit, store);
     }
 }
 
@@ -395,11 +423,123 @@ scan_offsets_kernel(const Pointers p) {
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// Duplication: output slot k belongs to the depth-ranked Gaussian r with off[r] <= k < off[r] + tiles_touched;
-// its j = k - off[r]-th tile in row-major rect order is written as (tile << 32 | id).  Load-balanced by OUTPUT
-// chunk (a splat covering thousands of tiles is spread over many blocks).
+// Duplication FUSED with the first tile pass.  Output slot k of the duplication ("duplicates the surviving
+// primitives across intersecting tiles") belongs to the depth-ranked Gaussian r with off[r] <= k < off[r] +
+// tiles_touched; its j = k - off[r]-th tile in row-major rect order gives the entry (tile << 32 | id).  The entries are
+// never written to HBM in that order: every block GENERATES the 256 * ITEMS consecutive entries of its radix tile in
+// shared memory (4 consecutive slots per thread and 1 024-slot chunk: one binary search in the chunk's staged
+// offsets, then an incremental walk over columns / rows / ranks) and sorts them on the low tile byte straight away.
+// Balanced by OUTPUT slot, so a splat covering 10^4 tiles is spread over many blocks.
+//   OUTK 0: (tile << 32 | id) out (u64)       -- three tile passes (> 65 536 tiles) or ids that need more than 24 bits
+//   OUTK 1: id out (u32)                      -- a single tile pass (<= 256 tiles): this IS the sorted id list
+//   OUTK 2: (tile >> 8) << 24 | id out (u32)  -- two tile passes, P <= 2^24: the second pass moves 4-byte entries
 // ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(DUP_THREADS)
+constexpr int GEN_ITEMS = 4;   // slots per thread and chunk; DUP_TILE = SORT_THREADS * GEN_ITEMS
+template <int ITEMS, int OUTK>
+__global__ void __launch_bounds__(SORT_THREADS, 4)
+dup_pass_kernel(const Frame f, const Pointers p, void* __restrict__ out_v, const uint32_t* __restrict__ ghist,
+                unsigned long long* __restrict__ status, uint32_t* __restrict__ tile_counter) {
+    using K = unsigned long long;
+    constexpr int TILE_N = SORT_THREADS * ITEMS;
+    static_assert(DUP_TILE == SORT_THREADS * GEN_ITEMS && ITEMS % GEN_ITEMS == 0, "chunking");
+    __shared__ SortSmem<ITEMS, K> sm;
+    __shared__ uint32_t s_off[DUP_TILE + 2];
+    __shared__ uint2 s_rect[DUP_TILE + 2];
+    __shared__ uint32_t s_id[DUP_TILE + 2];
+    griddep_sync();
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const unsigned long long n = p.ctrl->n_dup_eff;
+    const uint32_t n_vis = (uint32_t)p.ctrl->n_vis;
+    const uint32_t gx = (uint32_t)f.gx;
+    {
+        uint32_t tot;
+        sm.gbase[tid] = block_excl_scan_256(ghist[tid], sm.scan, tot);
+    }
+    auto digit = [](K k) -> uint32_t { return (uint32_t)(k >> 32) & 255u; };
+    auto store = [out_v](uint32_t pos, K k) {
+        if (OUTK == 0) static_cast<unsigned long long*>(out_v)[pos] = k;
+        else if (OUTK == 1) static_cast<uint32_t*>(out_v)[pos] = (uint32_t)k;
+        else static_cast<uint32_t*>(out_v)[pos] = ((uint32_t)(k >> 40) << 24) | ((uint32_t)k & 0xffffffu);
+    };
+    while (true) {
+        __syncthreads();
+        if (tid == 0) sm.tile = (int)atomicAdd(tile_counter, 1u);
+#pragma unroll
+        for (int k = 0; k < 8; k++) sm.hist[w][k * 32 + lane] = 0;
+        __syncthreads();
+        const int tile = sm.tile;
+        const unsigned long long tile_base = (unsigned long long)tile * TILE_N;
+        if (tile_base >= n) break;
+        const uint32_t tile_n = (uint32_t)min((unsigned long long)TILE_N, n - tile_base);
+        // ---- generate the tile's entries, chunk by chunk, in slot order into sm.sorted ---------------------------
+        for (int c = 0; c < ITEMS / GEN_ITEMS; c++) {
+            const unsigned long long k0 = tile_base + (unsigned long long)c * DUP_TILE;
+            if (k0 >= n) break;
+            const uint32_t cn = (uint32_t)min((unsigned long long)DUP_TILE, n - k0);
+            const unsigned long long ci = k0 / DUP_TILE;
+            const uint32_t r0 = p.chunk_start[ci];
+            const uint32_t r1 = (k0 + DUP_TILE < n) ? p.chunk_start[ci + 1] : (n_vis - 1);
+            const uint32_t nr = r1 - r0 + 1;  // <= DUP_TILE + 1 ranks can start inside one chunk
+            if (c) __syncthreads();           // the previous chunk's staged ranks are no longer read
+            for (uint32_t k = tid; k < nr; k += SORT_THREADS) {  // the chunk's ranks: all sequential reads
+                s_off[k] = p.dup_off[r0 + k];
+                s_rect[k] = p.rk_rect[r0 + k];
+                s_id[k] = (uint32_t)p.gkeyA[r0 + k];
+            }
+            __syncthreads();
+            const uint32_t lk0 = tid * GEN_ITEMS;
+            if (lk0 < cn) {
+                const uint32_t kk = (uint32_t)k0 + lk0;  // N_dup < 2^32
+                uint32_t lo = 0, hi = nr - 1;            // largest local rank with s_off <= kk
+                while (lo < hi) {
+                    const uint32_t mid = (lo + hi + 1) >> 1;
+                    if (s_off[mid] <= kk) lo = mid; else hi = mid - 1;
+                }
+                uint32_t lr = lo;
+                uint2 rc = s_rect[lr];
+                uint32_t id = s_id[lr];
+                uint32_t x0 = rc.x & 0xffffu, x1 = rc.y & 0xffffu, wdt = x1 - x0;
+                uint32_t left = wdt * ((rc.y >> 16) - (rc.x >> 16)) - (kk - s_off[lr]);  // slots of this rank still to emit
+                uint32_t ty, tx;
+                {   // the one division of this thread and chunk: row-major position of slot kk inside the rect
+                    const uint32_t j = kk - s_off[lr], row = j / wdt;
+                    ty = (rc.x >> 16) + row;
+                    tx = x0 + (j - row * wdt);
+                }
+                uint32_t tl = ty * gx + tx;
+                K* dst = &sm.sorted[c * DUP_TILE + lk0];
+#pragma unroll
+                for (int q = 0; q < GEN_ITEMS; q++) {
+                    if (lk0 + q < cn) dst[q] = ((K)tl << 32) | id;
+                    // advance to the next slot: next column, next row of the rect, or the next rank (every visible
+                    // rank has >= 1 tile).  Past the end of the chunk the values are never stored.
+                    tx++; tl++; left--;
+                    if (left == 0) {
+                        lr = min(lr + 1, nr - 1);
+                        rc = s_rect[lr]; id = s_id[lr];
+                        x0 = rc.x & 0xffffu; x1 = rc.y & 0xffffu; wdt = x1 - x0;
+                        left = wdt * ((rc.y >> 16) - (rc.x >> 16));
+                        tx = x0; ty = rc.x >> 16; tl = ty * gx + tx;
+                    } else if (tx == x1) {
+                        tx = x0; ty++; tl = ty * gx + tx;
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        // ---- pick the keys up warp-striped (the order radix_tile ranks in) and sort the tile ---------------------------
+        K key[ITEMS];
+        const uint32_t wbase = w * (32 * ITEMS) + lane;
+#pragma unroll
+        for (int j = 0; j < ITEMS; j++) key[j] = (wbase + j * 32 < tile_n) ? sm.sorted[wbase + j * 32] : (K)0;
+        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, digit, store);   // first barrier inside precedes its stores
+    }
+}
+
+// Stand-alone duplication for LARGE frames: the same walk, entries (tile << 32 | id) written to HBM in duplication
+// order.  Measured on the 10 M-Gaussian scene the fused kernel above is slower than this kernel plus a plain first
+// pass (its phases serialise inside a block); on small frames the fused kernel wins by a launch and 16 bytes per entry.
+__global__ void __launch_bounds__(SORT_THREADS)
 duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict__ ent) {
     __shared__ uint32_t s_off[DUP_TILE + 2];
     __shared__ uint2 s_rect[DUP_TILE + 2];
@@ -416,13 +556,13 @@ duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict
         const uint32_t r1 = ((chunk + 1) * DUP_TILE < n) ? p.chunk_start[chunk + 1] : (n_vis - 1);
         const uint32_t nr = r1 - r0 + 1;  // <= DUP_TILE + 1 ranks can start inside one chunk
         __syncthreads();
-        for (uint32_t k = tid; k < nr; k += DUP_THREADS) {  // the chunk's ranks: offsets, rects, ids -- all sequential reads
+        for (uint32_t k = tid; k < nr; k += SORT_THREADS) {  // the chunk's ranks: offsets, rects, ids -- all sequential reads
             s_off[k] = p.dup_off[r0 + k];
             s_rect[k] = p.rk_rect[r0 + k];
             s_id[k] = (uint32_t)p.gkeyA[r0 + k];
         }
         __syncthreads();
-        const uint32_t lk0 = tid * DUP_ITEMS;
+        const uint32_t lk0 = tid * GEN_ITEMS;
         if (lk0 < cn) {
             const uint32_t kk = (uint32_t)k0 + lk0;  // N_dup < 2^32
             uint32_t lo = 0, hi = nr - 1;            // largest local rank with s_off <= kk
@@ -442,9 +582,9 @@ duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict
                 tx = x0 + (j - row * wdt);
             }
             uint32_t tile = ty * gx + tx;
-            unsigned long long outv[DUP_ITEMS];
+            unsigned long long outv[GEN_ITEMS];
 #pragma unroll
-            for (int q = 0; q < DUP_ITEMS; q++) {
+            for (int q = 0; q < GEN_ITEMS; q++) {
                 outv[q] = ((unsigned long long)tile << 32) | id;
                 // advance to the next slot: next column, next row of the rect, or the next rank (every visible rank
                 // has >= 1 tile).  Past the end of the chunk the values are never stored.
@@ -460,12 +600,12 @@ duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict
                 }
             }
             unsigned long long* dst = ent + k0 + lk0;
-            if (lk0 + DUP_ITEMS <= cn) {
+            if (lk0 + GEN_ITEMS <= cn) {
 #pragma unroll
-                for (int q = 0; q < DUP_ITEMS; q += 2)
+                for (int q = 0; q < GEN_ITEMS; q += 2)
                     __stcs(reinterpret_cast<ulonglong2*>(dst + q), make_ulonglong2(outv[q], outv[q + 1]));
             } else {
-                for (int q = 0; q < DUP_ITEMS && lk0 + q < cn; q++) dst[q] = outv[q];
+                for (int q = 0; q < GEN_ITEMS && lk0 + q < cn; q++) dst[q] = outv[q];
             }
         }
     }
@@ -478,28 +618,26 @@ static int imin(long long a, long long b) { return (int)(a < b ? a : b); }
 
 // Launch one pass with the tile size chosen from the CAPACITY of the sorted array (sort_items_for, common.cuh): small
 // arrays use 1 024-key tiles (more blocks, shorter critical path), large ones 4 096-key tiles (less look-back traffic).
-template <bool OUT32>
-static void launch_pass(int items, int n_sm, unsigned long long capacity, const unsigned long long* in,
-                        unsigned long long* out, uint32_t* out32, const unsigned long long* n_ptr, int shift,
-                        const uint32_t* ghist, unsigned long long* status, uint32_t* tile_counter, cudaStream_t st) {
+template <int MODE>
+static void launch_pass(int items, int n_sm, unsigned long long capacity, const void* in, void* out,
+                        const unsigned long long* n_ptr, int shift, const uint32_t* ghist, unsigned long long* status,
+                        uint32_t* tile_counter, cudaStream_t st) {
     const long long tile_n = (long long)SORT_THREADS * items;
     const long long cap_tiles = ((long long)capacity + tile_n - 1) / tile_n;
-    if (items == 16) {
-        const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
-        launch_pdl(radix_pass_kernel<16, OUT32>, dim3(grid), dim3(SORT_THREADS), st, in, out, out32, n_ptr, shift, ghist, status, tile_counter);
-    } else {
-        const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
-        launch_pdl(radix_pass_kernel<4, OUT32>, dim3(grid), dim3(SORT_THREADS), st, in, out, out32, n_ptr, shift, ghist, status, tile_counter);
-    }
+    const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
+    if (items == 16)
+        launch_pdl(radix_pass_kernel<16, MODE>, dim3(grid), dim3(SORT_THREADS), st, in, out, n_ptr, shift, ghist, status, tile_counter);
+    else
+        launch_pdl(radix_pass_kernel<4, MODE>, dim3(grid), dim3(SORT_THREADS), st, in, out, n_ptr, shift, ghist, status, tile_counter);
 }
 
 void launch_depth_sort(const Frame& f, const Pointers& p, int n_sm, cudaStream_t st, int* launches) {
     unsigned long long* bufs[2] = {p.gkeyA, p.gkeyB};
     const int items = sort_items_for((unsigned long long)f.P);
     for (int pass = 0; pass < MAX_SORT_PASSES_DEPTH; pass++) {
-        launch_pass<false>(items, n_sm, (unsigned long long)f.P, bufs[pass & 1], bufs[(pass + 1) & 1], nullptr, &p.ctrl->n_sort,
-                           32 + 8 * pass, p.ctrl->depth_hist[pass], p.st_depth + (size_t)pass * p.n_depth_tiles * 256,
-                           &p.ctrl->tile_counter[TC_DEPTH0 + pass], st);
+        launch_pass<0>(items, n_sm, (unsigned long long)f.P, bufs[pass & 1], bufs[(pass + 1) & 1], &p.ctrl->n_sort,
+                       32 + 8 * pass, p.ctrl->depth_hist[pass], p.st_depth + (size_t)pass * p.n_depth_tiles * 256,
+                       &p.ctrl->tile_counter[TC_DEPTH0 + pass], st);
         (*launches)++;
     }
 }
@@ -516,25 +654,67 @@ void launch_scan_offsets(const Frame& f, const Pointers& p, int n_sm, cudaStream
     (*launches)++;
 }
 
-// Entries are first written into the buffer from which n_tile_passes ping-pong passes end in `ids`.
+// Duplication fused with the first tile pass, then the remaining tile passes:
+//   1 pass  (<= 256 tiles):                 fused pass writes the sorted ids
+//   2 passes, P <= 2^24:                    fused pass writes packed 4-byte entries, second pass (MODE 2) the ids
+//   2 passes, P >  2^24 / 3 passes:         fused pass writes 8-byte entries, 64-bit passes follow
+template <int OUTK>
+static void launch_dup_pass(int items, int n_sm, const Frame& f, const Pointers& p, void* out, cudaStream_t st) {
+    const long long tile_n = (long long)SORT_THREADS * items;
+    const long long cap_tiles = ((long long)f.max_dup + tile_n - 1) / tile_n;
+    const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
+    if (items == 8)
+        launch_pdl(dup_pass_kernel<8, OUTK>, dim3(grid), dim3(SORT_THREADS), st, f, p, out, p.ctrl->tile_hist[0], p.st_tile,
+                   &p.ctrl->tile_counter[TC_TILE0]);
+    else
+        launch_pdl(dup_pass_kernel<4, OUTK>, dim3(grid), dim3(SORT_THREADS), st, f, p, out, p.ctrl->tile_hist[0], p.st_tile,
+                   &p.ctrl->tile_counter[TC_TILE0]);
+}
+
 void launch_duplicate_and_tile_sort(const Frame& f, const Pointers& p, int n_sm, cudaStream_t st, int* launches,
                                     cudaEvent_t ev_after_duplicate) {
-    const long long cap_chunks = ((long long)f.max_dup + DUP_TILE - 1) / DUP_TILE;
-    const int dgrid = imin(cap_chunks > 0 ? cap_chunks : 1, (long long)n_sm * 8);
-    launch_pdl(duplicate_kernel, dim3(dgrid), dim3(DUP_THREADS), st, f, p, p.entA);
-    (*launches)++;
-    if (ev_after_duplicate) cudaEventRecord(ev_after_duplicate, st);
+    const int gen_items = dup_items_for(f.max_dup), items = sort_items_for(f.max_dup);
+    const bool packed = f.n_tile_passes == 2 && f.P <= (1 << 24);
+    const bool fused = f.max_dup <= FUSED_DUP_MAX;
     unsigned long long* bufs[2] = {p.entA, p.entB};
-    const int items = sort_items_for(f.max_dup);
-    for (int pass = 0; pass < f.n_tile_passes; pass++) {
+    int first_pass = 1;
+    if (fused) {
+        if (f.n_tile_passes == 1) launch_dup_pass<1>(gen_items, n_sm, f, p, p.ids, st);
+        else if (packed) launch_dup_pass<2>(gen_items, n_sm, f, p, p.entA, st);
+        else launch_dup_pass<0>(gen_items, n_sm, f, p, p.entA, st);
+        (*launches)++;
+        if (ev_after_duplicate) cudaEventRecord(ev_after_duplicate, st);
+    } else {   // entries to entB, first pass entB -> entA (packed or not), so that the later passes find them as in the fused path
+        const long long cap_chunks = ((long long)f.max_dup + DUP_TILE - 1) / DUP_TILE;
+        const int dgrid = imin(cap_chunks > 0 ? cap_chunks : 1, (long long)n_sm * 8);
+        launch_pdl(duplicate_kernel, dim3(dgrid), dim3(SORT_THREADS), st, f, p, p.entB);
+        (*launches)++;
+        if (ev_after_duplicate) cudaEventRecord(ev_after_duplicate, st);
+        if (f.n_tile_passes == 1)
+            launch_pass<1>(items, n_sm, f.max_dup, p.entB, p.ids, &p.ctrl->n_dup_eff, 32, p.ctrl->tile_hist[0], p.st_tile,
+                           &p.ctrl->tile_counter[TC_TILE0], st);
+        else if (packed)
+            launch_pass<3>(items, n_sm, f.max_dup, p.entB, p.entA, &p.ctrl->n_dup_eff, 32, p.ctrl->tile_hist[0], p.st_tile,
+                           &p.ctrl->tile_counter[TC_TILE0], st);
+        else {   // three passes: entB -> entA -> entB -> ids
+            launch_pass<0>(items, n_sm, f.max_dup, p.entB, p.entA, &p.ctrl->n_dup_eff, 32, p.ctrl->tile_hist[0], p.st_tile,
+                           &p.ctrl->tile_counter[TC_TILE0], st);
+        }
+        (*launches)++;
+    }
+    for (int pass = first_pass; pass < f.n_tile_passes; pass++) {
         const bool last = pass == f.n_tile_passes - 1;
         unsigned long long* status = p.st_tile + (size_t)pass * p.n_tile_tiles * 256;
-        if (last)
-            launch_pass<true>(items, n_sm, f.max_dup, bufs[pass & 1], nullptr, p.ids, &p.ctrl->n_dup_eff, 32 + 8 * pass,
-                              p.ctrl->tile_hist[pass], status, &p.ctrl->tile_counter[TC_TILE0 + pass], st);
+        const void* in = bufs[(pass - 1) & 1];
+        if (packed)
+            launch_pass<2>(items, n_sm, f.max_dup, in, p.ids, &p.ctrl->n_dup_eff, 0, p.ctrl->tile_hist[pass], status,
+                           &p.ctrl->tile_counter[TC_TILE0 + pass], st);
+        else if (last)
+            launch_pass<1>(items, n_sm, f.max_dup, in, p.ids, &p.ctrl->n_dup_eff, 32 + 8 * pass, p.ctrl->tile_hist[pass], status,
+                           &p.ctrl->tile_counter[TC_TILE0 + pass], st);
         else
-            launch_pass<false>(items, n_sm, f.max_dup, bufs[pass & 1], bufs[(pass + 1) & 1], nullptr, &p.ctrl->n_dup_eff,
-                               32 + 8 * pass, p.ctrl->tile_hist[pass], status, &p.ctrl->tile_counter[TC_TILE0 + pass], st);
+            launch_pass<0>(items, n_sm, f.max_dup, in, bufs[pass & 1], &p.ctrl->n_dup_eff, 32 + 8 * pass, p.ctrl->tile_hist[pass],
+                           status, &p.ctrl->tile_counter[TC_TILE0 + pass], st);
         (*launches)++;
     }
 }

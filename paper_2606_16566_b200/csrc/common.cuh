@@ -17,9 +17,10 @@ constexpr int COMPACT_MIN_P = 1 << 20;                // scenes below this size 
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_WARP_TILE = 32 * SCAN_ITEMS;        // 256 depth-sorted Gaussians per offset-scan tile (one warp)
-constexpr int DUP_THREADS = 256;
-constexpr int DUP_ITEMS = 8;
-constexpr int DUP_TILE = DUP_THREADS * DUP_ITEMS;     // 2048 duplicated entries per block
+constexpr unsigned long long FUSED_DUP_MAX = 4ull << 20;   // frames up to this capacity fuse the duplication into the first tile pass
+constexpr int DUP_TILE = 1024;                        // duplication chunk: output slots per staged set of depth ranks
+// keys per thread of the fused duplicate + first-tile-pass kernel (its tile also holds the staged ranks of a chunk)
+__host__ __device__ inline int dup_items_for(unsigned long long capacity) { return capacity <= (256ull << 10) ? 4 : 8; }
 
 // Control block at the start of the workspace; zeroed (with the tile-difference grid and the look-back status
 // arrays that follow it) by one cudaMemsetAsync per frame.

@@ -97,6 +97,30 @@ def _dist():
     return ws, int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0"))
 
 
+# Replicas only: the ranks never exchange data-path bytes; torch.distributed carries the barrier
+# around the timed region and the max-over-ranks of the device time.  Backend-agnostic so that the world-size-2 gloo
+# test (tests/test_replicas_gloo.py) exercises exactly these functions on CPU.
+def replica_barrier(ws):
+    if ws > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def replica_max(x, ws, device):
+    if ws == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_fps(ws, frames_per_rank, slowest_rank_ms):
+    """Whole-job frames/s: every rank rendered `frames_per_rank` frames; time = the slowest rank's device time."""
+    return ws * frames_per_rank / (slowest_rank_ms * 1e-3)
+
+
 # ----------------------------------------------------------------------------------------------------------------
 # reference arm: the CPU oracle, as it stands, on the host cores
 # ----------------------------------------------------------------------------------------------------------------
@@ -145,14 +169,27 @@ def _config_dict(config, cfg, sc, extra=None):
 # ----------------------------------------------------------------------------------------------------------------
 # our arm: the CUDA path through the C ABI
 # ----------------------------------------------------------------------------------------------------------------
-def _stage_bytes(P, K_sh, n_vis, n_dup, n_tile_passes):
+def _stage_bytes(P, K_sh, n_vis, n_dup, n_tile_passes, max_dup):
     """Algorithmic HBM bytes per frame of the memory-bound stages."""
+    compact = P >= (1 << 20)                  # common.cuh COMPACT_MIN_P: small scenes sort all P keys
+    n_sort = n_vis if compact else P
+    fused = max_dup <= (4 << 20)              # common.cuh FUSED_DUP_MAX
+    packed = n_tile_passes == 2 and P <= (1 << 24)
+    rank_bytes = n_vis * 20                   # depth-ordered id (8) + offset (4) + rect (8), read by the duplication
+    if n_tile_passes == 1:
+        first, rest = (4, 0) if fused else (8 + 8 + 4, 0)
+    elif packed:
+        first, rest = (4, 8) if fused else (8 + 8 + 4, 8)      # packed 4-byte entries between the two passes
+    else:
+        first, rest = (8, 16 * (n_tile_passes - 2) + 12) if fused else (8 + 16, 16 * (n_tile_passes - 2) + 12)
+    dup_only = rank_bytes + n_dup * (first if fused else 8)
+    sort_rest = n_dup * ((first - 8 if not fused else 0) + rest)
     return {
-        "preprocess": P * 40 + n_vis * (4 + 12 * K_sh) + P * 16 + n_vis * 56,
-        "depth_sort": 4 * 16 * n_vis,
-        "offset_scan": n_vis * (8 + 16 + 4),
-        "duplicate": n_vis * 28 + n_dup * 8,
-        "tile_sort": (n_tile_passes - 1) * 16 * n_dup + 12 * n_dup,
+        "preprocess": P * 40 + n_vis * (4 + 12 * K_sh) + P * 16 + n_vis * 64 + n_sort * 8,
+        "depth_sort": 4 * 16 * n_sort,
+        "offset_scan": n_vis * (8 + 16 + 4 + 8),
+        "duplicate": dup_only,
+        "tile_sort": sort_rest,
     }
 
 
@@ -183,18 +220,13 @@ def run_ours(args):
     W, H = cfg["W"], cfg["H"]
 
     def barrier():
-        if ws > 1:
-            dist.barrier()
+        replica_barrier(ws)
 
     def rank_max(x):
-        if ws == 1:
-            return float(x)
-        t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replica_max(x, ws, dev)
 
     # ---- size the workspace: largest N_dup over the poses (+5 %) -----------------------------------------------------
-    max_dup, need = 1 << 22, 0
+    max_dup, need = 1 << 21, 0
     r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True)
     r.upload(sc)
     per_pose = []
@@ -223,6 +255,7 @@ def run_ours(args):
         stats.append(binding.gs_get_stats(r.workspace))
         it = r.intermediates(copy=())
         per_pose.append((it.n_visible, it.n_dup))
+        max_dup = int(it.max_dup)   # the capacity the library recovered from the workspace size
     binding.gs_set_stats(False)
     launches_per_frame = binding.gs_last_launch_count()
     mean = lambda xs: float(sum(xs)) / max(len(xs), 1)
@@ -271,7 +304,7 @@ def run_ours(args):
     dev_ms = sum(e0.elapsed_time(e1) for e0, e1 in evs)
     dev_ms = rank_max(dev_ms)
     ms_per_step = dev_ms / K
-    fps = ws * n_pose * K / (dev_ms * 1e-3)
+    fps = aggregate_fps(ws, n_pose * K, dev_ms)
 
     # ---- per-stage device times: a second pass with the library's own CUDA events between its kernels -----------
     binding.gs_set_timing(True)
@@ -323,7 +356,7 @@ def run_ours(args):
                                      "pairs_blended": pairs_blend, "entries_staged": staged},
                 "ms_per_launch": stage_ms["render"]}
     n_tile_passes = (max(1, (((W + 15) // 16) * ((H + 15) // 16) - 1).bit_length()) + 7) // 8
-    sb = _stage_bytes(sc.P, (sc.sh_degree + 1) ** 2, n_vis_m, n_dup_m, n_tile_passes)
+    sb = _stage_bytes(sc.P, (sc.sh_degree + 1) ** 2, n_vis_m, n_dup_m, n_tile_passes, max_dup)
     kernels = []
     for n in ("preprocess", "depth_sort", "tile_grid", "offset_scan", "duplicate", "tile_sort", "render"):
         k = {"stage": n, "ms": stage_ms[n], "share": stage_ms[n] / max(stage_ms["frame"], 1e-9)}

@@ -18,6 +18,7 @@ from . import build as _build
 
 GS_OK, GS_ERR_BAD_ARG, GS_ERR_WORKSPACE, GS_ERR_OVERFLOW, GS_ERR_CUDA = 0, -1, -2, -3, -4
 GS_TILE = 16
+GS_DEFAULT_RENDER_VARIANT = 4   # include/gs.h: the B200 render kernel
 GS_N_TIMINGS = 8
 TIMING_NAMES = ("preprocess", "depth_sort", "tile_grid", "offset_scan", "duplicate", "tile_sort", "render", "frame")
 

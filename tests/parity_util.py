@@ -26,8 +26,8 @@ def run_gpu(scene, cam_index=0, max_dup=None, variant=None, count_contrib=True, 
     cam = scene.cameras[cam_index]
     if max_dup is None:
         max_dup = 1 << 20
-    if variant is not None:
-        binding.gs_set_render_variant(variant)
+    # the variant is process-wide state of the library: always set it, the product default when none is asked for
+    binding.gs_set_render_variant(binding.GS_DEFAULT_RENDER_VARIANT if variant is None else variant)
     r = renderer or Renderer(scene.P, cam.W, cam.H, max_dup, device=device, count_contrib=count_contrib)
     if renderer is None or r.scene is None:
         r.upload(scene)

@@ -34,7 +34,7 @@ def _sample_tiles(ref_counts, gx, gy, n, seed):
 # ------------------------------------------------------------------------------------------------------------------
 # config 1 (tiny) -- every render variant of the ablation ladder, whole image
 # ------------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", [4, 3, 2, 1, 0])
+@pytest.mark.parametrize("variant", [4, 5, 3, 2, 1, 0])
 def test_config1_all_variants(variant):
     sc = scenes.make_scene(1)
     rep, r, it, ref = pu.oracle_and_compare(sc, 0, variant=variant)
@@ -45,7 +45,7 @@ def test_config1_all_variants(variant):
 # ------------------------------------------------------------------------------------------------------------------
 # config 2 (object-centric, the bench workload) -- full size, whole image, several poses
 # ------------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("pose,variant", [(0, 4), (3, 4), (5, 4), (0, 3), (1, 0)])
+@pytest.mark.parametrize("pose,variant", [(0, 4), (3, 4), (5, 4), (0, 3), (1, 0), (2, 5)])
 def test_config2_full(pose, variant):
     sc = scenes.make_scene(2)
     rep, *_ = pu.oracle_and_compare(sc, pose, variant=variant)

@@ -345,10 +345,9 @@ def run_ours(args):
     alu_peak = n_sm * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12       # T thread-instr/s
     render_s = stage_ms["render"] * 1e-3
     achieved = pairs_eval * INSTR_PER_PAIR / render_s / 1e12
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp)).get("config%d" % args.config, {}).get("render_dram_bytes_per_launch")
+    # dram__bytes_read.sum + dram__bytes_write.sum of one render launch from the committed `ncu --set full` capture
+    # (profiles/r01_render_config2_final_ncu.md); only measured for the default workload
+    traffic = {2: 10132480}.get(args.config)
     roofline = {"kernel": "render_b200_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                 "unit": "T FP32-pipe thread-instr/s", "frac": achieved / alu_peak, "traffic": traffic,
                 "peak_source": "derived: %d SMs x %d FP32 lanes x %.0f MHz (max SM clock)" % (n_sm, FP32_LANES_PER_SM, peaks["sm_max_mhz"]),

@@ -11,7 +11,8 @@
  *     keeps no reference to any pointer after the call returns, except that gs_get_intermediates() returns
  *     pointers INTO the caller's workspace.
  *   - Matrices are 16 floats, row-major, column-vector convention (p_cam = V * [p;1]).
- *   - All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *   - All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream); one small
+ *     kernel runs on a library-owned side stream, forked from and joined back into `cuda_stream` with events.
  *     gs_render() returns after enqueueing; it performs NO host synchronisation unless timing is enabled.
  *   - Return value: 0 (GS_OK) or a negative error code; nothing is printed, thrown or exit()ed.
  *   - Not thread-safe per workspace; distinct workspaces on distinct streams may be used concurrently.
@@ -85,8 +86,10 @@ int gs_get_intermediates(const void* workspace, gs_intermediates* out);
 
 /* Per-stage device times (ms, CUDA events) of the last gs_render() on this workspace made while timing was
  * enabled with gs_set_timing(1): [0] preprocess, [1] depth sort, [2] tile grid, [3] offset scan, [4] duplicate,
- * [5] tile sort, [6] render, [7] whole frame.  Enabling timing adds event records and one stream synchronisation
- * per frame; it is off by default. */
+ * [5] tile sort, [6] render, [7] whole frame.  [4] is the duplication -- fused with the first tile pass on frames with a
+ * capacity of <= 4 M entries -- and [5] the remaining tile passes.  Enabling timing adds event records and one stream
+ * synchronisation per frame, serialises the tile-grid kernel (otherwise on a side stream, concurrent with the depth sort)
+ * and disables programmatic dependent launch, so that every stage time is that stage alone; it is off by default. */
 #define GS_N_TIMINGS 8
 int gs_set_timing(int enable);
 int gs_get_timings(const void* workspace, float ms[GS_N_TIMINGS]);
@@ -97,6 +100,7 @@ int gs_get_timings(const void* workspace, float ms[GS_N_TIMINGS]);
  *   2 = + warp-level culling (Eq. 13-21)
  *   3 = + warp-coherent blending (Eq. 22, branch-free)            -- the paper's full method
  *   4 = B200 design (default): 2 pixels/thread, packed f32x2, per-warp ballot compaction, prefetched staging
+ *   5 = experimental: variant 4's blend loop in warp-specialised persistent CTAs (producer / consumer warps, mbarrier ring)
  * Returns GS_ERR_BAD_ARG for an unknown variant.  Process-wide. */
 int gs_set_render_variant(int variant);
 int gs_get_render_variant(void);

@@ -101,6 +101,8 @@ int gs_get_timings(const void* workspace, float ms[GS_N_TIMINGS]);
  *   3 = + warp-coherent blending (Eq. 22, branch-free)            -- the paper's full method
  *   4 = B200 design (default): 2 pixels/thread, packed f32x2, per-warp ballot compaction, prefetched staging
  *   5 = experimental: variant 4's blend loop in warp-specialised persistent CTAs (producer / consumer warps, mbarrier ring)
+ *   6 = precision switch of PAPER.md Table V: variant 3 with the polynomial in GLOBAL pixel coordinates and fp32
+ *       coefficients (Eq. 11).  For measuring the error the tile-local form removes; NOT within the parity tolerance.
  * Returns GS_ERR_BAD_ARG for an unknown variant.  Process-wide. */
 int gs_set_render_variant(int variant);
 int gs_get_render_variant(void);

@@ -261,7 +261,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     launch_duplicate_and_tile_sort(f, p, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b)
     mark(6);
     const int variant = g_variant.load();                      // (4) render
-    if (variant >= 5) launch_render_ws(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
+    if (variant == 5) launch_render_ws(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
     else if (variant == 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
     else launch_render_ladder(variant, f, p, out_rgb, out_final_T, out_n_contrib, st);
     launches++;
@@ -387,7 +387,7 @@ int gs_copy_to_host(void* dst_host, const void* src_dev, size_t bytes) {
 }
 
 int gs_set_render_variant(int variant) {
-    if (variant < 0 || variant > 5) return GS_ERR_BAD_ARG;
+    if (variant < 0 || variant > 6) return GS_ERR_BAD_ARG;
     g_variant.store(variant);
     return GS_OK;
 }

@@ -4,6 +4,9 @@
 //   variant 1  + tile-local hoisting: log2(alpha) = V_hoisted . B_local, 5 FMA (Eq. 7-10)
 //   variant 2  + warp-level culling: 8-bit visibility mask, uniform skip (Eq. 13-21)
 //   variant 3  + warp-coherent blending: branch-free predicated blend, warp-uniform exit (Eq. 22)
+//   variant 6  = variant 3 with the polynomial in GLOBAL pixel coordinates and fp32 coefficients: the precision switch of
+//              PAPER.md Sec. III-B4 / Table V (Eq. 11: error bound 4 * 4000^2 * 2^-24 = 3.81 in ln alpha at 4K).  It
+//              exists to MEASURE that failure against the oracle; it does not meet the parity tolerance by design.
 // All variants implement termination rule R1 (reading S11) and produce the same image up to rounding.
 // The B200 design (variant 4) lives in render_b200.cu.  This TU may use approximate intrinsics.
 #include "render_common.cuh"
@@ -12,7 +15,21 @@ namespace gs {
 
 constexpr int RB = 256;  // batch = block size
 
-template <int VAR>
+// Eq. 8 evaluated the naive way: fp32 throughout, about an arbitrary origin (the global-coordinate variant uses (0, 0)).
+__device__ __forceinline__ Hoisted hoist_f32(float mux, float muy, float a, float b, float c, float log2o, float ox, float oy) {
+    const float k = LOG2E;
+    const float dx = mux - ox, dy = muy - oy;
+    Hoisted h;
+    h.A = -0.5f * k * a;
+    h.B = -k * b;
+    h.C = -0.5f * k * c;
+    h.D = k * (a * dx + b * dy);
+    h.E = k * (b * dx + c * dy);
+    h.F = log2o - 0.5f * k * (a * dx * dx + 2.0f * b * dx * dy + c * dy * dy);
+    return h;
+}
+
+template <int VAR, bool GLOBAL = false>
 __global__ void __launch_bounds__(256)
 render_ladder_kernel(const Frame f, const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ ids,
                      const float4* __restrict__ rec, float* __restrict__ out_rgb,
@@ -30,7 +47,7 @@ render_ladder_kernel(const Frame f, const uint32_t* __restrict__ ranges, const u
     const int px = Tx + lx, py = Ty + ly;
     const bool inside = px < f.W && py < f.H;
     const float fx_ = (float)px, fy_ = (float)py;     // baseline: global pixel coordinates
-    const float xl = (float)lx, yl = (float)ly;       // hoisted: tile-local coordinates (Eq. 1)
+    const float xl = GLOBAL ? fx_ : (float)lx, yl = GLOBAL ? fy_ : (float)ly;  // hoisted: tile-local coordinates (Eq. 1)
     const float bx2 = xl * xl, bxy = xl * yl, by2 = yl * yl;  // B_local (Eq. 9)
     const uint32_t start = ranges[tile], end = ranges[tile + 1];
     float T = 1.0f, Cr = 0.0f, Cg = 0.0f, Cb = 0.0f;
@@ -47,7 +64,8 @@ render_ladder_kernel(const Frame f, const uint32_t* __restrict__ ranges, const u
                 s_col[tid] = __ldg(rec + 4 * (size_t)id + 2);
                 const bool indefinite = __float_as_uint(g1.w) & 1u;
                 if (HOIST) {
-                    const Hoisted h = hoist(g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, (float)Tx, (float)Ty);
+                    const Hoisted h = GLOBAL ? hoist_f32(g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, 0.0f, 0.0f)
+                                             : hoist(g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, (float)Tx, (float)Ty);
                     s_q0[tid] = make_float4(h.A, h.B, h.C, h.F);
                     // power > 0  <=>  log2(alpha) > log2(o): only an indefinite conic can get there (C-R step 2)
                     s_q1[tid] = make_float4(h.D, h.E, indefinite ? g1.y : 3.0e38f, 0.0f);
@@ -145,6 +163,7 @@ void launch_render_ladder(int variant, const Frame& f, const Pointers& p, float*
         case 0: render_ladder_kernel<0><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n); break;
         case 1: render_ladder_kernel<1><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n); break;
         case 2: render_ladder_kernel<2><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n); break;
+        case 6: render_ladder_kernel<3, true><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n); break;
         default: render_ladder_kernel<3><<<grid, block, 0, st>>>(f, p.ranges, p.ids, p.rec, out_rgb, out_T, out_n); break;
     }
 }

@@ -234,3 +234,23 @@ def test_shared_atomic_rank_order_selftest():
     r = binding.gs_selftest_atomic_order(40)
     assert r["atomics_checked"] > 10_000_000
     assert r["violations"] == 0, r
+
+
+def test_global_coordinate_polynomial_loses_precision_at_4k():
+    """PAPER.md Sec. III-B4 / Table V: the expanded polynomial in GLOBAL pixel coordinates loses up to
+    4 * 4000^2 * 2^-24 = 3.81 in ln(alpha) at 4K (Eq. 11), the tile-local form 2.4e-4 (Eq. 12).  Variant 6 is variant 3
+    with global coordinates and fp32 coefficients; on a 4K frame it must miss the oracle by far more than variant 3,
+    which stays inside the parity tolerance."""
+    sc = scenes.make_scene(5, P=150_000, poses=1)          # 3840x2160, f = 3000: coordinates up to ~4000
+    ref = oracle.render(sc, 0, n_threads=8, fragile_delta=pu.DELTA)
+    err = {}
+    for variant in (3, 6):
+        r, it = pu.run_gpu_auto(sc, 0, variant=variant, start_dup=int(ref.n_dup) + 4096)
+        d = np.abs(r.out_rgb.cpu().numpy() - ref.image).max(axis=0)
+        err[variant] = (float(d.max()), float((d > pu.TOL_MOST).mean()))
+        if variant == 3:
+            pu.compare(r, it, ref)                         # the tile-local form is inside the tolerance
+    binding.gs_set_render_variant(binding.GS_DEFAULT_RENDER_VARIANT)
+    print("max |rgb - oracle|, share of pixels over 2e-3: tile-local %s, global %s" % (err[3], err[6]))
+    assert err[3][0] <= pu.TOL_ALL and err[3][1] <= 1e-3
+    assert err[6][0] > 10.0 * max(err[3][0], 1e-4) and err[6][0] > pu.TOL_ALL

@@ -325,9 +325,8 @@ def run_ours(args):
     def e2e_step():
         h2d = r.upload(sc)
         for i, cam in enumerate(cams):
-            r.render(cam, count_contrib=False)
-            r.read_image(i, n_pose)
-        torch.cuda.synchronize()
+            r.render_to_host(cam, i, n_pose)      # device -> pinned host copy of frame i overlaps the render of frame i+1
+        r.synchronize_readback()
         return h2d
     for _ in range(2):
         h2d_bytes = e2e_step()

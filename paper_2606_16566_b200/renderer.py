@@ -28,6 +28,7 @@ class Renderer:
         self.scene = None
         self._pinned = None   # host staging of the scene arrays (pinned), allocated on the first upload
         self._host_rgb = None
+        self._ring = None     # render_to_host(): two device images, a copy stream and the events that order them
 
     def upload(self, scene) -> int:
         """Host (numpy) scene -> device tensors: pinned staging, async copies on the current stream.  The staging and
@@ -43,12 +44,44 @@ class Renderer:
             nbytes += self._pinned[n].numel() * 4
         return nbytes
 
-    def render(self, cam, stream=None, count_contrib: bool = True) -> None:
+    def render(self, cam, stream=None, count_contrib: bool = True, out_rgb=None) -> None:
         s = self.scene
         binding.gs_render(s["means3D"], s["scales"], s["rotations"], s["opacities"], s["sh"], s["sh_degree"],
-                          cam.viewmatrix, cam.projmatrix, cam.fx, cam.fy, cam.W, cam.H, s["bg"], self.out_rgb,
+                          cam.viewmatrix, cam.projmatrix, cam.fx, cam.fy, cam.W, cam.H, s["bg"],
+                          self.out_rgb if out_rgb is None else out_rgb,
                           self.out_final_T, self.out_tile_counts, self.out_n_contrib if count_contrib else None,
                           self.workspace, stream)
+
+    def render_to_host(self, cam, slot: int = 0, n_slots: int = 1, count_contrib: bool = False) -> torch.Tensor:
+        """Render one frame and copy its RGB image to pinned host slot `slot`, with the copy of frame k overlapping the
+        render of frame k+1: two device images used alternately, the device -> host copy on a second stream, events in
+        both directions.  Returns the host tensor (valid after synchronize_readback())."""
+        if self._host_rgb is None or self._host_rgb.shape[0] < n_slots:
+            self._host_rgb = torch.empty((n_slots, 3, self.H, self.W), dtype=torch.float32).pin_memory()
+        if self._ring is None:
+            self._ring = dict(img=[self.out_rgb, torch.empty_like(self.out_rgb)], k=0,
+                              copy_stream=torch.cuda.Stream(device=self.device),
+                              rendered=[torch.cuda.Event(), torch.cuda.Event()], copied=[torch.cuda.Event(), torch.cuda.Event()],
+                              used=[False, False])
+        rg = self._ring
+        b = rg["k"] & 1
+        rg["k"] += 1
+        main = torch.cuda.current_stream(self.device)
+        if rg["used"][b]:
+            main.wait_event(rg["copied"][b])          # the image rendered two frames ago has left this buffer
+        self.render(cam, count_contrib=count_contrib, out_rgb=rg["img"][b])
+        rg["rendered"][b].record(main)
+        with torch.cuda.stream(rg["copy_stream"]):
+            rg["copy_stream"].wait_event(rg["rendered"][b])
+            self._host_rgb[slot].copy_(rg["img"][b], non_blocking=True)
+            rg["copied"][b].record(rg["copy_stream"])
+        rg["used"][b] = True
+        return self._host_rgb[slot]
+
+    def synchronize_readback(self) -> None:
+        if self._ring is not None:
+            self._ring["copy_stream"].synchronize()
+        torch.cuda.current_stream(self.device).synchronize()
 
     def read_image(self, slot: int = 0, n_slots: int = 1) -> torch.Tensor:
         """Async device -> pinned-host copy of the last frame's RGB image into host slot `slot`; returns the host

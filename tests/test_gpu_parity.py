@@ -254,3 +254,21 @@ def test_global_coordinate_polynomial_loses_precision_at_4k():
     print("max |rgb - oracle|, share of pixels over 2e-3: tile-local %s, global %s" % (err[3], err[6]))
     assert err[3][0] <= pu.TOL_ALL and err[3][1] <= 1e-3
     assert err[6][0] > 10.0 * max(err[3][0], 1e-4) and err[6][0] > pu.TOL_ALL
+
+
+def test_overlapped_readback_returns_the_same_images():
+    """Renderer.render_to_host() double-buffers the device image and copies on a second stream; the host images must be
+    the frames a plain render produces, pose by pose."""
+    sc = scenes.make_scene(2, P=20_000, W=320, H=240, f=400.0)
+    binding.gs_set_render_variant(binding.GS_DEFAULT_RENDER_VARIANT)
+    r = Renderer(sc.P, 320, 240, 1 << 20, device="cuda:0", count_contrib=False)
+    r.upload(sc)
+    n = len(sc.cameras)
+    host = [r.render_to_host(cam, i, n) for i, cam in enumerate(sc.cameras)]
+    r.synchronize_readback()
+    host = [h.clone() for h in host]
+    for i, cam in enumerate(sc.cameras):
+        r.render(cam, count_contrib=False)
+        torch.cuda.synchronize()
+        assert torch.equal(host[i], r.out_rgb.cpu()), "pose %d" % i
+    assert not torch.equal(host[0], host[1])

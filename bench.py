@@ -274,18 +274,28 @@ def run_ours(args):
         if e1 is not None:
             e1.record()
 
+    # A step = every pose of the configuration once, through the public batch call: `lanes` frames in flight on their own
+    # streams and workspaces (Renderer.render_batch).  The L2 is flushed before every step, outside the event pair.
+    lanes = args.lanes if args.lanes > 0 else (1 if r.workspace.numel() < (8 << 20) else (3 if r.workspace.numel() < (4 << 30) else 2))
+
+    def step(e0=None, e1=None):
+        flush.zero_()
+        if e0 is not None:
+            e0.record()
+        r.render_batch(cams, lanes=lanes)
+        if e1 is not None:
+            e1.record()
+
     # ---- pre-warm (clock ramp) + W warm-up steps -------------------------------------------------------------------------
     t0 = time.perf_counter()
     while time.perf_counter() - t0 < 0.5:
-        for cam in cams:
-            frame(cam)
+        step()
         torch.cuda.synchronize()
     for _ in range(args.warmup):
-        for cam in cams:
-            frame(cam)
+        step()
     # ---- timed region: exactly K steps ---------------------------------------------------------------------------------------
     K = args.steps
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K * n_pose)]
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
     sampler = ClockSampler(lrank)
     barrier()
     torch.cuda.synchronize()
@@ -293,10 +303,9 @@ def run_ours(args):
     wall0 = time.perf_counter()
     launches = 0
     for s in range(K):
-        for i, cam in enumerate(cams):
-            e0, e1 = evs[s * n_pose + i]
-            frame(cam, e0, e1)
-            launches += launches_per_frame
+        e0, e1 = evs[s]
+        step(e0, e1)
+        launches += launches_per_frame * n_pose
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
     clocks = sampler.result()
@@ -305,6 +314,18 @@ def run_ours(args):
     dev_ms = rank_max(dev_ms)
     ms_per_step = dev_ms / K
     fps = aggregate_fps(ws, n_pose * K, dev_ms)
+
+    # ---- latency: one frame at a time on one stream, L2 flushed before every frame (the first rounds' `value`) ---------
+    for cam in cams:
+        frame(cam)
+    fevs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(min(K, 20) * n_pose)]
+    torch.cuda.synchronize()
+    for s in range(min(K, 20)):
+        for i, cam in enumerate(cams):
+            e0, e1 = fevs[s * n_pose + i]
+            frame(cam, e0, e1)
+    torch.cuda.synchronize()
+    serial_ms_per_frame = rank_max(sum(e0.elapsed_time(e1) for e0, e1 in fevs) / len(fevs))
 
     # ---- per-stage device times: a second pass with the library's own CUDA events between its kernels -----------
     binding.gs_set_timing(True)
@@ -324,8 +345,7 @@ def run_ours(args):
     # ---- e2e: host buffers in, host images out, every step ----------------------------------------------------------------
     def e2e_step():
         h2d = r.upload(sc)
-        for i, cam in enumerate(cams):
-            r.render_to_host(cam, i, n_pose)      # device -> pinned host copy of frame i overlaps the render of frame i+1
+        r.render_batch(cams, lanes=lanes, to_host=True)   # device -> pinned host copies overlap the later frames
         r.synchronize_readback()
         return h2d
     for _ in range(2):
@@ -385,9 +405,12 @@ def run_ours(args):
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
                 "config": _config_dict(args.config, cfg, sc, extra={
-                    "frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every frame", "parallelism": "replicas x%d" % ws,
+                    "frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every step", "frames_in_flight": lanes,
+                    "parallelism": "replicas x%d" % ws,
                     "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "render_variant": binding.gs_get_render_variant()}),
                 "ms_per_frame": ms_per_step / n_pose, "wall_ms_per_step_incl_flush": 1e3 * wall / K,
+                "latency": {"ms_per_frame": serial_ms_per_frame, "frames_per_s": ws * 1e3 / serial_ms_per_frame,
+                            "how": "one frame in flight, one stream, L2 flushed before every frame"},
                 "clocks": clocks,
                 "e2e": {"value": e2e_fps, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes},
                 "gpu_launches": launches, "launches_per_frame": launches_per_frame,
@@ -407,6 +430,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=(1, 2, 3, 4, 5))
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = chosen from the workspace size)")
     ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -56,9 +56,7 @@ __device__ __forceinline__ void ffma2_acc(u64& acc, u64 a, u64 b) { asm("fma.rn.
 
 struct PixelPair {
     u64 bx2, bxy, by2, bx, by;  // B_local (Eq. 9) of the two pixels, tile-centre origin
-    u64 T, Cr, Cg, Cb;          // T scaled by K; touched by the unconditional blend only
-    u64 thr;                    // per pixel: 1e-4 K while the pixel is live, -(K w of the un-blended entries) once stopped
-    u64 dCr, dCg, dCb;          // colour of the un-blended entries (written by the rare branch only; added at the end)
+    u64 T, Cr, Cg, Cb;          // T scaled by K
     uint32_t n0, n1;
 };
 
@@ -130,27 +128,27 @@ __device__ __forceinline__ void blend_pair(PixelPair& s, const uint32_t a1, cons
         s.n0 += ((e0 > 0.0f) ? 1u : 0u) + ((g0 > 0.0f) ? 1u : 0u);
         s.n1 += ((e1 > 0.0f) ? 1u : 0u) + ((g1 > 0.0f) ? 1u : 0u);
     }
-    float t0, t1, h0, h1;
+    float t0, t1;
     unpk(s.T, t0, t1);
-    unpk(s.thr, h0, h1);
-    if (__any_sync(0xffffffffu, (t0 < h0) || (t1 < h1))) {   // rare; a stopped pixel has thr < 0 <= T: it never fires again
+    if (__any_sync(0xffffffffu, (t0 < TMIN_S) || (t1 < TMIN_S))) {   // rare; a stopped pixel keeps T >= 1e-4 K: it never fires again
         float u0, u1, w10, w11, w20, w21;
         unpk(T1, u0, u1); unpk(w1, w10, w11); unpk(w2, w20, w21);
-        const bool sa0 = u0 < h0, sa1 = u1 < h1;              // stopped at the first entry
-        const bool sb0 = t0 < h0, sb1 = t1 < h1;              // stopped at the first or the second entry
+        const bool sa0 = u0 < TMIN_S, sa1 = u1 < TMIN_S;      // stopped at the first entry
+        const bool sb0 = t0 < TMIN_S, sb1 = t1 < TMIN_S;      // stopped at the first or the second entry
         const u64 wm2 = pk(sb0 ? w20 : 0.0f, sb1 ? w21 : 0.0f), wm1 = pk(sa0 ? w10 : 0.0f, sa1 ? w11 : 0.0f);
-        // thr <- -(K wm1 + K wm2) on the stopping pixels (final T = T - thr there), unchanged elsewhere
-        const u64 live = pk(sb0 ? 0.0f : 1.0f, sb1 ? 0.0f : 1.0f);
-        s.thr = ffma2(bc(-K_SCALE), wm2, fmul2(s.thr, live));
-        ffma2_acc(s.thr, bc(-K_SCALE), wm1);
-        ffma2_acc(s.dCr, bc(-q1.z), wm2);
-        ffma2_acc(s.dCg, bc(-q1.w), wm2);
-        ffma2_acc(s.dCb, bc(-q2.x), wm2);
-        ffma2_acc(s.dCr, bc(-p1.z), wm1);
-        ffma2_acc(s.dCg, bc(-p1.w), wm1);
-        ffma2_acc(s.dCb, bc(-p2.x), wm1);
+        ffma2_acc(s.Cr, bc(-q1.z), wm2);
+        ffma2_acc(s.Cg, bc(-q1.w), wm2);
+        ffma2_acc(s.Cb, bc(-q2.x), wm2);
+        ffma2_acc(s.Cr, bc(-p1.z), wm1);
+        ffma2_acc(s.Cg, bc(-p1.w), wm1);
+        ffma2_acc(s.Cb, bc(-p2.x), wm1);
+        ffma2_acc(s.T, bc(K_SCALE), wm2);
+        ffma2_acc(s.T, bc(K_SCALE), wm1);
+        float r0, r1;
+        unpk(s.T, r0, r1);   // the T of rule R1 passed the test when it was formed: >= 1e-4 K up to the rounding of the repair
+        s.T = pk(sb0 ? fmaxf(r0, TMIN_S) : r0, sb1 ? fmaxf(r1, TMIN_S) : r1);
         ffma2_acc(s.bx2, pk(sb0 ? 1.0f : 0.0f, sb1 ? 1.0f : 0.0f), bc(POISON));
-        if (COUNT) {  // a pixel stopped at the first entry also counted the second one when its alpha was > 0
+        if (COUNT) {
             s.n0 -= (sa0 ? 1u + ((g0 > 0.0f) ? 1u : 0u) : (sb0 ? 1u : 0u));
             s.n1 -= (sa1 ? 1u + ((g1 > 0.0f) ? 1u : 0u) : (sb1 ? 1u : 0u));
         }
@@ -163,10 +161,12 @@ __device__ __forceinline__ void blend_pair(PixelPair& s, const uint32_t a1, cons
 // Walk of one warp's list (two entries per iteration; the list is padded to an even length with the null record).
 template <bool COUNT, bool GUARD>
 __device__ __forceinline__ void blend_list(PixelPair& s, uint32_t& lp, uint32_t& lend) {
+    uint2 aa = lds64u(lp);
     while (lp < lend) {
-        const uint2 aa = lds64u(lp);
         lp += 8;
+        const uint2 nx = lds64u(lp);   // the pair after this one (the list buffer has room for one pair past the padding)
         blend_pair<COUNT, GUARD>(s, aa.x, aa.y, lend);
+        aa = nx;
     }
 }
 
@@ -178,7 +178,7 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
     __shared__ __align__(16) unsigned char s_rec[2][(QB + 1) * REC];  // staged, hoisted records (double-buffered) + a null record
     __shared__ __align__(16) uint32_t s_ball[2][4][4];          // [buffer][staging warp][quadrant] mask ballots
     __shared__ __align__(16) uint32_t s_indef[2][4];                        // [buffer][staging warp] batch holds an indefinite conic
-    __shared__ __align__(16) uint32_t s_list[4][QB + 2];        // per-warp compacted lists of record addresses (padded to even length)
+    __shared__ __align__(16) uint32_t s_list[4][QB + 4];        // per-warp compacted lists of record addresses (padded to even length)
     griddep_sync();
     const int tid = threadIdx.x, lane = tid & 31;
     // warp index through a warp reduction: ptxas then KNOWS it is warp-uniform (it lives in a uniform register), so
@@ -204,8 +204,7 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
         s.bx = pk(x0, x1);
         s.by = pk(y, y);
         s.T = pk(K_SCALE, K_SCALE);
-        s.Cr = s.Cg = s.Cb = s.dCr = s.dCg = s.dCb = pk(0.0f, 0.0f);
-        s.thr = pk(TMIN_S, TMIN_S);
+        s.Cr = s.Cg = s.Cb = pk(0.0f, 0.0f);
         s.n0 = s.n1 = 0;
     }
     if (tid < 6) {  // null record of both buffers: F = -huge, alpha = 0 exactly; colours 0
@@ -291,15 +290,9 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
     }
     // ---- epilogue: out = C + T bg (reading S16) -------------------------------------------------------------------
     float T0, T1, c0r, c1r, c0g, c1g, c0b, c1b;
-    {   // fold the repairs of the stopped pixels in: T = T - thr where thr < 0, C = C + dC
-        float h0, h1, d0, d1;
-        unpk(s.T, T0, T1); unpk(s.thr, h0, h1);
-        T0 = (h0 < 0.0f ? T0 - h0 : T0) * K_INV;
-        T1 = (h1 < 0.0f ? T1 - h1 : T1) * K_INV;
-        unpk(s.Cr, c0r, c1r); unpk(s.dCr, d0, d1); c0r += d0; c1r += d1;
-        unpk(s.Cg, c0g, c1g); unpk(s.dCg, d0, d1); c0g += d0; c1g += d1;
-        unpk(s.Cb, c0b, c1b); unpk(s.dCb, d0, d1); c0b += d0; c1b += d1;
-    }
+    unpk(s.T, T0, T1);
+    T0 *= K_INV; T1 *= K_INV;
+    unpk(s.Cr, c0r, c1r); unpk(s.Cg, c0g, c1g); unpk(s.Cb, c0b, c1b);
     const size_t npix = (size_t)f.W * f.H, pix = (size_t)py * f.W + px;
     if (in1 && !(f.W & 1)) {  // both pixels inside, 8-byte aligned pair
         *reinterpret_cast<float2*>(out_rgb + pix) = make_float2(fmaf(T0, f.bg[0], c0r), fmaf(T1, f.bg[0], c1r));
@@ -369,7 +362,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 struct WsShared {
     __align__(16) unsigned char rec[WS_NSTAGE][WS_SB * REC];  // staged, hoisted records
     __align__(16) unsigned char null_rec[REC];                // F = -huge: alpha = 0 exactly (list padding)
-    __align__(16) uint32_t list[WS_NSTAGE][4][WS_SB + 2];     // per stage, per quadrant: record addresses, in list order
+    __align__(16) uint32_t list[WS_NSTAGE][4][WS_SB + 4];     // per stage, per quadrant: record addresses, in list order
     __align__(16) uint4 hdr[WS_NSTAGE];                       // {flags, tile, tile sequence number, 4 x 8-bit list lengths}
     __align__(8) unsigned long long full[WS_NSTAGE], empty[WS_NSTAGE];
     uint32_t qid[2 * WS_SB];                                  // producers: queue of Gaussian ids that reach the tile
@@ -384,15 +377,9 @@ __device__ __forceinline__ void ws_write_pixels(const Frame& f, const PixelPair&
                                                 float* __restrict__ out_rgb, float* __restrict__ out_T,
                                                 uint32_t* __restrict__ out_n) {
     float T0, T1, c0r, c1r, c0g, c1g, c0b, c1b;
-    {   // fold the repairs of the stopped pixels in: T = T - thr where thr < 0, C = C + dC
-        float h0, h1, d0, d1;
-        unpk(s.T, T0, T1); unpk(s.thr, h0, h1);
-        T0 = (h0 < 0.0f ? T0 - h0 : T0) * K_INV;
-        T1 = (h1 < 0.0f ? T1 - h1 : T1) * K_INV;
-        unpk(s.Cr, c0r, c1r); unpk(s.dCr, d0, d1); c0r += d0; c1r += d1;
-        unpk(s.Cg, c0g, c1g); unpk(s.dCg, d0, d1); c0g += d0; c1g += d1;
-        unpk(s.Cb, c0b, c1b); unpk(s.dCb, d0, d1); c0b += d0; c1b += d1;
-    }
+    unpk(s.T, T0, T1);
+    T0 *= K_INV; T1 *= K_INV;
+    unpk(s.Cr, c0r, c1r); unpk(s.Cg, c0g, c1g); unpk(s.Cb, c0b, c1b);
     const size_t npix = (size_t)f.W * f.H, pix = (size_t)py * f.W + px;
     if (in1 && !(f.W & 1)) {  // both pixels inside, 8-byte aligned pair
         __stcs(reinterpret_cast<float2*>(out_rgb + pix), make_float2(fmaf(T0, f.bg[0], c0r), fmaf(T1, f.bg[0], c1r)));
@@ -433,7 +420,7 @@ __device__ __forceinline__ void ws_consumer(const Frame& f, WsShared& sm, Ctrl* 
     s.by2 = pk(y * y, y * y);
     s.bx = pk(x0, x1);
     s.by = pk(y, y);
-    s.bx2 = s.T = s.Cr = s.Cg = s.Cb = s.dCr = s.dCg = s.dCb = s.thr = pk(0.0f, 0.0f);
+    s.bx2 = s.T = s.Cr = s.Cg = s.Cb = pk(0.0f, 0.0f);
     s.n0 = s.n1 = 0;
     bool wdone = true, written = true, in0 = false, in1 = false;
     int px = 0, py = 0;
@@ -450,8 +437,7 @@ __device__ __forceinline__ void ws_consumer(const Frame& f, WsShared& sm, Ctrl* 
             in0 = px < f.W && py < f.H; in1 = (px + 1) < f.W && py < f.H;
             s.bx2 = pk(in0 ? x0 * x0 : POISON, in1 ? x1 * x1 : POISON);
             s.T = pk(K_SCALE, K_SCALE);
-            s.Cr = s.Cg = s.Cb = s.dCr = s.dCg = s.dCb = pk(0.0f, 0.0f);
-            s.thr = pk(TMIN_S, TMIN_S);
+            s.Cr = s.Cg = s.Cb = pk(0.0f, 0.0f);
             s.n0 = s.n1 = 0;
             seq = h.z;
             written = false;
@@ -460,7 +446,7 @@ __device__ __forceinline__ void ws_consumer(const Frame& f, WsShared& sm, Ctrl* 
         }
         if (!wdone) {
             const uint32_t cnt = (h.w >> (8 * w)) & 255u;
-            uint32_t lp = list0 + slot * (uint32_t)(4 * (WS_SB + 2) * 4);
+            uint32_t lp = list0 + slot * (uint32_t)(4 * (WS_SB + 4) * 4);
             const uint32_t lp0 = lp;
             uint32_t lend = lp + 4 * cnt;
             if (h.x & WS_INDEF) blend_list<COUNT, true>(s, lp, lend);
@@ -644,7 +630,7 @@ __device__ __forceinline__ void ws_producer(const Frame& f, WsShared& sm, Ctrl* 
             // per-quadrant compacted lists of record addresses, in list order (warp 0's entries first)
             const uint32_t rec_addr = (uint32_t)__cvta_generic_to_shared(&sm.rec[slot][pt * REC]);
             uint32_t* L0 = &sm.list[slot][0][0];
-            constexpr int LS = WS_SB + 2;
+            constexpr int LS = WS_SB + 4;
             if (m & 1u) L0[0 * LS + (pw ? c0.x : 0u) + __popc(b0 & lt)] = rec_addr;
             if (m & 2u) L0[1 * LS + (pw ? c0.y : 0u) + __popc(b1 & lt)] = rec_addr;
             if (m & 4u) L0[2 * LS + (pw ? c0.z : 0u) + __popc(b2 & lt)] = rec_addr;

@@ -29,6 +29,8 @@ class Renderer:
         self._pinned = None   # host staging of the scene arrays (pinned), allocated on the first upload
         self._host_rgb = None
         self._ring = None     # render_to_host(): two device images, a copy stream and the events that order them
+        self._lanes = None    # render_batch(): per-lane stream, workspace and outputs
+        self._copy_stream = None
 
     def upload(self, scene) -> int:
         """Host (numpy) scene -> device tensors: pinned staging, async copies on the current stream.  The staging and
@@ -78,9 +80,81 @@ class Renderer:
         rg["used"][b] = True
         return self._host_rgb[slot]
 
+    # ---- several frames in flight ---------------------------------------------------------------------------------
+    def _lane(self, k: int):
+        """Lane k: its own stream, workspace and output buffers (lane 0 = this Renderer's own buffers, on its own
+        stream too, so that the caller's stream only forks and joins)."""
+        if self._lanes is None:
+            self._lanes = []
+        while len(self._lanes) <= k:
+            first = len(self._lanes) == 0
+            ln = dict(stream=torch.cuda.Stream(device=self.device),
+                      workspace=self.workspace if first else torch.empty_like(self.workspace),
+                      out_rgb=self.out_rgb if first else torch.empty_like(self.out_rgb),
+                      out_final_T=self.out_final_T if first else torch.empty_like(self.out_final_T),
+                      out_tile_counts=self.out_tile_counts if first else torch.empty_like(self.out_tile_counts),
+                      done=torch.cuda.Event(), copied=torch.cuda.Event(), copy_pending=False)
+            self._lanes.append(ln)
+        return self._lanes[k]
+
+    def render_batch(self, cams, lanes: int = 3, out_rgb=None, to_host: bool = False):
+        """Render every camera of `cams`, `lanes` frames in flight: frame i runs on lane i % lanes (own stream, own
+        workspace).  Frames are independent, so the small, latency-bound kernels of one frame's binning fill the GPU
+        under the render kernel of another; every frame is computed by exactly the same launches as render().
+          out_rgb   optional device tensor [len(cams), 3, H, W]: frame i writes its image there (otherwise the image of
+                    frame i stays in lane i % lanes until frame i + lanes overwrites it);
+          to_host   copy every image to pinned host memory on a copy stream, overlapping the later frames; returns the
+                    host tensor [len(cams), 3, H, W] (valid when this call returns control to the current stream's
+                    order: the current stream waits for all lanes and copies).
+        The current stream is joined to all lanes before returning, so later work on it sees the results."""
+        n = len(cams)
+        lanes = max(1, min(int(lanes), n))
+        main = torch.cuda.current_stream(self.device)
+        fork = torch.cuda.Event()
+        fork.record(main)
+        host = None
+        if to_host:
+            if self._host_rgb is None or self._host_rgb.shape[0] < n:
+                self._host_rgb = torch.empty((n, 3, self.H, self.W), dtype=torch.float32).pin_memory()
+            host = self._host_rgb[:n]
+            if self._copy_stream is None:
+                self._copy_stream = torch.cuda.Stream(device=self.device)
+        s = self.scene
+        for i, cam in enumerate(cams):
+            ln = self._lane(i % lanes)
+            st = ln["stream"]
+            if i < lanes:
+                st.wait_event(fork)
+            if ln["copy_pending"]:
+                st.wait_event(ln["copied"])          # the image of frame i - lanes has left this lane's buffer
+                ln["copy_pending"] = False
+            img = ln["out_rgb"] if out_rgb is None else out_rgb[i]
+            binding.gs_render(s["means3D"], s["scales"], s["rotations"], s["opacities"], s["sh"], s["sh_degree"],
+                              cam.viewmatrix, cam.projmatrix, cam.fx, cam.fy, cam.W, cam.H, s["bg"], img,
+                              ln["out_final_T"], ln["out_tile_counts"], None, ln["workspace"], st)
+            ln["done"].record(st)
+            if to_host:
+                cs = self._copy_stream
+                cs.wait_event(ln["done"])
+                with torch.cuda.stream(cs):
+                    host[i].copy_(img, non_blocking=True)
+                ln["copied"].record(cs)
+                ln["copy_pending"] = True
+        for k in range(lanes):
+            main.wait_event(self._lanes[k]["done"])
+        if to_host:
+            done = torch.cuda.Event()
+            done.record(self._copy_stream)
+            main.wait_event(done)
+            for k in range(lanes):
+                self._lanes[k]["copy_pending"] = False
+        return host
+
     def synchronize_readback(self) -> None:
         if self._ring is not None:
             self._ring["copy_stream"].synchronize()
+        if self._copy_stream is not None:
+            self._copy_stream.synchronize()
         torch.cuda.current_stream(self.device).synchronize()
 
     def read_image(self, slot: int = 0, n_slots: int = 1) -> torch.Tensor:

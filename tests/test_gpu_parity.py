@@ -272,3 +272,33 @@ def test_overlapped_readback_returns_the_same_images():
         torch.cuda.synchronize()
         assert torch.equal(host[i], r.out_rgb.cpu()), "pose %d" % i
     assert not torch.equal(host[0], host[1])
+
+
+@pytest.mark.parametrize("lanes", [1, 2, 3])
+def test_render_batch_frames_in_flight_equal_plain_renders(lanes):
+    """Renderer.render_batch() keeps several frames in flight, each on its own stream and workspace; every image (written
+    to a caller tensor, and copied to host memory on the copy stream) must be bit-identical to the frame a plain
+    render() of the same pose produces, and so must the tile counts of the last frame of every lane."""
+    sc = scenes.make_scene(2, P=20_000, W=320, H=240, f=400.0)
+    binding.gs_set_render_variant(binding.GS_DEFAULT_RENDER_VARIANT)
+    r = Renderer(sc.P, 320, 240, 1 << 20, device="cuda:0", count_contrib=False)
+    r.upload(sc)
+    cams = list(sc.cameras)
+    n = len(cams)
+    dev_imgs = torch.empty((n, 3, 240, 320), dtype=torch.float32, device="cuda:0")
+    for rep in range(2):                                   # the second batch reuses lanes, events and host slots
+        host = r.render_batch(cams, lanes=lanes, out_rgb=dev_imgs, to_host=True)
+        torch.cuda.current_stream().synchronize()
+        host = host.clone()
+        host2 = r.render_batch(cams, lanes=lanes, to_host=True)   # images left in the lanes' own buffers
+        torch.cuda.current_stream().synchronize()
+        assert torch.equal(host, host2.clone())
+    lane_counts = [r._lanes[k]["out_tile_counts"].clone() for k in range(min(lanes, n))]
+    for i, cam in enumerate(cams):
+        r.render(cam, count_contrib=False)
+        torch.cuda.synchronize()
+        assert torch.equal(host[i], r.out_rgb.cpu()), "pose %d (host copy)" % i
+        assert torch.equal(dev_imgs[i], r.out_rgb), "pose %d (device tensor)" % i
+        if i >= n - min(lanes, n):
+            assert torch.equal(lane_counts[i % lanes], r.out_tile_counts), "pose %d (tile counts)" % i
+    assert not torch.equal(host[0], host[1])

@@ -78,16 +78,20 @@ typedef struct gs_intermediates {
                                       [11] x*  [12] 1/c  [13] c*tau: per-Gaussian constants of the tight box
                                       (Eq. 13-18; tau = 2 ln(255 o) widened)   [14..15] 0                        */
     const uint64_t* depth_sorted;  /* dev [n_visible]: (depth bits << 32 | Gaussian id), ascending, stable       */
-    const uint32_t* dup_offsets;   /* dev [n_visible]: exclusive prefix sum of tiles_touched in depth order      */
+    const uint32_t* dup_offsets;   /* dev [n_visible]: exclusive prefix sum, in depth order, of the number of
+                                      SUPER-TILES (8 x 8 tiles) each Gaussian's tile rect reaches -- the level the
+                                      duplication and the sort run on (two-level binning)                        */
     const uint32_t* tile_ranges;   /* dev [n_tiles+1]: list of tile t is sorted_ids[tile_ranges[t] .. [t+1])     */
     const uint32_t* sorted_ids;    /* dev [min(n_dup,max_dup)]: Gaussian ids, by (tile, depth bits, id)          */
+    uint64_t n_coarse;             /* duplicated (super-tile, Gaussian) entries that were actually sorted        */
 } gs_intermediates;
 int gs_get_intermediates(const void* workspace, gs_intermediates* out);
 
 /* Per-stage device times (ms, CUDA events) of the last gs_render() on this workspace made while timing was
  * enabled with gs_set_timing(1): [0] preprocess, [1] depth sort, [2] tile grid, [3] offset scan, [4] duplicate,
- * [5] tile sort, [6] render, [7] whole frame.  [4] is the duplication -- fused with the first tile pass on frames with a
- * capacity of <= 4 M entries -- and [5] the remaining tile passes.  Enabling timing adds event records and one stream
+ * [5] tile sort, [6] render, [7] whole frame.  [4] is the duplication over super-tiles -- fused with the first radix pass
+ * on frames with a capacity of <= 4 M entries -- and [5] the remaining radix passes plus the expansion of the super-tile
+ * lists into the tile lists.  Enabling timing adds event records and one stream
  * synchronisation per frame, serialises the tile-grid kernel (otherwise on a side stream, concurrent with the depth sort)
  * and disables programmatic dependent launch, so that every stage time is that stage alone; it is off by default. */
 #define GS_N_TIMINGS 8

@@ -33,7 +33,7 @@ class _Intermediates(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("P", "W", "H", "grid_x", "grid_y", "n_tiles")] + [
         ("n_visible", C.c_uint32), ("n_dup", C.c_uint64), ("max_dup", C.c_uint64),
         ("per_gaussian", C.c_void_p), ("record", C.c_void_p), ("depth_sorted", C.c_void_p),
-        ("dup_offsets", C.c_void_p), ("tile_ranges", C.c_void_p), ("sorted_ids", C.c_void_p)]
+        ("dup_offsets", C.c_void_p), ("tile_ranges", C.c_void_p), ("sorted_ids", C.c_void_p), ("n_coarse", C.c_uint64)]
 
 
 class GsError(RuntimeError):
@@ -153,7 +153,8 @@ def gs_get_intermediates(workspace, copy=("per_gaussian", "tile_ranges", "sorted
     if rc not in (GS_OK, GS_ERR_OVERFLOW):
         raise GsError(rc, "gs_get_intermediates")
     out = SimpleNamespace(P=it.P, W=it.W, H=it.H, grid_x=it.grid_x, grid_y=it.grid_y, n_tiles=it.n_tiles,
-                          n_visible=int(it.n_visible), n_dup=int(it.n_dup), max_dup=int(it.max_dup), overflow=rc == GS_ERR_OVERFLOW)
+                          n_visible=int(it.n_visible), n_dup=int(it.n_dup), max_dup=int(it.max_dup), n_coarse=int(it.n_coarse),
+                          overflow=rc == GS_ERR_OVERFLOW)
     if rc == GS_ERR_OVERFLOW:
         e = GsError(rc, "gs_get_intermediates")
         e.n_dup = out.n_dup

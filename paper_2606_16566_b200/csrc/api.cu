@@ -15,8 +15,9 @@ int g_use_pdl = 1;
 void launch_preprocess(const Frame&, const Pointers&, const float*, const float*, const float*, const float*, const float*,
                        int, cudaStream_t);
 void launch_depth_sort(const Frame&, const Pointers&, int, cudaStream_t, int*);
-void launch_tile_grid(const Frame&, const Pointers&, uint32_t*, cudaStream_t, int*);
-void launch_scan_offsets(const Frame&, const Pointers&, int, cudaStream_t, int*);
+void launch_tile_grid(const Frame&, const Pointers&, uint32_t*, const Ctrl*, cudaStream_t, int*);
+void launch_scan_offsets(const Frame&, const Pointers&, int, int, cudaStream_t, int*);
+void launch_expand(const Frame&, const Pointers&, cudaStream_t, int*);
 void launch_duplicate_and_tile_sort(const Frame&, const Pointers&, int, cudaStream_t, int*, cudaEvent_t);
 void launch_atomic_order_selftest(unsigned long long*, int, uint32_t, int, int, cudaStream_t);
 void launch_render_ladder(int, const Frame&, const Pointers&, float*, float*, uint32_t*, cudaStream_t);
@@ -31,10 +32,12 @@ constexpr size_t ALIGN = 256;
 size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t ctrl, diff, st_pre, st_scan, st_depth, st_tile, zero_end;
-    size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, desc, entA, entB, ids, total;
+    size_t ctrl, cctrl, diff, cdiff, st_pre, st_scan, st_depth, st_tile, zero_end;
+    size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, desc, cranges, ccounts, entA, entB, cids, ids, total;
     size_t n_depth_tiles, n_tile_tiles;
     int gx, gy, n_tiles, tile_bits, n_tile_passes, diff_copies, diff_cells;
+    int cgx, cgy, n_ctiles, cdiff_cells;
+    bool two_level;
 };
 
 bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
@@ -44,8 +47,15 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     const long long nt = (long long)L.gx * L.gy;
     if (nt > (1ll << 24) || L.gx > 65535 || L.gy > 65535) return false;
     L.n_tiles = (int)nt;
+    // Large frames (capacity > FUSED_DUP_MAX) bin in TWO LEVELS: duplication + sort run on the super-tile grid, whose id
+    // width then sets the number of radix passes, and expand_kernel writes the tile lists.  Small frames sort tile ids.
+    L.two_level = max_dup > FUSED_DUP_MAX;
+    L.cgx = L.two_level ? (L.gx + SUPER - 1) / SUPER : 0;
+    L.cgy = L.two_level ? (L.gy + SUPER - 1) / SUPER : 0;
+    L.n_ctiles = L.cgx * L.cgy;
+    L.cdiff_cells = L.two_level ? (L.cgx + 1) * (L.cgy + 1) : 0;
     L.tile_bits = 1;
-    while ((1ll << L.tile_bits) < nt) L.tile_bits++;
+    while ((1ll << L.tile_bits) < (L.two_level ? (long long)L.n_ctiles : nt)) L.tile_bits++;
     L.n_tile_passes = (L.tile_bits + 7) / 8;
     const size_t Pz = (size_t)P;
     const size_t depth_tile = (size_t)SORT_THREADS * sort_items_for(Pz), ent_tile = (size_t)SORT_THREADS * dup_items_for(max_dup);  // the smaller of the tile passes' tiles
@@ -54,10 +64,12 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o = up(o + bytes); return at; };
     L.ctrl = take(sizeof(Ctrl));
+    L.cctrl = take(sizeof(Ctrl));
     L.diff_cells = (L.gx + 1) * (L.gy + 1);
     L.diff_copies = 1;   // replicas of the coverage grid (spreads the hot corner counters of small grids)
     while (L.diff_copies < 16 && (long long)L.diff_cells * L.diff_copies * 2 <= 65536) L.diff_copies *= 2;
     L.diff = take(sizeof(int) * (size_t)L.diff_cells * L.diff_copies);
+    L.cdiff = take(sizeof(int) * (size_t)L.cdiff_cells);
     L.st_pre = take(8 * ((Pz + 31) / 32 + 1));
     L.st_scan = take(8 * ((Pz + SCAN_WARP_TILE - 1) / SCAN_WARP_TILE + 1));
     L.st_depth = take(8 * 256 * L.n_depth_tiles * MAX_SORT_PASSES_DEPTH);
@@ -72,8 +84,14 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     L.chunk_start = take(4 * (((size_t)max_dup + DUP_TILE - 1) / DUP_TILE + 2));
     L.ranges = take(4 * ((size_t)L.n_tiles + 1));
     L.desc = take(16 * (size_t)L.n_tiles);
-    L.entA = take(8 * (size_t)max_dup);
+    L.cranges = take(4 * ((size_t)L.n_ctiles + 1));
+    L.ccounts = take(4 * (size_t)L.n_ctiles);
+    // Two-level frames with <= 2 radix passes over packed entries (P <= 2^24) use at most the first half of entA (packed
+    // 4-byte entries between the two passes), so the sorted super-tile ids (cids) live in its second half.
+    const bool cids_in_entA = L.two_level && L.n_tile_passes <= 2 && P <= (1 << 24);
+    L.entA = take(8 * (size_t)max_dup + (cids_in_entA ? 2 * ALIGN : 0));
     L.entB = take((L.n_tile_passes >= 3 || max_dup > FUSED_DUP_MAX) ? 8 * (size_t)max_dup : 0);
+    L.cids = !L.two_level ? L.entA : (cids_in_entA ? up(L.entA + 4 * (size_t)max_dup) : take(4 * (size_t)max_dup + 16));
     L.ids = take(4 * (size_t)max_dup + 16);
     L.total = o;
     return true;
@@ -105,7 +123,12 @@ Pointers carve(void* ws, const Layout& L) {
     char* b = static_cast<char*>(ws);
     Pointers p;
     p.ctrl = reinterpret_cast<Ctrl*>(b + L.ctrl);
+    p.cctrl = reinterpret_cast<Ctrl*>(b + L.cctrl);
     p.diff = reinterpret_cast<int*>(b + L.diff);
+    p.cdiff = reinterpret_cast<int*>(b + L.cdiff);
+    p.cranges = reinterpret_cast<uint32_t*>(b + L.cranges);
+    p.ccounts = reinterpret_cast<uint32_t*>(b + L.ccounts);
+    p.cids = reinterpret_cast<uint32_t*>(b + L.cids);
     p.st_pre = reinterpret_cast<unsigned long long*>(b + L.st_pre);
     p.st_scan = reinterpret_cast<unsigned long long*>(b + L.st_scan);
     p.st_depth = reinterpret_cast<unsigned long long*>(b + L.st_depth);
@@ -133,9 +156,10 @@ Pointers carve(void* ws, const Layout& L) {
 bool fit_max_dup(int P, int W, int H, size_t bytes, unsigned long long& max_dup) {
     Layout L;
     if (!make_layout(P, W, H, 0, L) || L.total > bytes) return false;
-    const unsigned long long edge = 256ull << 10;  // sort_items_for: capacity <= edge -> small tiles
-    const unsigned long long lo_of[2] = {edge + 1, 0}, hi_of[2] = {(1ull << 32) - 1, edge};
-    for (int r = 0; r < 2; r++) {
+    // regime edges: sort_items_for (256 K: small radix tiles) and FUSED_DUP_MAX (two-level binning, second entry buffer)
+    const unsigned long long e1 = 256ull << 10, e2 = FUSED_DUP_MAX;
+    const unsigned long long lo_of[3] = {e2 + 1, e1 + 1, 0}, hi_of[3] = {(1ull << 32) - 1, e2, e1};
+    for (int r = 0; r < 3; r++) {
         unsigned long long lo = lo_of[r], hi = hi_of[r];
         make_layout(P, W, H, lo, L);
         if (L.total > bytes) continue;
@@ -188,6 +212,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     f.tile_bits = L.tile_bits; f.n_tile_passes = L.n_tile_passes;
     f.compact = P >= COMPACT_MIN_P ? 1 : 0;
     f.diff_copies = L.diff_copies; f.diff_cells = L.diff_cells;
+    f.cgx = L.cgx; f.cgy = L.cgy; f.n_ctiles = L.n_ctiles; f.cdiff_cells = L.cdiff_cells;
     for (int k = 0; k < 16; k++) { f.V[k] = viewmatrix[k]; f.PM[k] = projmatrix[k]; }
     f.fx = fx; f.fy = fy;
     // camera centre of the rigid view matrix: campos = -Wv^T t (the north_star signature carries no campos)
@@ -197,6 +222,11 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     for (int c = 0; c < 3; c++) f.bg[c] = bg[c];
     f.max_dup = max_dup;
     const Pointers p = carve(workspace, L);
+    // the super-tile level of the binning: the same kernels on the coarse grid, with their own control block
+    Frame fc = f;
+    fc.gx = f.cgx; fc.gy = f.cgy; fc.n_tiles = f.n_ctiles; fc.diff_copies = 1; fc.diff_cells = f.cdiff_cells;
+    Pointers pc = p;
+    pc.ctrl = p.cctrl; pc.diff = p.cdiff; pc.ranges = p.cranges; pc.desc = nullptr; pc.ids = p.cids;
 
     const bool timed = g_timing.load() != 0;
     LastCall* lc;
@@ -245,20 +275,33 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     // The tile grid (counts, ranges, N_dup, tile-digit histograms) depends on the preprocess only: it runs on a side
     // stream, concurrently with the depth sort (fork / join with two events).  With timing enabled the stages are
     // serialised on the caller's stream so that every per-stage time is that stage alone.
+    const bool two_level = L.two_level;
     if (!timed) {
         cudaEventRecord(lc->ev_fork, st);
         cudaStreamWaitEvent(lc->side, lc->ev_fork, 0);
-        launch_tile_grid(f, p, out_tile_counts, lc->side, &launches);
+        launch_tile_grid(f, p, out_tile_counts, nullptr, lc->side, &launches);
+        if (two_level) launch_tile_grid(fc, pc, p.ccounts, p.ctrl, lc->side, &launches);
         cudaEventRecord(lc->ev_join, lc->side);
     }
     launch_depth_sort(f, p, g_n_sm, st, &launches);          // (3a) LSD passes over the depth bits, pre-duplication
     mark(2);
-    if (timed) launch_tile_grid(f, p, out_tile_counts, st, &launches);
-    else cudaStreamWaitEvent(st, lc->ev_join, 0);
+    if (timed) {
+        launch_tile_grid(f, p, out_tile_counts, nullptr, st, &launches);
+        if (two_level) launch_tile_grid(fc, pc, p.ccounts, p.ctrl, st, &launches);
+    } else {
+        cudaStreamWaitEvent(st, lc->ev_join, 0);
+    }
     mark(3);
-    launch_scan_offsets(f, p, g_n_sm, st, &launches);         // (2) prefix-sum offsets
-    mark(4);
-    launch_duplicate_and_tile_sort(f, p, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b)
+    if (two_level) {
+        launch_scan_offsets(fc, pc, SUPER_SHIFT, g_n_sm, st, &launches);   // (2) prefix-sum offsets of the super-tile duplicates
+        mark(4);
+        launch_duplicate_and_tile_sort(fc, pc, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b) on super-tiles
+        launch_expand(f, p, st, &launches);                  // (3c) super-tile lists -> tile lists, written in place
+    } else {
+        launch_scan_offsets(f, p, 0, g_n_sm, st, &launches);  // (2) prefix-sum offsets
+        mark(4);
+        launch_duplicate_and_tile_sort(f, p, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b)
+    }
     mark(6);
     const int variant = g_variant.load();                      // (4) render
     if (variant == 5) launch_render_ws(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
@@ -302,6 +345,12 @@ int gs_get_intermediates(const void* workspace, gs_intermediates* out) {
     out->dup_offsets = p.dup_off;
     out->tile_ranges = p.ranges;
     out->sorted_ids = p.ids;
+    {
+        Ctrl cc;
+        e = cudaMemcpy(&cc, static_cast<const char*>(workspace) + lc.L.cctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return cuda_fail(e);
+        out->n_coarse = lc.L.two_level ? cc.n_dup_eff : 0ull;
+    }
     return c.overflow ? GS_ERR_OVERFLOW : GS_OK;
 }
 

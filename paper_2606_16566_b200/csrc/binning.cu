@@ -206,7 +206,7 @@ __device__ __forceinline__ int lpt_bucket(uint32_t c) {
     return l - 4 > 7 ? 7 : l - 4;     // 64..127 -> 2, 128..255 -> 3, ..., >= 2048 -> 7
 }
 __global__ void __launch_bounds__(GRID_THREADS)
-tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts /* out_tile_counts */) {
+tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts /* out_tile_counts */, const Ctrl* __restrict__ parent) {
     __shared__ uint32_t s_hist[MAX_SORT_PASSES_TILE][256];
     __shared__ unsigned long long s_part[GRID_THREADS / 32];
     __shared__ unsigned long long s_total;
@@ -300,12 +300,13 @@ tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts 
 #pragma unroll
     for (int k = 0; k < LPT_BUCKETS; k++) pos[k] = s_bbase[k] + s_wb[w][k] + cinc[k] - cb[k];
     const unsigned long long total = s_total;
-    const bool overflow = total > f.max_dup;
+    // the super-tile level (parent != nullptr) follows the verdict of the tile level: its total is never larger
+    const bool overflow = total > f.max_dup || (parent != nullptr && parent->overflow != 0ull);
     unsigned long long run = s_part[w] + inc - sum;
     for (int t = t0; t < t1; t++) {
         const uint32_t c = counts[t];
         p.ranges[t] = overflow ? 0u : (uint32_t)run;
-        {   // tile descriptor at its slot of the render schedule
+        if (p.desc != nullptr) {   // tile descriptor at its slot of the render schedule
             const int bk = lpt_bucket(c);
             uint32_t slot = 0;
 #pragma unroll
@@ -324,6 +325,7 @@ tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts 
         p.ctrl->n_dup = total;
         p.ctrl->n_dup_eff = overflow ? 0ull : total;
         p.ctrl->overflow = overflow ? 1ull : 0ull;
+        if (parent != nullptr) p.ctrl->n_vis = parent->n_vis;
     }
     __syncthreads();
     for (int k = tid; k < MAX_SORT_PASSES_TILE * 256; k += GRID_THREADS) (&p.ctrl->tile_hist[0][0])[k] = (&s_hist[0][0])[k];
@@ -342,7 +344,7 @@ __device__ __forceinline__ uint32_t rect_tiles(const uint4 pg) {
 // One WARP per 256-rank tile (8 consecutive ranks per lane), chained through the look-back status words; no block
 // barrier.  The rect of every rank is gathered once here and stored in depth order for the duplicate kernel.
 __global__ void __launch_bounds__(SCAN_THREADS)
-scan_offsets_kernel(const Pointers p) {
+scan_offsets_kernel(const Pointers p, const int cshift) {
     griddep_sync();
     const int lane = threadIdx.x & 31;
     const unsigned long long n = p.ctrl->n_vis;
@@ -373,7 +375,14 @@ scan_offsets_kernel(const Pointers p) {
             tt[k] = 0;
             rc[k] = make_uint2(0u, 0u);
             if (id[k] != 0xffffffffu) {
-                const uint4 pg = __ldg(p.per_g + id[k]);
+                uint4 pg = __ldg(p.per_g + id[k]);
+                {   // the tile rect on the grid the duplication runs on: cells of 2^cshift x 2^cshift tiles, half-open
+                    const uint32_t r = (1u << cshift) - 1u;
+                    const uint32_t x0 = (pg.x & 0xffffu) >> cshift, y0 = (pg.x >> 16) >> cshift;
+                    const uint32_t x1 = ((pg.y & 0xffffu) + r) >> cshift, y1 = ((pg.y >> 16) + r) >> cshift;
+                    pg.x = x0 | (y0 << 16);
+                    pg.y = x1 | (y1 << 16);
+                }
                 rc[k] = make_uint2(pg.x, pg.y);
                 tt[k] = rect_tiles(pg);
             }
@@ -642,15 +651,15 @@ void launch_depth_sort(const Frame& f, const Pointers& p, int n_sm, cudaStream_t
     }
 }
 
-void launch_tile_grid(const Frame& f, const Pointers& p, uint32_t* out_tile_counts, cudaStream_t st, int* launches) {
-    launch_pdl(tile_grid_kernel, dim3(1), dim3(GRID_THREADS), st, f, p, out_tile_counts);
+void launch_tile_grid(const Frame& f, const Pointers& p, uint32_t* out_tile_counts, const Ctrl* parent, cudaStream_t st, int* launches) {
+    launch_pdl(tile_grid_kernel, dim3(1), dim3(GRID_THREADS), st, f, p, out_tile_counts, parent);
     (*launches)++;
 }
 
-void launch_scan_offsets(const Frame& f, const Pointers& p, int n_sm, cudaStream_t st, int* launches) {
+void launch_scan_offsets(const Frame& f, const Pointers& p, int cshift, int n_sm, cudaStream_t st, int* launches) {
     const long long cap_blocks = ((long long)f.P + SCAN_WARP_TILE * (SCAN_THREADS / 32) - 1) / (SCAN_WARP_TILE * (SCAN_THREADS / 32));
     const int grid = imin(cap_blocks > 0 ? cap_blocks : 1, (long long)n_sm * 8);
-    launch_pdl(scan_offsets_kernel, dim3(grid), dim3(SCAN_THREADS), st, p);
+    launch_pdl(scan_offsets_kernel, dim3(grid), dim3(SCAN_THREADS), st, p, cshift);
     (*launches)++;
 }
 
@@ -717,6 +726,74 @@ void launch_duplicate_and_tile_sort(const Frame& f, const Pointers& p, int n_sm,
                            status, &p.ctrl->tile_counter[TC_TILE0 + pass], st);
         (*launches)++;
     }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Expansion of the super-tile lists into the tile lists (second level of the binning).
+// cids holds, for every super-tile (SUPER x SUPER tiles), the ids of the Gaussians whose tile rect reaches it, in
+// (depth bits, id) order.  A tile's list is the sub-sequence of its super-tile's list whose rects contain the tile,
+// and it starts at ranges[tile] (known from the coverage grid) -- so it can be WRITTEN IN PLACE, in order, with no
+// sort: one block per (super-tile, tile row), one warp per tile of that row.  The block stages 256 list entries at a
+// time (id + the 8-bit mask of the row's columns its rect covers); every warp ballots its column bit over the staged
+// entries, 32 at a time, and appends the covered ids at its running offset.  Per entry of the final lists the HBM
+// traffic is the 4-byte id, written once; the (tile << 32 | id) entries of a one-level sort are never formed.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int EXP_THREADS = 32 * SUPER;
+__global__ void __launch_bounds__(EXP_THREADS)
+expand_kernel(const Frame f, const Pointers p) {
+    __shared__ uint32_t s_id[2][EXP_THREADS];
+    __shared__ uint32_t s_m[2][EXP_THREADS];
+    griddep_sync();
+    if (p.ctrl->overflow != 0ull) return;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int s = blockIdx.x >> SUPER_SHIFT, row = blockIdx.x & (SUPER - 1);
+    const int sy = s / f.cgx, sx = s - sy * f.cgx;
+    const uint32_t ty = (uint32_t)(sy * SUPER + row);
+    if (ty >= (uint32_t)f.gy) return;                       // the whole block: no barrier has been reached yet
+    const uint32_t X0 = (uint32_t)(sx * SUPER), tx = X0 + w;
+    const bool live = tx < (uint32_t)f.gx;
+    uint32_t o = live ? p.ranges[ty * f.gx + tx] : 0u;      // running end of this warp's tile list
+    const uint32_t c0 = p.cranges[s], c1 = p.cranges[s + 1];
+    const unsigned lt = (1u << lane) - 1u;
+    // software pipeline: rects of chunk k+1 and ids of chunk k+2 are in flight while chunk k is expanded
+    uint32_t id_c = 0, id_n = 0;
+    uint2 rc = make_uint2(0u, 0u);
+    if (c0 + tid < c1) {
+        id_c = p.cids[c0 + tid];
+        rc = __ldg(reinterpret_cast<const uint2*>(p.per_g + id_c));
+    }
+    if (c0 + EXP_THREADS + tid < c1) id_n = p.cids[c0 + EXP_THREADS + tid];
+    int buf = 0;
+    for (uint32_t base = c0; base < c1; base += EXP_THREADS, buf ^= 1) {
+        uint32_t m = 0;
+        if (base + tid < c1) {
+            const uint32_t x0 = rc.x & 0xffffu, y0 = rc.x >> 16, x1 = rc.y & 0xffffu, y1 = rc.y >> 16;
+            if (ty >= y0 && ty < y1) {
+                const uint32_t a = max(x0, X0) - X0, b = min(x1, X0 + SUPER) - X0;   // columns [a, b) of this row
+                if (b > a) m = ((1u << (b - a)) - 1u) << a;
+            }
+        }
+        s_id[buf][tid] = id_c;
+        s_m[buf][tid] = m;
+        id_c = id_n;
+        if (base + EXP_THREADS + tid < c1) rc = __ldg(reinterpret_cast<const uint2*>(p.per_g + id_c));
+        if (base + 2 * EXP_THREADS + tid < c1) id_n = p.cids[base + 2 * EXP_THREADS + tid];
+        __syncthreads();   // one barrier per chunk: the buffer written next was last read before the previous barrier
+        if (live) {
+#pragma unroll
+            for (int k = 0; k < EXP_THREADS / 32; k++) {
+                const bool cov = (s_m[buf][32 * k + lane] >> w) & 1u;
+                const unsigned b = __ballot_sync(0xffffffffu, cov);
+                if (cov) p.ids[o + __popc(b & lt)] = s_id[buf][32 * k + lane];
+                o += __popc(b);
+            }
+        }
+    }
+}
+
+void launch_expand(const Frame& f, const Pointers& p, cudaStream_t st, int* launches) {
+    launch_pdl(expand_kernel, dim3(f.n_ctiles * SUPER), dim3(EXP_THREADS), st, f, p);
+    (*launches)++;
 }
 
 // ------------------------------------------------------------------------------------------------------------

@@ -7,6 +7,9 @@
 namespace gs {
 
 constexpr int TILE = 16;
+constexpr int SUPER_SHIFT = 3;             // two-level binning: a super-tile is 8 x 8 tiles
+constexpr int SUPER = 1 << SUPER_SHIFT;
+constexpr int CDIFF_SMEM = 2304;           // coarse difference grids up to this many cells are accumulated in shared memory
 constexpr int MAX_SORT_PASSES_DEPTH = 4;   // 32 depth bits, 8-bit digits
 constexpr int MAX_SORT_PASSES_TILE = 3;    // up to 24 tile-id bits
 constexpr int SORT_THREADS = 256;
@@ -35,6 +38,9 @@ struct Ctrl {
     uint32_t tile_hist[MAX_SORT_PASSES_TILE][256];    // global digit histograms of the tile ids (from tile counts)
     unsigned long long stats[4];        // render statistics (gs_set_stats): warp slots walked, pairs blended, entries staged
 };
+// The workspace holds TWO control blocks: `ctrl` (frame-level counters + the FINE tile grid: n_dup, overflow) and
+// `cctrl` (the same fields for the SUPER-TILE grid that duplication and sort run on: n_vis is copied there,
+// n_dup / tile_hist / tile_counter are the coarse ones).
 enum { TC_PRE = 0, TC_DEPTH0 = 1, TC_SCAN = 5, TC_TILE0 = 6 };
 
 // Look-back status word: [63:62] flag, [61:0] value.
@@ -45,7 +51,8 @@ constexpr unsigned long long ST_MASK = (1ull << 62) - 1;
 
 struct Frame {              // per-frame constants, passed by value to the kernels
     int P, W, H, gx, gy, n_tiles, deg, K;
-    int tile_bits, n_tile_passes;
+    int cgx, cgy, n_ctiles, cdiff_cells;   // super-tile grid (SUPER x SUPER tiles each) and its difference grid
+    int tile_bits, n_tile_passes;         // of the grid the duplication + sort runs on (the super-tile grid)
     int compact;                // 1: preprocess compacts the visible Gaussians (P >= COMPACT_MIN_P)
     int diff_copies, diff_cells; // replicas of the coverage difference grid (power of two) and cells per replica
     float V[16], PM[16];
@@ -57,6 +64,11 @@ struct Frame {              // per-frame constants, passed by value to the kerne
 
 struct Pointers {           // device pointers carved from the workspace
     Ctrl* ctrl;
+    Ctrl* cctrl;                            // control block of the super-tile level
+    int* cdiff;                             // [(cgy+1)*(cgx+1)] difference grid of super-tile coverage
+    uint32_t* cranges;                      // [n_ctiles + 1] ranges of the super-tile lists in cids
+    uint32_t* ccounts;                      // [n_ctiles]
+    uint32_t* cids;                         // [max_dup] Gaussian ids sorted by (super-tile, depth bits, id)
     int* diff;                              // [diff_copies][(gy+1)*(gx+1)] 2-D difference grid of tile coverage
     unsigned long long* st_pre;             // [pre tiles]    look-back status: compaction of visible Gaussians
     unsigned long long* st_scan;            // [scan tiles]   look-back status: duplicate offsets

@@ -195,9 +195,15 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
                   const float* __restrict__ rots, const float* __restrict__ opac, const float* __restrict__ sh) {
     __shared__ uint32_t s_hist[MAX_SORT_PASSES_DEPTH][256];
     __shared__ uint32_t s_nvis;
+    __shared__ int s_cdiff[CDIFF_SMEM];   // super-tile coverage (difference grid) of this block's Gaussians
     griddep_sync();
     const int tid = threadIdx.x, lane = tid & 31;
     for (int k = tid; k < MAX_SORT_PASSES_DEPTH * 256; k += PRE_THREADS) (&s_hist[0][0])[k] = 0;
+    const bool cdiff_shared = f.cdiff_cells <= CDIFF_SMEM;
+    if (cdiff_shared)
+        for (int k = tid; k < f.cdiff_cells; k += PRE_THREADS) s_cdiff[k] = 0;
+    int* const cdiff = cdiff_shared ? s_cdiff : p.cdiff;
+    const int cgw = f.cgx + 1;
     if (tid == 0) s_nvis = 0;
     __syncthreads();
     const int n_tiles = (f.P + 31) / 32;
@@ -256,6 +262,14 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             atomicAdd(diff + s.ymin * gw + s.xmax, -1);
             atomicAdd(diff + s.ymax * gw + s.xmin, -1);
             atomicAdd(diff + s.ymax * gw + s.xmax, 1);
+            if (f.n_ctiles) {   // the same rect on the super-tile grid (two-level binning: the grid duplication + sort run on)
+                const int cx0 = s.xmin >> SUPER_SHIFT, cy0 = s.ymin >> SUPER_SHIFT;
+                const int cx1 = (s.xmax + SUPER - 1) >> SUPER_SHIFT, cy1 = (s.ymax + SUPER - 1) >> SUPER_SHIFT;
+                atomicAdd(cdiff + cy0 * cgw + cx0, 1);
+                atomicAdd(cdiff + cy0 * cgw + cx1, -1);
+                atomicAdd(cdiff + cy1 * cgw + cx0, -1);
+                atomicAdd(cdiff + cy1 * cgw + cx1, 1);
+            }
             if (COMPACT) {
                 const uint32_t db = __float_as_uint(s.depth);
                 atomicAdd(&s_hist[0][db & 255u], 1u);
@@ -295,6 +309,11 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
         const uint32_t c = (&s_hist[0][0])[k];
         if (c) atomicAdd(&p.ctrl->depth_hist[0][0] + k, c);
     }
+    if (cdiff_shared)
+        for (int k = tid; k < f.cdiff_cells; k += PRE_THREADS) {
+            const int c = s_cdiff[k];
+            if (c) atomicAdd(p.cdiff + k, c);
+        }
     if (!COMPACT && tid == 0) {
         if (s_nvis) atomicAdd(&p.ctrl->n_vis, (unsigned long long)s_nvis);
         if (blockIdx.x == 0) p.ctrl->n_sort = (unsigned long long)f.P;

@@ -33,7 +33,8 @@ def test_workspace_bytes_and_error_strings_host_only():
     c = binding.gs_workspace_bytes(2000, 128, 128, 10_000)
     assert 0 < a < b and a < c and a % 256 == 0
     # small frames fuse the duplication into the first tile pass: 8 (entries) + 4 (ids) bytes per duplicate;
-    # large frames keep a second 8-byte entry buffer for the stand-alone duplication
+    # large frames keep a second 8-byte entry buffer for the stand-alone duplication (the sorted super-tile ids of the
+    # two-level binning share the first one)
     small = binding.gs_workspace_bytes(0, 800, 800, 1 << 20) - binding.gs_workspace_bytes(0, 800, 800, 0)
     large = binding.gs_workspace_bytes(0, 800, 800, 8 << 20) - binding.gs_workspace_bytes(0, 800, 800, 0)
     assert (1 << 20) * 12 <= small < (1 << 20) * 16

@@ -169,21 +169,26 @@ def _config_dict(config, cfg, sc, extra=None):
 # ----------------------------------------------------------------------------------------------------------------
 # our arm: the CUDA path through the C ABI
 # ----------------------------------------------------------------------------------------------------------------
-def _stage_bytes(P, K_sh, n_vis, n_dup, n_tile_passes, max_dup):
-    """Algorithmic HBM bytes per frame of the memory-bound stages."""
+def _stage_bytes(P, K_sh, n_vis, n_dup, n_coarse, n_sort_passes, max_dup):
+    """Algorithmic HBM bytes per frame of the memory-bound stages.  n_coarse > 0:
+    two-level binning -- the entries that are duplicated and sorted are the n_coarse (super-tile, Gaussian) pairs, and
+    the expansion reads every sorted id (4) + its rect (8) and writes the n_dup ids of the tile lists once."""
     compact = P >= (1 << 20)                  # common.cuh COMPACT_MIN_P: small scenes sort all P keys
     n_sort = n_vis if compact else P
-    fused = max_dup <= (4 << 20)              # common.cuh FUSED_DUP_MAX
-    packed = n_tile_passes == 2 and P <= (1 << 24)
+    fused = max_dup <= (4 << 20)              # common.cuh FUSED_DUP_MAX (= one-level binning)
+    n_ent = n_coarse if n_coarse > 0 else n_dup
+    packed = n_sort_passes == 2 and P <= (1 << 24)
     rank_bytes = n_vis * 20                   # depth-ordered id (8) + offset (4) + rect (8), read by the duplication
-    if n_tile_passes == 1:
+    if n_sort_passes == 1:
         first, rest = (4, 0) if fused else (8 + 8 + 4, 0)
     elif packed:
         first, rest = (4, 8) if fused else (8 + 8 + 4, 8)      # packed 4-byte entries between the two passes
     else:
-        first, rest = (8, 16 * (n_tile_passes - 2) + 12) if fused else (8 + 16, 16 * (n_tile_passes - 2) + 12)
-    dup_only = rank_bytes + n_dup * (first if fused else 8)
-    sort_rest = n_dup * ((first - 8 if not fused else 0) + rest)
+        first, rest = (8, 16 * (n_sort_passes - 2) + 12) if fused else (8 + 16, 16 * (n_sort_passes - 2) + 12)
+    dup_only = rank_bytes + n_ent * (first if fused else 8)
+    sort_rest = n_ent * ((first - 8 if not fused else 0) + rest)
+    if n_coarse > 0:
+        sort_rest += n_coarse * 12 + n_dup * 4
     return {
         "preprocess": P * 40 + n_vis * (4 + 12 * K_sh) + P * 16 + n_vis * 64 + n_sort * 8,
         "depth_sort": 4 * 16 * n_sort,
@@ -254,7 +259,7 @@ def run_ours(args):
         r.render(cam, count_contrib=True)
         stats.append(binding.gs_get_stats(r.workspace))
         it = r.intermediates(copy=())
-        per_pose.append((it.n_visible, it.n_dup))
+        per_pose.append((it.n_visible, it.n_dup, it.n_coarse))
         max_dup = int(it.max_dup)   # the capacity the library recovered from the workspace size
     binding.gs_set_stats(False)
     launches_per_frame = binding.gs_last_launch_count()
@@ -262,7 +267,7 @@ def run_ours(args):
     pairs_eval = mean([s["pairs_evaluated"] for s in stats])
     pairs_blend = mean([s["pairs_blended"] for s in stats])
     staged = mean([s["entries_staged"] for s in stats])
-    n_vis_m, n_dup_m = mean([p[0] for p in per_pose]), mean([p[1] for p in per_pose])
+    n_vis_m, n_dup_m, n_coarse_m = mean([p[0] for p in per_pose]), mean([p[1] for p in per_pose]), mean([p[2] for p in per_pose])
 
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
 
@@ -276,7 +281,7 @@ def run_ours(args):
 
     # A step = every pose of the configuration once, through the public batch call: `lanes` frames in flight on their own
     # streams and workspaces (Renderer.render_batch).  The L2 is flushed before every step, outside the event pair.
-    lanes = args.lanes if args.lanes > 0 else (1 if r.workspace.numel() < (8 << 20) else (3 if r.workspace.numel() < (4 << 30) else 2))
+    lanes = args.lanes if args.lanes > 0 else 1     # 0: chosen below, by timing warm-up steps
 
     def step(e0=None, e1=None):
         flush.zero_()
@@ -286,11 +291,27 @@ def run_ours(args):
         if e1 is not None:
             e1.record()
 
-    # ---- pre-warm (clock ramp) + W warm-up steps -------------------------------------------------------------------------
+    # ---- pre-warm (clock ramp), choice of the frames in flight, W warm-up steps -----------------------------------------
     t0 = time.perf_counter()
     while time.perf_counter() - t0 < 0.5:
         step()
         torch.cuda.synchronize()
+    if args.lanes <= 0:   # untimed tuning: the fastest of 1, 2, 3, 4 frames in flight over a few warm-up steps (rank 0 decides)
+        cands = [1, 2, 3, 4] if r.workspace.numel() < (8 << 30) else [1, 2]
+        best = (None, 1)
+        for cand in cands:
+            lanes = cand
+            step(); step()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            tt = 0.0
+            for _ in range(3):
+                step(e0, e1)
+                torch.cuda.synchronize()
+                tt += e0.elapsed_time(e1)
+            if best[0] is None or tt < best[0]:
+                best = (tt, cand)
+        lanes = int(rank_max(best[1])) if ws > 1 else best[1]
     for _ in range(args.warmup):
         step()
     # ---- timed region: exactly K steps ---------------------------------------------------------------------------------------
@@ -373,8 +394,10 @@ def run_ours(args):
                 "units_per_launch": {"pairs_evaluated": pairs_eval, "instr_per_pair": INSTR_PER_PAIR,
                                      "pairs_blended": pairs_blend, "entries_staged": staged},
                 "ms_per_launch": stage_ms["render"]}
-    n_tile_passes = (max(1, (((W + 15) // 16) * ((H + 15) // 16) - 1).bit_length()) + 7) // 8
-    sb = _stage_bytes(sc.P, (sc.sh_degree + 1) ** 2, n_vis_m, n_dup_m, n_tile_passes, max_dup)
+    gx, gy = (W + 15) // 16, (H + 15) // 16
+    n_sorted_cells = ((gx + 7) // 8) * ((gy + 7) // 8) if n_coarse_m > 0 else gx * gy   # super-tiles or tiles
+    n_sort_passes = (max(1, (n_sorted_cells - 1).bit_length()) + 7) // 8
+    sb = _stage_bytes(sc.P, (sc.sh_degree + 1) ** 2, n_vis_m, n_dup_m, n_coarse_m, n_sort_passes, max_dup)
     kernels = []
     for n in ("preprocess", "depth_sort", "tile_grid", "offset_scan", "duplicate", "tile_sort", "render"):
         k = {"stage": n, "ms": stage_ms[n], "share": stage_ms[n] / max(stage_ms["frame"], 1e-9)}
@@ -407,7 +430,8 @@ def run_ours(args):
                 "config": _config_dict(args.config, cfg, sc, extra={
                     "frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every step", "frames_in_flight": lanes,
                     "parallelism": "replicas x%d" % ws,
-                    "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "render_variant": binding.gs_get_render_variant()}),
+                    "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "n_coarse_mean": n_coarse_m,
+                    "binning": "two-level (8x8-tile super-tiles)" if n_coarse_m > 0 else "one-level", "render_variant": binding.gs_get_render_variant()}),
                 "ms_per_frame": ms_per_step / n_pose, "wall_ms_per_step_incl_flush": 1e3 * wall / K,
                 "latency": {"ms_per_frame": serial_ms_per_frame, "frames_per_s": ws * 1e3 / serial_ms_per_frame,
                             "how": "one frame in flight, one stream, L2 flushed before every frame"},
@@ -430,7 +454,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=(1, 2, 3, 4, 5))
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = chosen from the workspace size)")
+    ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = the fastest of 1-4 over a few warm-up steps)")
     ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

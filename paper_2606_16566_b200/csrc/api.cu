@@ -36,7 +36,7 @@ struct Layout {
     size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, desc, cranges, ccounts, entA, entB, cids, ids, total;
     size_t n_depth_tiles, n_tile_tiles;
     int gx, gy, n_tiles, tile_bits, n_tile_passes, diff_copies, diff_cells;
-    int cgx, cgy, n_ctiles, cdiff_cells;
+    int cshift, cgx, cgy, n_ctiles, cdiff_cells;
     bool two_level;
 };
 
@@ -50,6 +50,8 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     // Large frames (capacity > FUSED_DUP_MAX) bin in TWO LEVELS: duplication + sort run on the super-tile grid, whose id
     // width then sets the number of radix passes, and expand_kernel writes the tile lists.  Small frames sort tile ids.
     L.two_level = max_dup > FUSED_DUP_MAX;
+    L.cshift = L.two_level ? SUPER_SHIFT : 0;
+    const int SUPER = 1 << L.cshift;
     L.cgx = L.two_level ? (L.gx + SUPER - 1) / SUPER : 0;
     L.cgy = L.two_level ? (L.gy + SUPER - 1) / SUPER : 0;
     L.n_ctiles = L.cgx * L.cgy;
@@ -156,11 +158,13 @@ Pointers carve(void* ws, const Layout& L) {
 bool fit_max_dup(int P, int W, int H, size_t bytes, unsigned long long& max_dup) {
     Layout L;
     if (!make_layout(P, W, H, 0, L) || L.total > bytes) return false;
-    // regime edges: sort_items_for (256 K: small radix tiles) and FUSED_DUP_MAX (two-level binning, second entry buffer)
-    const unsigned long long e1 = 256ull << 10, e2 = FUSED_DUP_MAX;
-    const unsigned long long lo_of[3] = {e2 + 1, e1 + 1, 0}, hi_of[3] = {(1ull << 32) - 1, e2, e1};
-    for (int r = 0; r < 3; r++) {
-        unsigned long long lo = lo_of[r], hi = hi_of[r];
+    // regime starts: sort_items_for (256 K: small radix tiles) and FUSED_DUP_MAX (two-level binning, second entry buffer)
+    const unsigned long long starts[3] = {0ull, (256ull << 10) + 1, FUSED_DUP_MAX + 1};
+    const unsigned long long top = (1ull << 32) - 1;
+    for (int r = 2; r >= 0; r--) {
+        unsigned long long lo = starts[r], hi = (r == 2 ? top : starts[r + 1] - 1);
+        if (lo > top || hi < lo) continue;
+        if (hi > top) hi = top;
         make_layout(P, W, H, lo, L);
         if (L.total > bytes) continue;
         while (lo < hi) {
@@ -212,7 +216,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     f.tile_bits = L.tile_bits; f.n_tile_passes = L.n_tile_passes;
     f.compact = P >= COMPACT_MIN_P ? 1 : 0;
     f.diff_copies = L.diff_copies; f.diff_cells = L.diff_cells;
-    f.cgx = L.cgx; f.cgy = L.cgy; f.n_ctiles = L.n_ctiles; f.cdiff_cells = L.cdiff_cells;
+    f.cshift = L.cshift; f.cgx = L.cgx; f.cgy = L.cgy; f.n_ctiles = L.n_ctiles; f.cdiff_cells = L.cdiff_cells;
     for (int k = 0; k < 16; k++) { f.V[k] = viewmatrix[k]; f.PM[k] = projmatrix[k]; }
     f.fx = fx; f.fy = fy;
     // camera centre of the rigid view matrix: campos = -Wv^T t (the north_star signature carries no campos)
@@ -293,7 +297,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     }
     mark(3);
     if (two_level) {
-        launch_scan_offsets(fc, pc, SUPER_SHIFT, g_n_sm, st, &launches);   // (2) prefix-sum offsets of the super-tile duplicates
+        launch_scan_offsets(fc, pc, f.cshift, g_n_sm, st, &launches);   // (2) prefix-sum offsets of the super-tile duplicates
         mark(4);
         launch_duplicate_and_tile_sort(fc, pc, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b) on super-tiles
         launch_expand(f, p, st, &launches);                  // (3c) super-tile lists -> tile lists, written in place

@@ -730,19 +730,22 @@ void launch_duplicate_and_tile_sort(const Frame& f, const Pointers& p, int n_sm,
 
 // ------------------------------------------------------------------------------------------------------------
 // Expansion of the super-tile lists into the tile lists (second level of the binning).
-// cids holds, for every super-tile (SUPER x SUPER tiles), the ids of the Gaussians whose tile rect reaches it, in
+// cids holds, for every super-tile (S x S tiles, S = 2^SH = 8), the ids of the Gaussians whose tile rect reaches it, in
 // (depth bits, id) order.  A tile's list is the sub-sequence of its super-tile's list whose rects contain the tile,
 // and it starts at ranges[tile] (known from the coverage grid) -- so it can be WRITTEN IN PLACE, in order, with no
-// sort: one block per (super-tile, tile row), one warp per tile of that row.  The block stages 256 list entries at a
-// time (id + the 8-bit mask of the row's columns its rect covers); every warp ballots its column bit over the staged
+// sort: one block per (super-tile, tile row), one warp per tile of that row.  The block stages 32 S list entries at a
+// time (id + the S-bit mask of the row's columns its rect covers); every warp ballots its column bit over the staged
 // entries, 32 at a time, and appends the covered ids at its running offset.  Per entry of the final lists the HBM
 // traffic is the 4-byte id, written once; the (tile << 32 | id) entries of a one-level sort are never formed.
 // ------------------------------------------------------------------------------------------------------------
-constexpr int EXP_THREADS = 32 * SUPER;
-__global__ void __launch_bounds__(EXP_THREADS)
+template <int SH>
+__global__ void __launch_bounds__(32 << SH)
 expand_kernel(const Frame f, const Pointers p) {
+    constexpr int SUPER = 1 << SH, SUPER_SHIFT = SH, EXP_THREADS = 32 * SUPER;
+    // staged chunk: the ids, and for every tile column c the ballot over each 32-entry group k of "entry covers (row, c)"
+    // -- taken once by the staging warp, so the expanding warps only read their column's eight words (broadcast loads)
     __shared__ uint32_t s_id[2][EXP_THREADS];
-    __shared__ uint32_t s_m[2][EXP_THREADS];
+    __shared__ __align__(16) uint32_t s_b[2][SUPER][EXP_THREADS / 32];   // [buffer][column][group]
     griddep_sync();
     if (p.ctrl->overflow != 0ull) return;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -752,7 +755,7 @@ expand_kernel(const Frame f, const Pointers p) {
     if (ty >= (uint32_t)f.gy) return;                       // the whole block: no barrier has been reached yet
     const uint32_t X0 = (uint32_t)(sx * SUPER), tx = X0 + w;
     const bool live = tx < (uint32_t)f.gx;
-    uint32_t o = live ? p.ranges[ty * f.gx + tx] : 0u;      // running end of this warp's tile list
+    uint32_t* __restrict__ out = p.ids + (live ? p.ranges[ty * f.gx + tx] : 0u);   // running end of this warp's tile list
     const uint32_t c0 = p.cranges[s], c1 = p.cranges[s + 1];
     const unsigned lt = (1u << lane) - 1u;
     // software pipeline: rects of chunk k+1 and ids of chunk k+2 are in flight while chunk k is expanded
@@ -774,25 +777,38 @@ expand_kernel(const Frame f, const Pointers p) {
             }
         }
         s_id[buf][tid] = id_c;
-        s_m[buf][tid] = m;
+        {   // lane c < 8 keeps the ballot of column c (every lane sees all eight ballot words)
+            uint32_t mine = 0;
+#pragma unroll
+            for (int c = 0; c < SUPER; c++) {
+                const unsigned b = __ballot_sync(0xffffffffu, (m >> c) & 1u);
+                if (lane == c) mine = b;
+            }
+            if (lane < SUPER) s_b[buf][lane][w] = mine;
+        }
         id_c = id_n;
         if (base + EXP_THREADS + tid < c1) rc = __ldg(reinterpret_cast<const uint2*>(p.per_g + id_c));
         if (base + 2 * EXP_THREADS + tid < c1) id_n = p.cids[base + 2 * EXP_THREADS + tid];
         __syncthreads();   // one barrier per chunk: the buffer written next was last read before the previous barrier
         if (live) {
+            uint32_t b8[SUPER];
 #pragma unroll
-            for (int k = 0; k < EXP_THREADS / 32; k++) {
-                const bool cov = (s_m[buf][32 * k + lane] >> w) & 1u;
-                const unsigned b = __ballot_sync(0xffffffffu, cov);
-                if (cov) p.ids[o + __popc(b & lt)] = s_id[buf][32 * k + lane];
-                o += __popc(b);
+            for (int k = 0; k < SUPER; k += 4) {
+                const uint4 v = *reinterpret_cast<const uint4*>(&s_b[buf][w][k]);
+                b8[k] = v.x; b8[k + 1] = v.y; b8[k + 2] = v.z; b8[k + 3] = v.w;
+            }
+#pragma unroll
+            for (int k = 0; k < SUPER; k++) {
+                const unsigned b = b8[k];
+                if ((b >> lane) & 1u) out[__popc(b & lt)] = s_id[buf][32 * k + lane];
+                out += __popc(b);
             }
         }
     }
 }
 
 void launch_expand(const Frame& f, const Pointers& p, cudaStream_t st, int* launches) {
-    launch_pdl(expand_kernel, dim3(f.n_ctiles * SUPER), dim3(EXP_THREADS), st, f, p);
+    launch_pdl(expand_kernel<SUPER_SHIFT>, dim3(f.n_ctiles << SUPER_SHIFT), dim3(32 << SUPER_SHIFT), st, f, p);
     (*launches)++;
 }
 

@@ -26,6 +26,7 @@ __device__ __forceinline__ float dot3(float a0, float a1, float a2, float b0, fl
     return add(add(mul(a0, b0), mul(a1, b1)), mul(a2, b2));
 }
 
+struct float5 { float a, b, c, d, e; };
 struct Splat {
     float mux, muy, ca, cb, cc, depth;
     int radius, xmin, ymin, xmax, ymax;
@@ -179,17 +180,12 @@ __device__ __forceinline__ float3 sh_colour_direct(const Frame& f, const float* 
     return make_float3(fmaxf(r, 0.0f), fmaxf(g, 0.0f), fmaxf(b, 0.0f));
 }
 
-// One WARP processes one 32-Gaussian sub-tile at a time; there is no block barrier inside the loop.
-//
-// COMPACT = true (large scenes): order-preserving compaction of the visible Gaussians.  The warp takes a sub-tile per
-//   atomic ticket, publishes the sub-tile's count of visible Gaussians at once, does all the heavy work (SH colour,
-//   records, coverage grid, histograms), and only then looks back for its exclusive prefix -- by which time the
-//   predecessors have long published.
-// COMPACT = false (small scenes, one wave of warps): a single wave gives the look-back nothing to overlap with -- the
-//   inclusive prefixes advance 32 sub-tiles per L2 round trip, ~25 us for 100 000 Gaussians -- so nothing is
-//   compacted: every Gaussian writes a key, culled ones the all-ones key that sorts behind every depth, and the depth
-//   sort runs over all P keys.  Sub-tiles are assigned statically; there is no inter-warp dependency at all.
-template <int DEG, bool COMPACT>
+// Small scenes (P < COMPACT_MIN_P, one wave of warps): one WARP processes one 32-Gaussian sub-tile at a time, sub-tiles
+// assigned statically, no inter-warp dependency and no block barrier inside the loop.  Nothing is compacted: a single
+// wave gives a chained scan nothing to overlap with (its inclusive prefixes advance 32 sub-tiles per L2 round trip,
+// ~25 us for 100 000 Gaussians), so every Gaussian writes a key -- culled ones the all-ones key that sorts behind every
+// depth -- and the depth sort runs over all P keys.
+template <int DEG>
 __global__ void __launch_bounds__(PRE_THREADS)
 preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ means, const float* __restrict__ scales,
                   const float* __restrict__ rots, const float* __restrict__ opac, const float* __restrict__ sh) {
@@ -208,18 +204,11 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
     __syncthreads();
     const int n_tiles = (f.P + 31) / 32;
     const int gw = f.gx + 1;
-    const unsigned lt = (1u << lane) - 1u;
     const int gwarp = blockIdx.x * (PRE_THREADS / 32) + (tid >> 5), n_warps = gridDim.x * (PRE_THREADS / 32);
     // coverage grid copy of this warp: the corner counters of a small grid are hot (hundreds of atomics per address,
     // serialised in L2), so they are spread over diff_copies replicas that tile_grid_kernel adds up
     int* diff = p.diff + (size_t)(gwarp & (f.diff_copies - 1)) * f.diff_cells;
-    int tile = gwarp;
-    while (true) {
-        if (COMPACT) {
-            if (lane == 0) tile = (int)atomicAdd(&p.ctrl->tile_counter[TC_PRE], 1u);
-            tile = __shfl_sync(0xffffffffu, tile, 0);
-        }
-        if (tile >= n_tiles) break;
+    for (int tile = gwarp; tile < n_tiles; tile += n_warps) {
         const int i = tile * 32 + lane;
         Splat s = {};
         bool vis = false;
@@ -231,14 +220,8 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             const float4 q = __ldcs(reinterpret_cast<const float4*>(rots) + i);
             vis = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, s);
         }
-        const unsigned vb = __ballot_sync(0xffffffffu, vis);
-        const uint32_t cnt = __popc(vb);
-        if (COMPACT) {
-            if (lane == 0) st_status(p.st_pre + tile, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)cnt);
-        } else if (lane == 0 && cnt) {
-            atomicAdd(&s_nvis, cnt);
-        }
-        // ---- everything that does not need the compact index --------------------------------------------------
+        const uint32_t cnt = __popc(__ballot_sync(0xffffffffu, vis));
+        if (lane == 0 && cnt) atomicAdd(&s_nvis, cnt);
         if (i < f.P) {
             uint4 pg = make_uint4(0u, 0u, 0u, 0u);
             if (vis) {
@@ -248,14 +231,13 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
                 pg.w = (uint32_t)s.radius;
             }
             p.per_g[i] = pg;
-            if (!COMPACT) {  // a culled Gaussian sorts behind every depth: digit 255 in all four passes
-                const uint32_t db = vis ? __float_as_uint(s.depth) : 0xffffffffu;
-                atomicAdd(&s_hist[0][db & 255u], 1u);
-                atomicAdd(&s_hist[1][(db >> 8) & 255u], 1u);
-                atomicAdd(&s_hist[2][(db >> 16) & 255u], 1u);
-                atomicAdd(&s_hist[3][db >> 24], 1u);
-                p.gkeyA[i] = vis ? (((unsigned long long)db << 32) | (unsigned)i) : ~0ull;
-            }
+            // a culled Gaussian sorts behind every depth: digit 255 in all four passes
+            const uint32_t db = vis ? __float_as_uint(s.depth) : 0xffffffffu;
+            atomicAdd(&s_hist[0][db & 255u], 1u);
+            atomicAdd(&s_hist[1][(db >> 8) & 255u], 1u);
+            atomicAdd(&s_hist[2][(db >> 16) & 255u], 1u);
+            atomicAdd(&s_hist[3][db >> 24], 1u);
+            p.gkeyA[i] = vis ? (((unsigned long long)db << 32) | (unsigned)i) : ~0ull;
         }
         if (vis) {
             atomicAdd(diff + s.ymin * gw + s.xmin, 1);
@@ -263,19 +245,13 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             atomicAdd(diff + s.ymax * gw + s.xmin, -1);
             atomicAdd(diff + s.ymax * gw + s.xmax, 1);
             if (f.n_ctiles) {   // the same rect on the super-tile grid (two-level binning: the grid duplication + sort run on)
-                const int cx0 = s.xmin >> SUPER_SHIFT, cy0 = s.ymin >> SUPER_SHIFT;
-                const int cx1 = (s.xmax + SUPER - 1) >> SUPER_SHIFT, cy1 = (s.ymax + SUPER - 1) >> SUPER_SHIFT;
+                const int cs = f.cshift, cr = (1 << cs) - 1;
+                const int cx0 = s.xmin >> cs, cy0 = s.ymin >> cs;
+                const int cx1 = (s.xmax + cr) >> cs, cy1 = (s.ymax + cr) >> cs;
                 atomicAdd(cdiff + cy0 * cgw + cx0, 1);
                 atomicAdd(cdiff + cy0 * cgw + cx1, -1);
                 atomicAdd(cdiff + cy1 * cgw + cx0, -1);
                 atomicAdd(cdiff + cy1 * cgw + cx1, 1);
-            }
-            if (COMPACT) {
-                const uint32_t db = __float_as_uint(s.depth);
-                atomicAdd(&s_hist[0][db & 255u], 1u);
-                atomicAdd(&s_hist[1][(db >> 8) & 255u], 1u);
-                atomicAdd(&s_hist[2][(db >> 16) & 255u], 1u);
-                atomicAdd(&s_hist[3][db >> 24], 1u);
             }
             const float o = __ldcs(opac + i);
             const float3 col = sh_colour_direct<DEG>(f, sh, i, px, py, pz);
@@ -291,17 +267,174 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             rec[2] = make_float4(col.x, col.y, col.z, tb.xstar);
             rec[3] = make_float4(tb.ic, tb.ct, 0.0f, 0.0f);
         }
-        if (COMPACT) {
-            // ---- exclusive prefix by decoupled look-back ("parallel prefix scan") ------------------
-            const unsigned long long excl = tile > 0 ? lookback_warp(p.st_pre, tile) : 0ull;
-            const unsigned long long run = excl + cnt;
-            if (lane == 0) {
-                st_status(p.st_pre + tile, ST_INC | run);
-                if (tile == n_tiles - 1) { p.ctrl->n_vis = run; p.ctrl->n_sort = run; }
+    }
+    __syncthreads();
+    for (int k = tid; k < MAX_SORT_PASSES_DEPTH * 256; k += PRE_THREADS) {
+        const uint32_t c = (&s_hist[0][0])[k];
+        if (c) atomicAdd(&p.ctrl->depth_hist[0][0] + k, c);
+    }
+    if (cdiff_shared)
+        for (int k = tid; k < f.cdiff_cells; k += PRE_THREADS) {
+            const int c = s_cdiff[k];
+            if (c) atomicAdd(p.cdiff + k, c);
+        }
+    if (tid == 0) {
+        if (s_nvis) atomicAdd(&p.ctrl->n_vis, (unsigned long long)s_nvis);
+        if (blockIdx.x == 0) p.ctrl->n_sort = (unsigned long long)f.P;
+    }
+}
+
+// Large scenes (P >= COMPACT_MIN_P): TWO-PHASE preprocess with order-preserving compaction of the visible Gaussians.
+// A warp takes 96 consecutive Gaussians per atomic ticket.
+//   Phase A (all 96, three rounds): the mean only -- view-space depth against the near plane (C-P0, the exact test
+//     project() starts with).  In the camera-inside scenes about half of the Gaussians end here, having cost ~30
+//     instructions instead of ~1 000; the survivors' indices are queued, in index order, in shared memory.
+//   Phase B (survivors, DENSE lanes: two rounds when <= 64 survived): C-P0..C-P8, then -- visible ones only -- SH
+//     colour, render record, coverage grids, depth histograms.
+// The tile's count of visible Gaussians is published before the heavy part of phase B and the exclusive prefix is
+// looked back for after it ("parallel prefix scan"; decoupled look-back), by which time the predecessors
+// have long published.  Index order is kept throughout (queue in index order, rounds in order), which the stable
+// depth sort needs for the tie-break of reading S10.
+constexpr int PRE2_TILE = 96;
+template <int DEG>
+__global__ void __launch_bounds__(PRE_THREADS, 4)
+preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ means, const float* __restrict__ scales,
+                   const float* __restrict__ rots, const float* __restrict__ opac, const float* __restrict__ sh) {
+    __shared__ uint32_t s_hist[MAX_SORT_PASSES_DEPTH][256];
+    __shared__ int s_cdiff[CDIFF_SMEM];
+    __shared__ uint32_t s_q[PRE_THREADS / 32][PRE2_TILE];
+    griddep_sync();
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    for (int k = tid; k < MAX_SORT_PASSES_DEPTH * 256; k += PRE_THREADS) (&s_hist[0][0])[k] = 0;
+    const bool cdiff_shared = f.cdiff_cells <= CDIFF_SMEM;
+    if (cdiff_shared)
+        for (int k = tid; k < f.cdiff_cells; k += PRE_THREADS) s_cdiff[k] = 0;
+    int* const cdiff = cdiff_shared ? s_cdiff : p.cdiff;
+    const int cgw = f.cgx + 1;
+    __syncthreads();
+    const int n_tiles = (f.P + PRE2_TILE - 1) / PRE2_TILE;
+    const int gw = f.gx + 1;
+    const unsigned lt = (1u << lane) - 1u;
+    const int gwarp = blockIdx.x * (PRE_THREADS / 32) + w;
+    int* diff = p.diff + (size_t)(gwarp & (f.diff_copies - 1)) * f.diff_cells;
+    const uint4 zero4 = make_uint4(0u, 0u, 0u, 0u);
+    while (true) {
+        int tile = 0;
+        if (lane == 0) tile = (int)atomicAdd(&p.ctrl->tile_counter[TC_PRE], 1u);
+        tile = __shfl_sync(0xffffffffu, tile, 0);
+        if (tile >= n_tiles) break;
+        const int i0 = tile * PRE2_TILE;
+        // ---- phase A: near-plane test on the mean, survivors queued in index order ---------------------------------
+        uint32_t n_alive = 0;
+#pragma unroll
+        for (int r = 0; r < PRE2_TILE / 32; r++) {
+            const int i = i0 + 32 * r + lane;
+            bool alive = false;
+            if (i < f.P) {
+                const float px = __ldg(means + 3 * (size_t)i), py = __ldg(means + 3 * (size_t)i + 1), pz = __ldg(means + 3 * (size_t)i + 2);
+                alive = affine(f.V + 8, px, py, pz) > 0.2f;     // C-P0 (reading S2), the operation project() repeats
+                if (!alive) p.per_g[i] = zero4;
             }
-            if (vis) p.gkeyA[excl + __popc(vb & lt)] = ((unsigned long long)__float_as_uint(s.depth) << 32) | (unsigned)i;
-        } else {
-            tile += n_warps;
+            const unsigned ba = __ballot_sync(0xffffffffu, alive);
+            if (alive) s_q[w][n_alive + __popc(ba & lt)] = (uint32_t)i;
+            n_alive += __popc(ba);
+        }
+        __syncwarp();
+        // ---- phase B, part 1: projection of the survivors, dense lanes ------------------------------------------------
+        // carried to part 2 per round: index, 2-D mean and conic (rect / depth / radius are re-read from per_g)
+        float5 g[PRE2_TILE / 32];
+        bool vis[PRE2_TILE / 32];
+        int idx[PRE2_TILE / 32];
+        unsigned vb[PRE2_TILE / 32];
+        uint32_t cnt = 0;
+#pragma unroll
+        for (int h = 0; h < PRE2_TILE / 32; h++) {
+            vis[h] = false; idx[h] = 0; vb[h] = 0u; g[h] = float5{};
+            if (32u * h < n_alive) {   // warp-uniform
+                if (32u * h + lane < n_alive) {
+                    const int i = (int)s_q[w][32 * h + lane];
+                    idx[h] = i;
+                    const float px = __ldg(means + 3 * (size_t)i), py = __ldg(means + 3 * (size_t)i + 1), pz = __ldg(means + 3 * (size_t)i + 2);
+                    const float sx = __ldg(scales + 3 * (size_t)i), sy = __ldg(scales + 3 * (size_t)i + 1), sz = __ldg(scales + 3 * (size_t)i + 2);
+                    const float4 q = __ldcs(reinterpret_cast<const float4*>(rots) + i);
+                    Splat t;
+                    vis[h] = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, t);
+                    uint4 pg = zero4;
+                    if (vis[h]) {
+                        pg.x = (uint32_t)t.xmin | ((uint32_t)t.ymin << 16);
+                        pg.y = (uint32_t)t.xmax | ((uint32_t)t.ymax << 16);
+                        pg.z = __float_as_uint(t.depth);
+                        pg.w = (uint32_t)t.radius;
+                        g[h] = float5{t.mux, t.muy, t.ca, t.cb, t.cc};
+                    }
+                    p.per_g[i] = pg;
+                }
+                vb[h] = __ballot_sync(0xffffffffu, vis[h]);
+                cnt += __popc(vb[h]);
+            }
+        }
+        __syncwarp();   // the queue is re-used by the next ticket
+        if (lane == 0) st_status(p.st_pre + tile, (tile == 0 ? ST_INC : ST_AGG) | (unsigned long long)cnt);
+        // ---- phase B, part 2: everything that does not need the compact index --------------------------------------
+        uint32_t depth_bits[PRE2_TILE / 32];
+#pragma unroll
+        for (int h = 0; h < PRE2_TILE / 32; h++) depth_bits[h] = 0u;
+#pragma unroll
+        for (int h = 0; h < PRE2_TILE / 32; h++) {
+            if (vb[h] == 0u) continue;   // warp-uniform
+            if (vis[h]) {
+                const int i = idx[h];
+                const uint4 pg = p.per_g[i];     // this thread's own store of part 1
+                struct { int xmin, ymin, xmax, ymax; float mux, muy, ca, cb, cc; } t = {
+                    (int)(pg.x & 0xffffu), (int)(pg.x >> 16), (int)(pg.y & 0xffffu), (int)(pg.y >> 16),
+                    g[h].a, g[h].b, g[h].c, g[h].d, g[h].e};
+                depth_bits[h] = pg.z;
+                const float px = __ldg(means + 3 * (size_t)i), py = __ldg(means + 3 * (size_t)i + 1), pz = __ldg(means + 3 * (size_t)i + 2);
+                atomicAdd(diff + t.ymin * gw + t.xmin, 1);
+                atomicAdd(diff + t.ymin * gw + t.xmax, -1);
+                atomicAdd(diff + t.ymax * gw + t.xmin, -1);
+                atomicAdd(diff + t.ymax * gw + t.xmax, 1);
+                if (f.n_ctiles) {   // the same rect on the super-tile grid (two-level binning)
+                    const int cs = f.cshift, cr = (1 << cs) - 1;
+                    const int cx0 = t.xmin >> cs, cy0 = t.ymin >> cs;
+                    const int cx1 = (t.xmax + cr) >> cs, cy1 = (t.ymax + cr) >> cs;
+                    atomicAdd(cdiff + cy0 * cgw + cx0, 1);
+                    atomicAdd(cdiff + cy0 * cgw + cx1, -1);
+                    atomicAdd(cdiff + cy1 * cgw + cx0, -1);
+                    atomicAdd(cdiff + cy1 * cgw + cx1, 1);
+                }
+                const uint32_t db = pg.z;
+                atomicAdd(&s_hist[0][db & 255u], 1u);
+                atomicAdd(&s_hist[1][(db >> 8) & 255u], 1u);
+                atomicAdd(&s_hist[2][(db >> 16) & 255u], 1u);
+                atomicAdd(&s_hist[3][db >> 24], 1u);
+                const float o = __ldcs(opac + i);
+                const float3 col = sh_colour_direct<DEG>(f, sh, i, px, py, pz);
+                // det of the STORED conic, exact products in double (24+24 bits): the form is indefinite iff det <= 0,
+                // and the tight box of the render stage needs det without fp32 cancellation (needle-like splats)
+                const double dd = (double)t.ca * (double)t.cc - (double)t.cb * (double)t.cb;
+                const float l2o = log2f(o);
+                const TightBox tb = tight_box_constants(t.ca, t.cb, t.cc, (float)dd, l2o);
+                const uint32_t flags = (!(dd > 0.0) || tb.degenerate) ? 1u : 0u;
+                float4* rec = p.rec + 4 * (size_t)i;  // 64-byte render record (include/gs.h: gs_intermediates.record)
+                rec[0] = make_float4(t.mux, t.muy, t.ca, t.cb);
+                rec[1] = make_float4(t.cc, l2o, (float)dd, __uint_as_float(flags));
+                rec[2] = make_float4(col.x, col.y, col.z, tb.xstar);
+                rec[3] = make_float4(tb.ic, tb.ct, 0.0f, 0.0f);
+            }
+        }
+        // ---- exclusive prefix by decoupled look-back; keys of the visible Gaussians in index order ------------------
+        const unsigned long long excl = tile > 0 ? lookback_warp(p.st_pre, tile) : 0ull;
+        const unsigned long long run = excl + cnt;
+        if (lane == 0) {
+            st_status(p.st_pre + tile, ST_INC | run);
+            if (tile == n_tiles - 1) { p.ctrl->n_vis = run; p.ctrl->n_sort = run; }
+        }
+        uint32_t before = 0;
+#pragma unroll
+        for (int h = 0; h < PRE2_TILE / 32; h++) {
+            if (vis[h]) p.gkeyA[excl + before + __popc(vb[h] & lt)] = ((unsigned long long)depth_bits[h] << 32) | (unsigned)idx[h];
+            before += __popc(vb[h]);
         }
     }
     __syncthreads();
@@ -314,17 +447,13 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             const int c = s_cdiff[k];
             if (c) atomicAdd(p.cdiff + k, c);
         }
-    if (!COMPACT && tid == 0) {
-        if (s_nvis) atomicAdd(&p.ctrl->n_vis, (unsigned long long)s_nvis);
-        if (blockIdx.x == 0) p.ctrl->n_sort = (unsigned long long)f.P;
-    }
 }
 
 template <int DEG>
 static void launch_pre(const Frame& f, const Pointers& p, const float* means, const float* scales, const float* rots,
                        const float* opac, const float* sh, int grid, cudaStream_t st) {
-    if (f.compact) launch_pdl(preprocess_kernel<DEG, true>, dim3(grid), dim3(PRE_THREADS), st, f, p, means, scales, rots, opac, sh);
-    else launch_pdl(preprocess_kernel<DEG, false>, dim3(grid), dim3(PRE_THREADS), st, f, p, means, scales, rots, opac, sh);
+    if (f.compact) launch_pdl(preprocess2_kernel<DEG>, dim3(grid), dim3(PRE_THREADS), st, f, p, means, scales, rots, opac, sh);
+    else launch_pdl(preprocess_kernel<DEG>, dim3(grid), dim3(PRE_THREADS), st, f, p, means, scales, rots, opac, sh);
 }
 
 void launch_preprocess(const Frame& f, const Pointers& p, const float* means, const float* scales, const float* rots,

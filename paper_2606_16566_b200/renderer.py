@@ -109,6 +109,10 @@ class Renderer:
         The current stream is joined to all lanes before returning, so later work on it sees the results."""
         n = len(cams)
         lanes = max(1, min(int(lanes), n))
+        if lanes == 1 and not to_host:      # one frame in flight: the caller's stream, no forks, no events
+            for i, cam in enumerate(cams):
+                self.render(cam, count_contrib=False, out_rgb=None if out_rgb is None else out_rgb[i])
+            return None
         main = torch.cuda.current_stream(self.device)
         fork = torch.cuda.Event()
         fork.record(main)

@@ -302,3 +302,29 @@ def test_render_batch_frames_in_flight_equal_plain_renders(lanes):
         if i >= n - min(lanes, n):
             assert torch.equal(lane_counts[i % lanes], r.out_tile_counts), "pose %d (tile counts)" % i
     assert not torch.equal(host[0], host[1])
+
+
+@pytest.mark.parametrize("config,P,W,H,f", [(3, 120_000, 637, 419, 500.0), (5, 1_100_000, 1283, 727, 1000.0)])
+def test_one_level_and_two_level_binning_give_the_same_frame(config, P, W, H, f):
+    """The binning strategy follows the workspace CAPACITY (<= 4 M entries: one radix sort over tile ids; above: sort
+    over 8x8-tile super-tiles + expand_kernel) and the preprocess kernel follows P (below 2^20: no compaction; above:
+    two-phase with compaction).  The frame may depend on neither: every integer output, the sorted lists and the
+    images must be bit-identical between a small and a large workspace, for a small and a large scene."""
+    sc = scenes.make_scene(config, P=P, W=W, H=H, f=f)
+    res = []
+    for cap in (3 << 20, 9 << 20):
+        r = pu.run_gpu(sc, 1, max_dup=cap, count_contrib=True)
+        it = r.intermediates(copy=("per_gaussian", "tile_ranges", "sorted_ids"))
+        assert it.n_dup <= 3 << 20, "pick a smaller scene: the one-level workspace must hold the frame"
+        assert (it.n_coarse > 0) == (cap > 4 << 20)
+        res.append((r, it))
+    (r1, i1), (r2, i2) = res
+    assert i1.n_dup == i2.n_dup and i1.n_visible == i2.n_visible
+    assert np.array_equal(i1.rect, i2.rect) and np.array_equal(i1.depth_bits, i2.depth_bits)
+    assert np.array_equal(i1.tile_ranges, i2.tile_ranges)
+    assert np.array_equal(i1.sorted_ids, i2.sorted_ids)
+    assert torch.equal(r1.out_tile_counts, r2.out_tile_counts)
+    assert torch.equal(r1.out_rgb, r2.out_rgb) and torch.equal(r1.out_final_T, r2.out_final_T)
+    assert torch.equal(r1.out_n_contrib, r2.out_n_contrib)
+    ref = oracle.render(sc, 1, n_threads=8, fragile_delta=pu.DELTA)
+    print(pu.compare(r2, i2, ref))

@@ -386,8 +386,8 @@ def run_ours(args):
     render_s = stage_ms["render"] * 1e-3
     achieved = pairs_eval * INSTR_PER_PAIR / render_s / 1e12
     # dram__bytes_read.sum + dram__bytes_write.sum of one render launch from the committed `ncu --set full` capture
-    # (profiles/r01_render_config2_final_ncu.md); only measured for the default workload
-    traffic = {2: 10132480}.get(args.config)
+    # (profiles/r01_render_config2_end_ncu.md); only measured for the default workload
+    traffic = {2: 10130944}.get(args.config)
     roofline = {"kernel": "render_b200_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                 "unit": "T FP32-pipe thread-instr/s", "frac": achieved / alu_peak, "traffic": traffic,
                 "peak_source": "derived: %d SMs x %d FP32 lanes x %.0f MHz (max SM clock)" % (n_sm, FP32_LANES_PER_SM, peaks["sm_max_mhz"]),

@@ -11,8 +11,8 @@
  *     keeps no reference to any pointer after the call returns, except that gs_get_intermediates() returns
  *     pointers INTO the caller's workspace.
  *   - Matrices are 16 floats, row-major, column-vector convention (p_cam = V * [p;1]).
- *   - All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream); one small
- *     kernel runs on a library-owned side stream, forked from and joined back into `cuda_stream` with events.
+ *   - All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream); the tile-grid
+ *     kernels run on a library-owned side stream, forked from and joined back into `cuda_stream` with events.
  *     gs_render() returns after enqueueing; it performs NO host synchronisation unless timing is enabled.
  *   - Return value: 0 (GS_OK) or a negative error code; nothing is printed, thrown or exit()ed.
  *   - Not thread-safe per workspace; distinct workspaces on distinct streams may be used concurrently.
@@ -53,8 +53,12 @@ size_t gs_workspace_bytes(int P, int W, int H, uint64_t max_dup);
  *    out_tile_counts [gy*gx] u32, gx=(W+15)/16, gy=(H+15)/16: length of each tile's sorted list
  *    out_n_contrib   [H,W]   u32 number of Gaussians blended into the pixel, or NULL
  *  workspace: dev, 256-byte aligned, >= gs_workspace_bytes(P, W, H, max_dup) bytes; max_dup is recovered from
- *    workspace_bytes (the largest capacity that fits).  If the frame produces more duplicates than fit, the image
- *    is rendered from the truncated lists and gs_get_intermediates() reports GS_ERR_OVERFLOW.
+ *    workspace_bytes (the largest capacity that fits).  If the frame produces more duplicates than fit, every tile
+ *    list is left empty (the image is the background) and gs_get_intermediates() reports GS_ERR_OVERFLOW with the
+ *    n_dup the frame needs.  The capacity also selects the binning strategy -- up to 4 Mi entries: one radix sort over
+ *    tile ids; above: radix sort over super-tiles of 8 x 8 tiles, then every tile list is written in place from its
+ *    super-tile's list -- and P the preprocess kernel (from 2^20 Gaussians: two-phase, compacting).  The outputs do
+ *    not depend on either choice.
  */
 int gs_render(int P, const float* means3D, const float* scales, const float* rotations, const float* opacities,
               const float* sh_coeffs, int sh_degree, const float* viewmatrix, const float* projmatrix, float fx,

@@ -293,6 +293,12 @@ def test_render_batch_frames_in_flight_equal_plain_renders(lanes):
         host2 = r.render_batch(cams, lanes=lanes, to_host=True)   # images left in the lanes' own buffers
         torch.cuda.current_stream().synchronize()
         assert torch.equal(host, host2.clone())
+    plain = torch.empty_like(dev_imgs)                     # no host copy: with one lane this is the plain-stream path
+    r.render_batch(cams, lanes=lanes, out_rgb=plain)
+    torch.cuda.current_stream().synchronize()
+    assert torch.equal(plain, dev_imgs)
+    r.render_batch(cams, lanes=lanes, to_host=True)        # leaves the last frame of every lane in the lane's buffers
+    torch.cuda.current_stream().synchronize()
     lane_counts = [r._lanes[k]["out_tile_counts"].clone() for k in range(min(lanes, n))]
     for i, cam in enumerate(cams):
         r.render(cam, count_contrib=False)

@@ -334,3 +334,18 @@ def test_one_level_and_two_level_binning_give_the_same_frame(config, P, W, H, f)
     assert torch.equal(r1.out_n_contrib, r2.out_n_contrib)
     ref = oracle.render(sc, 1, n_threads=8, fragile_delta=pu.DELTA)
     print(pu.compare(r2, i2, ref))
+
+
+@pytest.mark.parametrize("cap", [8000, (256 << 10), (256 << 10) + 1, (4 << 20), (4 << 20) + 1, 6_000_000])
+def test_capacity_recovered_from_the_workspace_size_is_never_below_the_one_asked_for(cap):
+    """gs_render recovers max_dup from workspace_bytes; the layout changes regime at 256 Ki (radix tile size) and 4 Mi
+    entries (binning levels), where its size is not monotone.  A workspace sized by gs_workspace_bytes(.., cap) must give
+    back at least `cap`, and the frame must be the same on both sides of every edge."""
+    sc = scenes.make_scene(1)
+    r = pu.run_gpu(sc, 0, max_dup=cap, count_contrib=True)
+    it = r.intermediates(copy=("tile_ranges", "sorted_ids"))
+    assert it.max_dup >= cap, (it.max_dup, cap)
+    ref = pu.run_gpu(sc, 0, max_dup=1 << 20, count_contrib=True)
+    it0 = ref.intermediates(copy=("tile_ranges", "sorted_ids"))
+    assert np.array_equal(it.sorted_ids, it0.sorted_ids) and np.array_equal(it.tile_ranges, it0.tile_ranges)
+    assert torch.equal(r.out_rgb, ref.out_rgb) and torch.equal(r.out_n_contrib, ref.out_n_contrib)

@@ -296,8 +296,8 @@ def run_ours(args):
     while time.perf_counter() - t0 < 0.5:
         step()
         torch.cuda.synchronize()
-    if args.lanes <= 0:   # untimed tuning: the fastest of 1, 2, 3, 4 frames in flight over a few warm-up steps (rank 0 decides)
-        cands = [1, 2, 3, 4] if r.workspace.numel() < (8 << 30) else [1, 2]
+    if args.lanes <= 0:   # untimed tuning: the fastest of 1, 2, 3, 4, 6 frames in flight over a few warm-up steps (rank 0 decides)
+        cands = [1, 2, 3, 4, 6] if r.workspace.numel() < (4 << 30) else [1, 2]
         best = (None, 1)
         for cand in cands:
             lanes = cand
@@ -454,7 +454,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=(1, 2, 3, 4, 5))
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = the fastest of 1-4 over a few warm-up steps)")
+    ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = the fastest of 1-6 over a few warm-up steps)")
     ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

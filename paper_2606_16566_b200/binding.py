@@ -24,7 +24,8 @@ TIMING_NAMES = ("preprocess", "depth_sort", "tile_grid", "offset_scan", "duplica
 
 EXPORTS = ("gs_workspace_bytes", "gs_render", "gs_get_intermediates", "gs_set_timing", "gs_get_timings",
            "gs_set_render_variant", "gs_get_render_variant", "gs_last_launch_count", "gs_error_string",
-           "gs_last_cuda_error", "gs_copy_to_host", "gs_set_stats", "gs_get_stats", "gs_selftest_atomic_order")
+           "gs_last_cuda_error", "gs_copy_to_host", "gs_set_stats", "gs_get_stats", "gs_selftest_atomic_order",
+           "gs_set_render_stream")
 GS_N_STATS = 4
 STATS_NAMES = ("warp_slots_walked", "pairs_blended", "entries_staged", "pairs_evaluated")
 
@@ -71,6 +72,8 @@ def lib():
         L.gs_set_render_variant.restype = C.c_int
         L.gs_set_render_variant.argtypes = [C.c_int]
         L.gs_get_render_variant.restype = C.c_int
+        L.gs_set_render_stream.restype = C.c_int
+        L.gs_set_render_stream.argtypes = [C.c_int]
         L.gs_last_launch_count.restype = C.c_int
         L.gs_error_string.restype = C.c_char_p
         L.gs_error_string.argtypes = [C.c_int]
@@ -178,6 +181,10 @@ def gs_get_intermediates(workspace, copy=("per_gaussian", "tile_ranges", "sorted
     if "sorted_ids" in copy:
         out.sorted_ids = _copy_out(it.sorted_ids, min(it.n_dup, it.max_dup), np.uint32, dev)
     return out
+
+
+def gs_set_render_stream(enable: bool) -> None:
+    lib().gs_set_render_stream(1 if enable else 0)
 
 
 def gs_set_timing(enable: bool) -> None:

@@ -109,11 +109,13 @@ struct LastCall {
     bool have_events = false;
     cudaStream_t side = nullptr;          // tile-grid kernel runs here, concurrently with the depth sort
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaStream_t rstream = nullptr;       // gs_set_render_stream(1): the render kernel runs on this lowest-priority stream
+    cudaEvent_t ev_r0 = nullptr, ev_r1 = nullptr;
 };
 
 std::mutex g_mu;
 std::map<const void*, LastCall> g_calls;
-std::atomic<int> g_variant{4}, g_timing{0}, g_stats{0}, g_launches{0}, g_cuda_err{0};
+std::atomic<int> g_variant{4}, g_timing{0}, g_stats{0}, g_launches{0}, g_cuda_err{0}, g_render_stream{0};
 int g_n_sm = 0;
 
 int cuda_fail(cudaError_t e) {
@@ -308,9 +310,27 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     }
     mark(6);
     const int variant = g_variant.load();                      // (4) render
-    if (variant == 5) launch_render_ws(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
-    else if (variant == 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, st);
-    else launch_render_ladder(variant, f, p, out_rgb, out_final_T, out_n_contrib, st);
+    const bool render_stream = g_render_stream.load() != 0;
+    cudaStream_t rs = st;
+    if (render_stream && !timed) {
+        if (!lc->rstream) {
+            int lo = 0, hi = 0;
+            cudaDeviceGetStreamPriorityRange(&lo, &hi);
+            cudaStreamCreateWithPriority(&lc->rstream, cudaStreamNonBlocking, lo);
+            cudaEventCreateWithFlags(&lc->ev_r0, cudaEventDisableTiming);
+            cudaEventCreateWithFlags(&lc->ev_r1, cudaEventDisableTiming);
+        }
+        rs = lc->rstream;
+        cudaEventRecord(lc->ev_r0, st);
+        cudaStreamWaitEvent(rs, lc->ev_r0, 0);
+    }
+    if (variant == 5) launch_render_ws(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, rs);
+    else if (variant == 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, rs);
+    else launch_render_ladder(variant, f, p, out_rgb, out_final_T, out_n_contrib, rs);
+    if (rs != st) {
+        cudaEventRecord(lc->ev_r1, rs);
+        cudaStreamWaitEvent(st, lc->ev_r1, 0);
+    }
     launches++;
     mark(7);
     g_launches.store(launches);
@@ -445,6 +465,10 @@ int gs_set_render_variant(int variant) {
     return GS_OK;
 }
 int gs_get_render_variant(void) { return g_variant.load(); }
+int gs_set_render_stream(int enable) {
+    g_render_stream.store(enable ? 1 : 0);
+    return GS_OK;
+}
 int gs_last_launch_count(void) { return g_launches.load(); }
 int gs_last_cuda_error(void) { return g_cuda_err.load(); }
 

@@ -88,7 +88,7 @@ class Renderer:
             self._lanes = []
         while len(self._lanes) <= k:
             first = len(self._lanes) == 0
-            ln = dict(stream=torch.cuda.Stream(device=self.device),
+            ln = dict(stream=torch.cuda.Stream(device=self.device, priority=-1),   # above the library's render stream
                       workspace=self.workspace if first else torch.empty_like(self.workspace),
                       out_rgb=self.out_rgb if first else torch.empty_like(self.out_rgb),
                       out_final_T=self.out_final_T if first else torch.empty_like(self.out_final_T),
@@ -116,6 +116,9 @@ class Renderer:
         main = torch.cuda.current_stream(self.device)
         fork = torch.cuda.Event()
         fork.record(main)
+        # several frames in flight: binning kernels on the lanes' high-priority streams, render kernels on the library's
+        # lowest-priority stream of each workspace (include/gs.h: gs_set_render_stream)
+        binding.gs_set_render_stream(lanes > 1)
         host = None
         if to_host:
             if self._host_rgb is None or self._host_rgb.shape[0] < n:
@@ -144,6 +147,7 @@ class Renderer:
                     host[i].copy_(img, non_blocking=True)
                 ln["copied"].record(cs)
                 ln["copy_pending"] = True
+        binding.gs_set_render_stream(False)
         for k in range(lanes):
             main.wait_event(self._lanes[k]["done"])
         if to_host:

@@ -219,7 +219,11 @@ def run_ours(args):
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
 
     cfg = scenes.config_defaults(args.config)
-    sc = scenes.make_scene(args.config)
+    if args.res_scale != 1:   # PAPER.md Table VI's 1x / 2x resolution axis: same scene, image and focal length scaled
+        cfg = dict(cfg, W=cfg["W"] * args.res_scale, H=cfg["H"] * args.res_scale, f=cfg["f"] * args.res_scale)
+        sc = scenes.make_scene(args.config, W=cfg["W"], H=cfg["H"], f=cfg["f"])
+    else:
+        sc = scenes.make_scene(args.config)
     cams = sc.cameras
     n_pose = len(cams)
     W, H = cfg["W"], cfg["H"]
@@ -431,7 +435,7 @@ def run_ours(args):
                     "frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every step", "frames_in_flight": lanes,
                     "parallelism": "replicas x%d" % ws,
                     "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "n_coarse_mean": n_coarse_m,
-                    "binning": "two-level (8x8-tile super-tiles)" if n_coarse_m > 0 else "one-level", "render_variant": binding.gs_get_render_variant()}),
+                    "binning": "two-level (8x8-tile super-tiles)" if n_coarse_m > 0 else "one-level", "res_scale": args.res_scale, "render_variant": binding.gs_get_render_variant()}),
                 "ms_per_frame": ms_per_step / n_pose, "wall_ms_per_step_incl_flush": 1e3 * wall / K,
                 "latency": {"ms_per_frame": serial_ms_per_frame, "frames_per_s": ws * 1e3 / serial_ms_per_frame,
                             "how": "one frame in flight, one stream, L2 flushed before every frame"},
@@ -455,6 +459,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = the fastest of 1-6 over a few warm-up steps)")
+    ap.add_argument("--res-scale", type=int, default=1, choices=(1, 2), help="render at 1x or 2x the configuration's resolution (our arm only)")
     ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -349,3 +349,40 @@ def test_capacity_recovered_from_the_workspace_size_is_never_below_the_one_asked
     it0 = ref.intermediates(copy=("tile_ranges", "sorted_ids"))
     assert np.array_equal(it.sorted_ids, it0.sorted_ids) and np.array_equal(it.tile_ranges, it0.tile_ranges)
     assert torch.equal(r.out_rgb, ref.out_rgb) and torch.equal(r.out_n_contrib, ref.out_n_contrib)
+
+
+def test_two_level_binning_edge_cases():
+    """The large-capacity path (two-level binning) on the degenerate frames: nothing visible, an overflowing frame
+    (every list left empty, the need reported, the workspace reusable afterwards), and a one-tile-wide image whose
+    super-tile grid is a single partial cell."""
+    cap = 5 << 20                                               # > 4 Mi entries: two levels
+    bg = np.array([0.25, 0.5, 0.75], np.float32)
+    # (a) everything behind the camera
+    sc = scenes.make_scene(1, P=500, W=70, H=45)
+    sc.means3D[:, 2] = -sc.means3D[:, 2]
+    sc.bg = bg
+    r = pu.run_gpu(sc, 0, max_dup=cap)
+    it = r.intermediates()
+    assert it.n_dup == 0 and it.n_coarse == 0 and int(r.out_tile_counts.sum()) == 0
+    assert torch.equal(r.out_final_T, torch.ones_like(r.out_final_T))
+    assert np.array_equal(r.out_rgb.cpu().numpy(), np.broadcast_to(bg[:, None, None], (3, 45, 70)))
+    # (b) overflow above the two-level threshold: config 3's distribution, ~6.7 M entries into 5 Mi... then enough room
+    sc = scenes.make_scene(3, P=500_000, W=1264, H=832)
+    need = int(oracle.render(sc, 0, flags=oracle.NO_LISTS).n_dup)
+    assert need > cap, need
+    r = pu.run_gpu(sc, 0, max_dup=cap)
+    with pytest.raises(binding.GsError) as ei:
+        r.intermediates()
+    assert ei.value.code == binding.GS_ERR_OVERFLOW and ei.value.n_dup == need
+    assert torch.equal(r.out_final_T, torch.ones_like(r.out_final_T))
+    del r
+    torch.cuda.empty_cache()
+    rep, *_ = pu.oracle_and_compare(sc, 0)                      # grows the workspace from the reported need
+    print(rep)
+    # (c) a 16 x 200 image: one tile column, super-tile grid 1 x 2 with partial cells
+    sc = scenes.make_scene(1, P=2000, W=16, H=200, f=100.0)
+    r = pu.run_gpu(sc, 0, max_dup=cap)
+    it = r.intermediates()
+    ref = oracle.render(sc, 0, n_threads=4, fragile_delta=pu.DELTA)
+    assert it.n_coarse > 0
+    print(pu.compare(r, it, ref))

@@ -366,6 +366,10 @@ preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ me
                         pg.z = __float_as_uint(t.depth);
                         pg.w = (uint32_t)t.radius;
                         g[h] = float5{t.mux, t.muy, t.ca, t.cb, t.cc};
+                        // the SH block is read in part 2: start it towards L2 now (12 K floats = 1-2 lines of 128 bytes)
+                        const char* shp = reinterpret_cast<const char*>(sh + (size_t)i * (3 * (DEG + 1) * (DEG + 1)));
+#pragma unroll
+                        for (int o = 0; o < 12 * (DEG + 1) * (DEG + 1); o += 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(shp + o));
                     }
                     p.per_g[i] = pg;
                 }

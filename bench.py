@@ -377,9 +377,17 @@ def run_ours(args):
         h2d_bytes = e2e_step()
     barrier()
     torch.cuda.synchronize()
+    # K steps, each with its own host -> device copy of the scene and its own device -> host copies of the images; the
+    # upload of step k+1 goes to a second set of device buffers on an upload stream while step k is rendered and read back
     t0 = time.perf_counter()
-    for _ in range(K):
-        e2e_step()
+    r.upload_async(sc)
+    for k in range(K):
+        r.activate_uploaded()
+        if k + 1 < K:
+            r.upload_async(sc)
+        r.render_batch(cams, lanes=lanes, to_host=True)
+    r.synchronize_readback()
+    torch.cuda.synchronize()
     e2e_s = rank_max(time.perf_counter() - t0)
     h2d_bytes += n_pose * (16 + 16 + 3) * 4
     d2h_bytes = n_pose * 3 * H * W * 4
@@ -419,7 +427,7 @@ def run_ours(args):
         cores = os.cpu_count() or 1
         t0 = time.perf_counter()
         nf = 0
-        while nf < 2 * n_pose and (time.perf_counter() - t0 < 8.0 or nf == 0):
+        while nf < 8 * n_pose and (time.perf_counter() - t0 < 10.0 or nf == 0):
             oracle.render(sc, nf % n_pose, n_threads=cores)
             nf += 1
         dt = time.perf_counter() - t0

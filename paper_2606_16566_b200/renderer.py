@@ -31,6 +31,8 @@ class Renderer:
         self._ring = None     # render_to_host(): two device images, a copy stream and the events that order them
         self._lanes = None    # render_batch(): per-lane stream, workspace and outputs
         self._copy_stream = None
+        self._standby = None  # upload_async(): second set of scene buffers, upload stream and its events
+        self._upload_stream = None
 
     def upload(self, scene) -> int:
         """Host (numpy) scene -> device tensors: pinned staging, async copies on the current stream.  The staging and
@@ -45,6 +47,37 @@ class Renderer:
             self.scene[n].copy_(self._pinned[n], non_blocking=True)
             nbytes += self._pinned[n].numel() * 4
         return nbytes
+
+    def upload_async(self, scene) -> int:
+        """Host -> device copy of the scene into the STANDBY set of device buffers, on an upload stream: it overlaps the
+        frames that are being rendered from the active set (PCIe is full duplex: the images of those frames travel the
+        other way).  activate_uploaded() makes the new set the active one.  Returns the bytes copied."""
+        if self._pinned is None:
+            self.upload(scene)                 # first use: allocates the pinned staging and the first device set
+        if self._standby is None:
+            self._standby = {n: torch.empty_like(self.scene[n]) for n in _SCENE_ARRAYS}
+            self._upload_stream = torch.cuda.Stream(device=self.device)
+            self._uploaded, self._released = torch.cuda.Event(), torch.cuda.Event()
+            self._released.record(torch.cuda.current_stream(self.device))
+        up = self._upload_stream
+        up.wait_event(self._released)          # the frames that read the standby set (two activations ago) are done
+        nbytes = 0
+        with torch.cuda.stream(up):
+            for n in _SCENE_ARRAYS:
+                self._standby[n].copy_(self._pinned[n], non_blocking=True)
+                nbytes += self._pinned[n].numel() * 4
+        self._uploaded.record(up)
+        return nbytes
+
+    def activate_uploaded(self) -> None:
+        """Later renders (enqueued on the current stream or forked from it) read the set upload_async() filled."""
+        main = torch.cuda.current_stream(self.device)
+        self._released.record(main)            # everything enqueued so far read the old active set
+        main.wait_event(self._uploaded)
+        old = {n: self.scene[n] for n in _SCENE_ARRAYS}
+        for n in _SCENE_ARRAYS:
+            self.scene[n] = self._standby[n]
+        self._standby = old
 
     def render(self, cam, stream=None, count_contrib: bool = True, out_rgb=None) -> None:
         s = self.scene

@@ -386,3 +386,41 @@ def test_two_level_binning_edge_cases():
     ref = oracle.render(sc, 0, n_threads=4, fragile_delta=pu.DELTA)
     assert it.n_coarse > 0
     print(pu.compare(r, it, ref))
+
+
+def test_overlapped_scene_upload_switches_buffer_sets_safely():
+    """Renderer.upload_async() fills a second set of scene buffers on an upload stream while frames are rendered from the
+    active one; activate_uploaded() switches.  Alternating two DIFFERENT scenes of the same size through it must give, for
+    each, exactly the frames a fresh renderer produces -- a copy that overtook the frames still reading its target set,
+    or a frame that started before its upload finished, would show up as a mismatch."""
+    sa = scenes.make_scene(2, P=20_000, W=320, H=240, f=400.0)
+    sb = scenes.make_scene(2, P=20_000, W=320, H=240, f=400.0)
+    sb.means3D = (sb.means3D[::-1] * np.float32(0.9)).copy()       # a different scene with the same shapes
+    binding.gs_set_render_variant(binding.GS_DEFAULT_RENDER_VARIANT)
+    want = []
+    for sc in (sa, sb):
+        r0 = Renderer(sc.P, 320, 240, 1 << 20, device="cuda:0", count_contrib=False)
+        r0.upload(sc)
+        host = r0.render_batch(list(sc.cameras), lanes=1, to_host=True)
+        torch.cuda.synchronize()
+        want.append(host.clone())
+    assert not torch.equal(want[0], want[1])
+    r = Renderer(sa.P, 320, 240, 1 << 20, device="cuda:0", count_contrib=False)
+    r.upload(sa)
+    pinned = {0: r._pinned}
+    r2 = Renderer(sb.P, 320, 240, 1 << 20, device="cuda:0", count_contrib=False)
+    r2.upload(sb)
+    pinned[1] = r2._pinned                                          # pinned staging of the second scene
+    torch.cuda.synchronize()
+    got = []
+    r._pinned = pinned[0]
+    r.upload_async(sa)
+    for k in range(6):
+        r.activate_uploaded()
+        r._pinned = pinned[(k + 1) & 1]
+        r.upload_async(sb if (k + 1) & 1 else sa)                   # overlaps the frames of this step
+        host = r.render_batch(list(sa.cameras), lanes=3, to_host=True)
+        torch.cuda.current_stream().synchronize()
+        got.append(host.clone())
+    for k in range(6):
+        assert torch.equal(got[k], want[k & 1]), "step %d" % k

@@ -76,11 +76,13 @@ typedef struct gs_intermediates {
     const uint32_t* per_gaussian;  /* dev [P,4] u32: {xmin | ymin<<16, xmax | ymax<<16, depth bits, radius};
                                       rect in tiles, half-open; all zero for a culled Gaussian                   */
     const float* record;           /* dev [P,16], the 64-byte render record, defined only where tiles_touched > 0:
-                                      [0..1] mu_x, mu_y (pixels)   [2..4] conic a, b, c (Eq. 5)
-                                      [5] log2(opacity)   [6] a*c-b*b   [7] flags (bits; 1 = degenerate conic)
-                                      [8..10] r, g, b (SH colour clamped at 0)
-                                      [11] x*  [12] 1/c  [13] c*tau: per-Gaussian constants of the tight box
-                                      (Eq. 13-18; tau = 2 ln(255 o) widened)   [14..15] 0                        */
+                                      first 32 bytes -- all the tight box (Eq. 13-18) of the render stage reads:
+                                      [0..1] mu_x, mu_y (pixels)   [2] conic b (Eq. 5)   [3] a*c-b*b
+                                      [4] x*  [5] 1/c  [6] c*tau: per-Gaussian constants of the tight box (tau =
+                                      2 ln(255 o) widened)   [7] flags (bits; 1 = degenerate conic)
+                                      second 32 bytes -- read only for entries that reach a pixel (hoist, Eq. 8):
+                                      [8] conic a  [9] conic c  [10] log2(opacity)
+                                      [11..13] r, g, b (SH colour clamped at 0)   [14..15] 0                       */
     const uint64_t* depth_sorted;  /* dev [n_visible]: (depth bits << 32 | Gaussian id), ascending, stable       */
     const uint32_t* dup_offsets;   /* dev [n_visible]: exclusive prefix sum, in depth order, of the number of
                                       SUPER-TILES (8 x 8 tiles) each Gaussian's tile rect reaches -- the level the

@@ -171,8 +171,9 @@ def gs_get_intermediates(workspace, copy=("per_gaussian", "tile_ranges", "sorted
         out.tiles_touched = ((out.rect[:, 2] - out.rect[:, 0]) * (out.rect[:, 3] - out.rect[:, 1])).astype(np.uint32)
     if "geom" in copy:
         out.record = _copy_out(it.record, 16 * it.P, np.float32, dev).reshape(it.P, 16)
-        out.geom = out.record[:, 0:8]
-        out.colour = out.record[:, 8:12]
+        rc = out.record   # layout: include/gs.h {mu_x, mu_y, b, det | x*, 1/c, c tau, flags | a, c, log2 o, r | g, b, -, -}
+        out.geom = np.stack([rc[:, 0], rc[:, 1], rc[:, 8], rc[:, 2], rc[:, 9], rc[:, 10], rc[:, 3], rc[:, 7]], axis=1)  # mu, conic a b c, log2 o, det, flags
+        out.colour = np.stack([rc[:, 11], rc[:, 12], rc[:, 13]], axis=1)
     if "depth_sorted" in copy:
         out.depth_sorted = _copy_out(it.depth_sorted, it.n_visible, np.uint64, dev)
         out.dup_offsets = _copy_out(it.dup_offsets, it.n_visible, np.uint32, dev)

@@ -25,7 +25,7 @@ UNITS = {
     "render.cu": ["-use_fast_math"],
     "render_b200.cu": ["-use_fast_math"],
 }
-HEADERS = ["common.cuh", "render_common.cuh"]
+HEADERS = ["common.cuh", "render_common.cuh", "render_blend.cuh"]
 
 
 def _nvcc() -> str:

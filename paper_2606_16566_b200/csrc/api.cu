@@ -22,7 +22,6 @@ void launch_duplicate_and_tile_sort(const Frame&, const Pointers&, int, cudaStre
 void launch_atomic_order_selftest(unsigned long long*, int, uint32_t, int, int, cudaStream_t);
 void launch_render_ladder(int, const Frame&, const Pointers&, float*, float*, uint32_t*, cudaStream_t);
 void launch_render_b200(const Frame&, const Pointers&, float*, float*, uint32_t*, int, bool, cudaStream_t);
-void launch_render_ws(const Frame&, const Pointers&, float*, float*, uint32_t*, int, bool, cudaStream_t);
 }  // namespace gs
 
 namespace {
@@ -324,8 +323,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
         cudaEventRecord(lc->ev_r0, st);
         cudaStreamWaitEvent(rs, lc->ev_r0, 0);
     }
-    if (variant == 5) launch_render_ws(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, rs);
-    else if (variant == 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, rs);
+    if (variant == 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, rs);
     else launch_render_ladder(variant, f, p, out_rgb, out_final_T, out_n_contrib, rs);
     if (rs != st) {
         cudaEventRecord(lc->ev_r1, rs);
@@ -460,7 +458,7 @@ int gs_copy_to_host(void* dst_host, const void* src_dev, size_t bytes) {
 }
 
 int gs_set_render_variant(int variant) {
-    if (variant < 0 || variant > 6) return GS_ERR_BAD_ARG;
+    if (variant < 0 || variant > 6 || variant == 5) return GS_ERR_BAD_ARG;
     g_variant.store(variant);
     return GS_OK;
 }

@@ -262,10 +262,10 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             const TightBox tb = tight_box_constants(s.ca, s.cb, s.cc, (float)dd, l2o);
             const uint32_t flags = (!(dd > 0.0) || tb.degenerate) ? 1u : 0u;
             float4* rec = p.rec + 4 * (size_t)i;  // 64-byte render record (include/gs.h: gs_intermediates.record)
-            rec[0] = make_float4(s.mux, s.muy, s.ca, s.cb);
-            rec[1] = make_float4(s.cc, l2o, (float)dd, __uint_as_float(flags));
-            rec[2] = make_float4(col.x, col.y, col.z, tb.xstar);
-            rec[3] = make_float4(tb.ic, tb.ct, 0.0f, 0.0f);
+            rec[0] = make_float4(s.mux, s.muy, s.cb, (float)dd);          // the half the tight box needs ...
+            rec[1] = make_float4(tb.xstar, tb.ic, tb.ct, __uint_as_float(flags));
+            rec[2] = make_float4(s.ca, s.cc, l2o, col.x);                   // ... and the half only the hoist needs
+            rec[3] = make_float4(col.y, col.z, 0.0f, 0.0f);
         }
     }
     __syncthreads();
@@ -421,10 +421,10 @@ preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ me
                 const TightBox tb = tight_box_constants(t.ca, t.cb, t.cc, (float)dd, l2o);
                 const uint32_t flags = (!(dd > 0.0) || tb.degenerate) ? 1u : 0u;
                 float4* rec = p.rec + 4 * (size_t)i;  // 64-byte render record (include/gs.h: gs_intermediates.record)
-                rec[0] = make_float4(t.mux, t.muy, t.ca, t.cb);
-                rec[1] = make_float4(t.cc, l2o, (float)dd, __uint_as_float(flags));
-                rec[2] = make_float4(col.x, col.y, col.z, tb.xstar);
-                rec[3] = make_float4(tb.ic, tb.ct, 0.0f, 0.0f);
+                rec[0] = make_float4(t.mux, t.muy, t.cb, (float)dd);          // the half the tight box needs ...
+                rec[1] = make_float4(tb.xstar, tb.ic, tb.ct, __uint_as_float(flags));
+                rec[2] = make_float4(t.ca, t.cc, l2o, col.x);                   // ... and the half only the hoist needs
+                rec[3] = make_float4(col.y, col.z, 0.0f, 0.0f);
             }
         }
         // ---- exclusive prefix by decoupled look-back; keys of the visible Gaussians in index order ------------------

@@ -60,8 +60,11 @@ render_ladder_kernel(const Frame f, const uint32_t* __restrict__ ranges, const u
             const uint32_t k = base + tid;
             if (k < end) {
                 const uint32_t id = ids[k];
-                const float4 g0 = __ldg(rec + 4 * (size_t)id), g1 = __ldg(rec + 4 * (size_t)id + 1);
-                s_col[tid] = __ldg(rec + 4 * (size_t)id + 2);
+                // 64-byte render record (include/gs.h): {mu_x, mu_y, b, det | x*, 1/c, c tau, flags | a, c, log2 o, r | g, b, -, -}
+                const float4 k0 = __ldg(rec + 4 * (size_t)id), k1 = __ldg(rec + 4 * (size_t)id + 1),
+                             k2 = __ldg(rec + 4 * (size_t)id + 2), k3 = __ldg(rec + 4 * (size_t)id + 3);
+                const float4 g0 = make_float4(k0.x, k0.y, k2.x, k0.z), g1 = make_float4(k2.y, k2.z, k0.w, k1.w);
+                s_col[tid] = make_float4(k2.w, k3.x, k3.y, 0.0f);
                 const bool indefinite = __float_as_uint(g1.w) & 1u;
                 if (HOIST) {
                     const Hoisted h = GLOBAL ? hoist_f32(g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, 0.0f, 0.0f)

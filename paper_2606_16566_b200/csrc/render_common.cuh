@@ -31,6 +31,13 @@ __device__ __forceinline__ double f2d(float x) {
     asm("cvt.f64.f32 %0, %1;" : "=d"(d) : "f"(x));
     return d;
 }
+// round-to-nearest fp64 -> fp32 conversion (plain cvt: under -use_fast_math a C++ cast adds a compare and a multiply per
+// value to flush denormal results, which no coefficient here can be)
+__device__ __forceinline__ float d2f(double x) {
+    float f;
+    asm("cvt.rn.f32.f64 %0, %1;" : "=f"(f) : "d"(x));
+    return f;
+}
 __device__ __forceinline__ Hoisted hoist(float mux, float muy, float a, float b, float c, float log2o, float ox, float oy,
                                          float bias = 0.0f) {
     const double k = 1.4426950408889634;
@@ -38,12 +45,12 @@ __device__ __forceinline__ Hoisted hoist(float mux, float muy, float a, float b,
     const double da = f2d(a), db = f2d(b), dc = f2d(c);
     const double gx = da * dx + db * dy, gy = db * dx + dc * dy;
     Hoisted h;
-    h.A = (float)(-0.5 * k * da);
-    h.B = (float)(-k * db);
-    h.C = (float)(-0.5 * k * dc);
-    h.D = (float)(k * gx);
-    h.E = (float)(k * gy);
-    h.F = (float)((f2d(log2o) + (double)bias) - 0.5 * k * (gx * dx + gy * dy));
+    h.A = d2f(-0.5 * k * da);
+    h.B = d2f(-k * db);
+    h.C = d2f(-0.5 * k * dc);
+    h.D = d2f(k * gx);
+    h.E = d2f(k * gy);
+    h.F = d2f((f2d(log2o) + f2d(bias)) - 0.5 * k * (gx * dx + gy * dy));
     return h;
 }
 

@@ -5,6 +5,8 @@ binding.gs_render -- no arithmetic of the method lives here.
 """
 from __future__ import annotations
 
+from types import SimpleNamespace
+
 import numpy as np
 import torch
 
@@ -26,7 +28,8 @@ class Renderer:
         self.out_tile_counts = torch.empty((self.gy * self.gx,), dtype=torch.int32, device=self.device)
         self.out_n_contrib = torch.empty((H, W), dtype=torch.int32, device=self.device) if count_contrib else None
         self.scene = None
-        self._pinned = None   # host staging of the scene arrays (pinned), allocated on the first upload
+        self._pinned = None   # two pinned host staging sets of the scene arrays, allocated on first use
+        self._pinned_read = None
         self._host_rgb = None
         self._ring = None     # render_to_host(): two device images, a copy stream and the events that order them
         self._lanes = None    # render_batch(): per-lane stream, workspace and outputs
@@ -34,38 +37,87 @@ class Renderer:
         self._standby = None  # upload_async(): second set of scene buffers, upload stream and its events
         self._upload_stream = None
 
-    def upload(self, scene) -> int:
-        """Host (numpy) scene -> device tensors: pinned staging, async copies on the current stream.  The staging and
-        device buffers are allocated on the first call and reused.  Returns the bytes copied host -> device."""
+    # ---- host -> device ---------------------------------------------------------------------------------------------
+    @staticmethod
+    def pin_scene(scene):
+        """A copy of `scene` whose arrays are pinned torch tensors: upload() / upload_async() copy from those directly
+        (no staging pass).  The caller must not modify them while a copy is in flight."""
+        out = SimpleNamespace(sh_degree=int(scene.sh_degree), bg=np.array(scene.bg, dtype=np.float32), cameras=getattr(scene, "cameras", None))
+        for n in _SCENE_ARRAYS:
+            setattr(out, n, torch.from_numpy(np.array(getattr(scene, n), dtype=np.float32, order="C")).pin_memory())
+        return out
+
+    def _stage_to_pinned(self, scene, k: int):
+        """Host arrays of `scene` as pinned tensors: the scene's own tensors when they are pinned already, else pinned
+        staging set k (allocated on first use), filled after the host -> device copy that last read that set has
+        finished.  Checks P and the array shapes.  Returns (dict of pinned tensors, bytes)."""
+        if int(scene.means3D.shape[0]) != self.P:
+            raise ValueError("scene has %d Gaussians, this Renderer was built for %d" % (scene.means3D.shape[0], self.P))
         if self._pinned is None:
-            self._pinned = {n: torch.from_numpy(np.array(getattr(scene, n), dtype=np.float32, order="C")).pin_memory()
-                            for n in _SCENE_ARRAYS}
-            dev = {n: torch.empty_like(t, device=self.device) for n, t in self._pinned.items()}
-            self.scene = dict(dev, sh_degree=int(scene.sh_degree), bg=np.array(scene.bg, dtype=np.float32))
+            self._pinned = [None, None]
+            self._pinned_read = [torch.cuda.Event(), torch.cuda.Event()]
+        if all(isinstance(getattr(scene, n), torch.Tensor) and getattr(scene, n).is_pinned() for n in _SCENE_ARRAYS):
+            src = {n: getattr(scene, n) for n in _SCENE_ARRAYS}
+            for n, t in src.items():
+                if t.dtype != torch.float32 or not t.is_contiguous() or (self.scene is not None and tuple(t.shape) != tuple(self.scene[n].shape)):
+                    raise ValueError("%s must be a contiguous float32 tensor of the shape this Renderer was sized for" % n)
+            return src, sum(t.numel() * 4 for t in src.values())
+        if self._pinned[k] is None:
+            self._pinned[k] = {n: torch.empty(tuple(np.shape(getattr(scene, n))), dtype=torch.float32).pin_memory()
+                               for n in _SCENE_ARRAYS}
+        else:
+            self._pinned_read[k].synchronize()      # the previous copy out of this staging set has completed
         nbytes = 0
         for n in _SCENE_ARRAYS:
-            self.scene[n].copy_(self._pinned[n], non_blocking=True)
-            nbytes += self._pinned[n].numel() * 4
+            src = np.ascontiguousarray(getattr(scene, n), dtype=np.float32)
+            dst = self._pinned[k][n]
+            if tuple(src.shape) != tuple(dst.shape):
+                raise ValueError("%s has shape %s, this Renderer was sized for %s" % (n, src.shape, tuple(dst.shape)))
+            dst.numpy()[...] = src
+            nbytes += src.nbytes
+        return self._pinned[k], nbytes
+
+    def _scene_meta(self, scene):
+        return int(scene.sh_degree), np.array(scene.bg, dtype=np.float32)
+
+    def upload(self, scene) -> int:
+        """Host (numpy) scene -> device tensors, every call: the arrays are staged into pinned memory and copied
+        asynchronously on the current stream; sh_degree and bg follow the scene.  Staging and device buffers are
+        allocated on the first call and reused.  Returns the bytes copied host -> device."""
+        src, nbytes = self._stage_to_pinned(scene, 0)
+        deg, bg = self._scene_meta(scene)
+        if self.scene is None:
+            self.scene = {n: torch.empty_like(t, device=self.device) for n, t in src.items()}
+        for n in _SCENE_ARRAYS:
+            self.scene[n].copy_(src[n], non_blocking=True)
+        self._pinned_read[0].record(torch.cuda.current_stream(self.device))
+        self.scene["sh_degree"], self.scene["bg"] = deg, bg
         return nbytes
 
     def upload_async(self, scene) -> int:
-        """Host -> device copy of the scene into the STANDBY set of device buffers, on an upload stream: it overlaps the
+        """Host -> device copy of `scene` into the STANDBY set of device buffers, on an upload stream: it overlaps the
         frames that are being rendered from the active set (PCIe is full duplex: the images of those frames travel the
-        other way).  activate_uploaded() makes the new set the active one.  Returns the bytes copied."""
-        if self._pinned is None:
-            self.upload(scene)                 # first use: allocates the pinned staging and the first device set
+        other way).  Two pinned staging sets are used alternately, so the host-side staging of one upload never
+        overwrites memory a previous copy still reads.  activate_uploaded() makes the new set (and the scene's
+        sh_degree / bg) the active one.  Returns the bytes copied."""
+        if self.scene is None:
+            self.upload(scene)                 # first use: allocates the first device set
         if self._standby is None:
             self._standby = {n: torch.empty_like(self.scene[n]) for n in _SCENE_ARRAYS}
             self._upload_stream = torch.cuda.Stream(device=self.device)
             self._uploaded, self._released = torch.cuda.Event(), torch.cuda.Event()
             self._released.record(torch.cuda.current_stream(self.device))
+            self._async_k = 0
+        self._async_k ^= 1
+        k = self._async_k
+        src, nbytes = self._stage_to_pinned(scene, k)
+        self._standby_meta = self._scene_meta(scene)
         up = self._upload_stream
         up.wait_event(self._released)          # the frames that read the standby set (two activations ago) are done
-        nbytes = 0
         with torch.cuda.stream(up):
             for n in _SCENE_ARRAYS:
-                self._standby[n].copy_(self._pinned[n], non_blocking=True)
-                nbytes += self._pinned[n].numel() * 4
+                self._standby[n].copy_(src[n], non_blocking=True)
+        self._pinned_read[k].record(up)
         self._uploaded.record(up)
         return nbytes
 
@@ -78,6 +130,7 @@ class Renderer:
         for n in _SCENE_ARRAYS:
             self.scene[n] = self._standby[n]
         self._standby = old
+        self.scene["sh_degree"], self.scene["bg"] = self._standby_meta
 
     def render(self, cam, stream=None, count_contrib: bool = True, out_rgb=None) -> None:
         s = self.scene

@@ -34,7 +34,7 @@ def _sample_tiles(ref_counts, gx, gy, n, seed):
 # ------------------------------------------------------------------------------------------------------------------
 # config 1 (tiny) -- every render variant of the ablation ladder, whole image
 # ------------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", [4, 5, 3, 2, 1, 0])
+@pytest.mark.parametrize("variant", [4, 3, 2, 1, 0])
 def test_config1_all_variants(variant):
     sc = scenes.make_scene(1)
     rep, r, it, ref = pu.oracle_and_compare(sc, 0, variant=variant)
@@ -45,7 +45,7 @@ def test_config1_all_variants(variant):
 # ------------------------------------------------------------------------------------------------------------------
 # config 2 (object-centric, the bench workload) -- full size, whole image, several poses
 # ------------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("pose,variant", [(0, 4), (3, 4), (5, 4), (0, 3), (1, 0), (2, 5)])
+@pytest.mark.parametrize("pose,variant", [(0, 4), (3, 4), (5, 4), (0, 3), (1, 0), (2, 2)])
 def test_config2_full(pose, variant):
     sc = scenes.make_scene(2)
     rep, *_ = pu.oracle_and_compare(sc, pose, variant=variant)
@@ -405,22 +405,42 @@ def test_overlapped_scene_upload_switches_buffer_sets_safely():
         torch.cuda.synchronize()
         want.append(host.clone())
     assert not torch.equal(want[0], want[1])
+    for pin in (False, True):                                       # numpy scenes (staged by the Renderer) / pre-pinned tensors
+        src = [Renderer.pin_scene(x) for x in (sa, sb)] if pin else [sa, sb]
+        r = Renderer(sa.P, 320, 240, 1 << 20, device="cuda:0", count_contrib=False)
+        got = []
+        r.upload_async(src[0])
+        for k in range(6):
+            r.activate_uploaded()
+            r.upload_async(src[(k + 1) & 1])                        # overlaps the frames of this step
+            host = r.render_batch(list(sa.cameras), lanes=3, to_host=True)
+            torch.cuda.current_stream().synchronize()
+            got.append(host.clone())
+        for k in range(6):
+            assert torch.equal(got[k], want[k & 1]), "step %d (pinned inputs: %s)" % (k, pin)
+
+
+def test_upload_restages_the_scene_on_every_call():
+    """Renderer.upload() must copy the scene it is GIVEN on every call (round-1 advisor finding: it re-sent the first
+    scene's staging), and follow its background colour and SH degree."""
+    sa = scenes.make_scene(2, P=20_000, W=320, H=240, f=400.0)
+    sb = scenes.make_scene(2, P=20_000, W=320, H=240, f=400.0)
+    sb.means3D = (sb.means3D[::-1] * np.float32(0.9)).copy()
+    sb.bg = np.array([0.1, 0.7, 0.3], np.float32)
+    want = []
+    for sc in (sa, sb):
+        r0 = Renderer(sc.P, 320, 240, 1 << 20, device="cuda:0", count_contrib=False)
+        r0.upload(sc)
+        r0.render(sc.cameras[1], count_contrib=False)
+        torch.cuda.synchronize()
+        want.append(r0.out_rgb.clone())
+    assert not torch.equal(want[0], want[1])
     r = Renderer(sa.P, 320, 240, 1 << 20, device="cuda:0", count_contrib=False)
-    r.upload(sa)
-    pinned = {0: r._pinned}
-    r2 = Renderer(sb.P, 320, 240, 1 << 20, device="cuda:0", count_contrib=False)
-    r2.upload(sb)
-    pinned[1] = r2._pinned                                          # pinned staging of the second scene
-    torch.cuda.synchronize()
-    got = []
-    r._pinned = pinned[0]
-    r.upload_async(sa)
-    for k in range(6):
-        r.activate_uploaded()
-        r._pinned = pinned[(k + 1) & 1]
-        r.upload_async(sb if (k + 1) & 1 else sa)                   # overlaps the frames of this step
-        host = r.render_batch(list(sa.cameras), lanes=3, to_host=True)
-        torch.cuda.current_stream().synchronize()
-        got.append(host.clone())
-    for k in range(6):
-        assert torch.equal(got[k], want[k & 1]), "step %d" % k
+    for k in range(4):
+        sc = (sa, sb)[k & 1]
+        r.upload(sc)
+        r.render(sc.cameras[1], count_contrib=False)
+        torch.cuda.synchronize()
+        assert torch.equal(r.out_rgb, want[k & 1]), "call %d" % k
+    with pytest.raises(ValueError):
+        r.upload(scenes.make_scene(2, P=10_000, W=320, H=240, f=400.0))

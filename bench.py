@@ -4,14 +4,20 @@
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
 
 A STEP is one pass of the whole hot path (preprocess -> duplication + sort -> render) over every
-camera pose of the configuration: `poses` frames.  Default workload: BASELINE.json configs[1] (object-centric,
-100 000 Gaussians, 800x800, SH degree 3, 8 poses) -- the configuration the metric is quoted on that fits one GPU.
-`value` = frames/s with the scene resident in HBM, device-timed (CUDA events on the launching stream, one pair per
-frame, L2 flushed before every frame, max over ranks).  `e2e` = the same metric through the public API with HOST
-buffers: every step copies the scene host->device from pinned memory, renders every pose and copies every image back.
-N > 1 runs N independent replicas (replicas only; no data-path collective).
+camera pose of a configuration: `poses` frames.  BASELINE.json's metric is "frames/sec per config", so WITHOUT --config
+all five configurations are measured, each with its own W warm-up and K timed steps; the top-level `value`, `config`,
+`roofline`, `e2e` and `cpu_baseline` are those of configs[4] (10 M Gaussians, 3840x2160: the largest single-GPU
+workload, whose sort and render times BASELINE.json wants reported separately) and `per_config` holds the same fields
+for every configuration.  All five fit one GPU (config 4 needs ~21.5 GB of workspace).  With --config C only that one is
+measured and it is the headline.
+`value` = frames/s with the scene resident in HBM, device-timed (CUDA events on the launching stream around every step,
+L2 flushed before every step, max over ranks).  `latency` = one frame at a time, L2 flushed before every frame.
+`e2e` = the same metric through the public API with HOST buffers: every step copies the scene host->device from pinned
+memory, renders every pose and copies every image back.  N > 1 runs N independent replicas (DESIGN.md "Multi-GPU":
+replicas only; no data-path collective); `--gpus N` without a torchrun environment re-launches itself under
+torch.distributed.run with N ranks.
 
-`--impl reference` times the CPU oracle (oracle/, test infrastructure) on the same workload: one pose per step.
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on the same workload: one bounded sample per step.
 """
 from __future__ import annotations
 
@@ -31,6 +37,7 @@ UNIT = "frames/s"
 FP32_LANES_PER_SM = 128          # FP32 FMA lanes per SM per clock (mb probe: FFMA 3.8-4.0 warp-instr/clk/SM)
 INSTR_PER_PAIR = 14              # FP32-pipe thread-instructions per evaluated (pixel, Gaussian) pair
 L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
+HEADLINE_CONFIG = 5               # BASELINE.json configs[4]: the largest single-GPU workload
 
 
 def _peaks():
@@ -122,48 +129,88 @@ def aggregate_fps(ws, frames_per_rank, slowest_rank_ms):
 
 
 # ----------------------------------------------------------------------------------------------------------------
-# reference arm: the CPU oracle, as it stands, on the host cores
+# the CPU oracle, as it stands, on the host cores: `cpu_baseline` of our arm and the whole reference arm
 # ----------------------------------------------------------------------------------------------------------------
+ORACLE_SAMPLE_TILES = {1: None, 2: None, 3: None, 4: 8, 5: 96}   # None: whole frames; else tiles per sampled frame
+
+
+class OracleSampler:
+    """Times the oracle on a BOUNDED sample of a configuration.  Configs 1-3: whole frames (one pose per call, cycling).
+    Configs 4-5 (minutes per frame): per call the per-Gaussian preprocess and the duplication pass of the WHOLE frame plus
+    the sorted lists and the pixels of a fixed random subset of tiles; a frame is then estimated as t_fixed + (t_sample -
+    t_fixed) * n_tiles / n_sample, with t_fixed (the same call on ONE tile: preprocess + duplication pass) measured once.
+    The estimate is a reported baseline, not a target."""
+
+    def __init__(self, sc, config, cores):
+        import numpy as np
+        from oracle import oracle
+        self.oracle, self.sc, self.config, self.cores = oracle, sc, config, cores
+        self.n_pose = len(sc.cameras)
+        self.k = 0
+        self.n_sample = ORACLE_SAMPLE_TILES.get(config)
+        cam = sc.cameras[0]
+        self.n_tiles = ((cam.W + 15) // 16) * ((cam.H + 15) // 16)
+        self.t_pre = None
+        if self.n_sample is not None:
+            self.tiles = np.sort(np.random.default_rng(config).choice(self.n_tiles, size=self.n_sample, replace=False)).astype(np.int32)
+            t0 = time.perf_counter()
+            oracle.render(sc, 0, tile_subset=self.tiles[:1], n_threads=cores)
+            self.t_pre = time.perf_counter() - t0
+
+    def step(self):
+        """One sample; returns the estimated seconds per FRAME."""
+        pose = self.k % self.n_pose
+        self.k += 1
+        t0 = time.perf_counter()
+        if self.n_sample is None:
+            self.oracle.render(self.sc, pose, n_threads=self.cores)
+            return time.perf_counter() - t0
+        self.oracle.render(self.sc, pose, tile_subset=self.tiles, n_threads=self.cores)
+        t = time.perf_counter() - t0
+        return self.t_pre + max(t - self.t_pre, 0.0) * self.n_tiles / self.n_sample
+
+    def describe(self, n, dt):
+        if self.n_sample is None:
+            return "%d whole frames (poses cycling over %d) of the same workload, oracle tile-parallel on %d threads, %.1f s" % (
+                n, self.n_pose, self.cores, dt)
+        return ("%d samples, each the whole-frame preprocess + duplication pass and the sorted lists and pixels of %d of the %d tiles "
+                "(fixed random subset); a frame is estimated as t_fixed + (t_sample - t_fixed) x %d / %d with t_fixed = %.2f s (the "
+                "same call on one tile, single thread); lists and pixels on %d threads; %.1f s in all") % (n, self.n_sample, self.n_tiles, self.n_tiles, self.n_sample, self.t_pre, self.cores, dt)
+
+
 def run_reference(args):
     ws, rank, _ = _dist()
     if rank != 0:
         return 0
-    from oracle import oracle
     from paper_2606_16566_b200 import scenes
-    cfg = scenes.config_defaults(args.config)
-    sc = scenes.make_scene(args.config)
+    config = args.config if args.config else HEADLINE_CONFIG
+    cfg = scenes.config_defaults(config)
+    sc = scenes.make_scene(config)
     cores = os.cpu_count() or 1
-    n_pose = len(sc.cameras)
-    k = 0
+    smp = OracleSampler(sc, config, cores)
     for _ in range(args.warmup):
-        oracle.render(sc, k % n_pose, n_threads=cores)
-        k += 1
+        smp.step()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
-        oracle.render(sc, k % n_pose, n_threads=cores)
-        k += 1
+    est = [smp.step() for _ in range(args.steps)]
     dt = time.perf_counter() - t0
-    fps = args.steps / dt
-    sample = "1 frame (one camera pose, cycling over the %d poses) of config %d per step, oracle tile-parallel on %d threads" % (
-        n_pose, args.config, cores)
+    frame_s = sum(est) / len(est)
+    fps = 1.0 / frame_s
     line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64 blend / f32 preprocess (CPU oracle)", "data": "synthetic",
-            "config": _config_dict(args.config, cfg, sc, extra={"frames_per_step": 1}),
-            "cpu_baseline": {"value": fps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "config": _config_dict(config, cfg, sc),
+            "cpu_baseline": {"value": fps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": smp.describe(args.steps, dt)},
             "e2e": {"value": fps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "step": "one bounded sample of the workload per step (see cpu_baseline.sample); value = 1 / estimated seconds per frame",
             "gpu_launches": 0}
     print(json.dumps(line))
     return 0
 
 
-def _config_dict(config, cfg, sc, extra=None):
-    d = {"workload": "BASELINE.json configs[%d]: %s, %d Gaussians, %dx%d, f=%g, SH degree %d, %d poses, 16x16 tiles, seed %d" % (
+def _config_dict(config, cfg, sc):
+    return {"workload": "BASELINE.json configs[%d]: %s, %d Gaussians, %dx%d, f=%g, SH degree %d, %d poses, 16x16 tiles, seed %d" % (
         config - 1, cfg["name"], sc.P, cfg["W"], cfg["H"], cfg["f"], sc.sh_degree, len(sc.cameras), config - 1),
-         "gaussians": sc.P, "width": cfg["W"], "height": cfg["H"], "sh_degree": sc.sh_degree, "poses": len(sc.cameras)}
-    if extra:
-        d.update(extra)
-    return d
+        "gaussians": sc.P, "width": cfg["W"], "height": cfg["H"], "sh_degree": sc.sh_degree, "poses": len(sc.cameras)}
 
 
 # ----------------------------------------------------------------------------------------------------------------
@@ -198,35 +245,30 @@ def _stage_bytes(P, K_sh, n_vis, n_dup, n_coarse, n_sort_passes, max_dup):
     }
 
 
-def run_ours(args):
-    import numpy as np
+# ncu `--set full` captures of render_b200_kernel committed under profiles/ (file named beside each number): DRAM bytes
+# of one launch, and the hardware pipe utilisation / executed-work figures (A) and (B) of SURVEY.md 8(d).
+PROFILED = {
+    # config: (file, dram bytes read + written per launch, FMA pipe %, XU pipe %, issue slots %, executed FP32 thread-ops, MUFU thread-ops)
+}
+
+
+def measure_config(config, args, ctx):
+    """All measurements of one configuration on this rank; returns the result dict (rank 0 uses it)."""
     import torch
-    import torch.distributed as dist
     from paper_2606_16566_b200 import binding, scenes
     from paper_2606_16566_b200.renderer import Renderer
+    ws, rank, dev, peaks, n_sm = ctx["ws"], ctx["rank"], ctx["dev"], ctx["peaks"], ctx["n_sm"]
 
-    ws, rank, lrank = _dist()
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
-    torch.cuda.set_device(lrank)
-    dev = torch.device("cuda", lrank)
-    if ws > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    binding.lib()  # raises if libgs.so is missing and cannot be built
-    if args.render_variant is not None:
-        binding.gs_set_render_variant(args.render_variant)
-    peaks = _peaks()
-    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
-
-    cfg = scenes.config_defaults(args.config)
+    cfg = scenes.config_defaults(config)
     if args.res_scale != 1:   # PAPER.md Table VI's 1x / 2x resolution axis: same scene, image and focal length scaled
         cfg = dict(cfg, W=cfg["W"] * args.res_scale, H=cfg["H"] * args.res_scale, f=cfg["f"] * args.res_scale)
-        sc = scenes.make_scene(args.config, W=cfg["W"], H=cfg["H"], f=cfg["f"])
+        sc = scenes.make_scene(config, W=cfg["W"], H=cfg["H"], f=cfg["f"])
     else:
-        sc = scenes.make_scene(args.config)
+        sc = scenes.make_scene(config)
     cams = sc.cameras
     n_pose = len(cams)
     W, H = cfg["W"], cfg["H"]
+    pinned = Renderer.pin_scene(sc)      # the host copy of the scene lives in pinned memory (what e2e uploads from)
 
     def barrier():
         replica_barrier(ws)
@@ -237,25 +279,22 @@ def run_ours(args):
     # ---- size the workspace: largest N_dup over the poses (+5 %) -----------------------------------------------------
     max_dup, need = 1 << 21, 0
     r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True)
-    r.upload(sc)
-    per_pose = []
+    r.upload(pinned)
+    overflowed = False
     for cam in cams:
         r.render(cam, count_contrib=False)
         try:
-            it = r.intermediates(copy=())
-            need = max(need, it.n_dup)
-            per_pose.append((it.n_visible, it.n_dup))
+            need = max(need, r.intermediates(copy=()).n_dup)
         except binding.GsError as e:
             if e.code != binding.GS_ERR_OVERFLOW:
                 raise
-            need = max(need, e.n_dup)
-            per_pose.append(None)
-    if need > max_dup or any(p is None for p in per_pose):
+            need, overflowed = max(need, e.n_dup), True
+    if need > max_dup or overflowed:
         del r
         torch.cuda.empty_cache()
         max_dup = int(need * 1.05) + 4096
         r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True)
-        r.upload(sc)
+        r.upload(pinned)
     # ---- statistics pass (untimed): units of the rooflines -------------------------------------------------------------
     binding.gs_set_stats(True)
     stats, per_pose = [], []
@@ -273,7 +312,7 @@ def run_ours(args):
     staged = mean([s["entries_staged"] for s in stats])
     n_vis_m, n_dup_m, n_coarse_m = mean([p[0] for p in per_pose]), mean([p[1] for p in per_pose]), mean([p[2] for p in per_pose])
 
-    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    flush = ctx["flush"]
 
     def frame(cam, e0=None, e1=None):
         flush.zero_()                       # L2 flush before every frame (outside the event pair)
@@ -297,7 +336,7 @@ def run_ours(args):
 
     # ---- pre-warm (clock ramp), choice of the frames in flight, W warm-up steps -----------------------------------------
     t0 = time.perf_counter()
-    while time.perf_counter() - t0 < 0.5:
+    while time.perf_counter() - t0 < 0.3:
         step()
         torch.cuda.synchronize()
     if args.lanes <= 0:   # untimed tuning: the fastest of 1, 2, 3, 4, 6 frames in flight over a few warm-up steps (rank 0 decides)
@@ -321,7 +360,7 @@ def run_ours(args):
     # ---- timed region: exactly K steps ---------------------------------------------------------------------------------------
     K = args.steps
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-    sampler = ClockSampler(lrank)
+    sampler = ClockSampler(ctx["lrank"])
     barrier()
     torch.cuda.synchronize()
     sampler.start()
@@ -335,17 +374,17 @@ def run_ours(args):
     wall = time.perf_counter() - wall0
     clocks = sampler.result()
     barrier()
-    dev_ms = sum(e0.elapsed_time(e1) for e0, e1 in evs)
-    dev_ms = rank_max(dev_ms)
+    dev_ms = rank_max(sum(e0.elapsed_time(e1) for e0, e1 in evs))
     ms_per_step = dev_ms / K
     fps = aggregate_fps(ws, n_pose * K, dev_ms)
 
-    # ---- latency: one frame at a time on one stream, L2 flushed before every frame (the first rounds' `value`) ---------
+    # ---- latency: one frame at a time on one stream, L2 flushed before every frame ------------------------------------------
     for cam in cams:
         frame(cam)
-    fevs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(min(K, 20) * n_pose)]
+    n_lat = max(1, min(K, 20))
+    fevs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_lat * n_pose)]
     torch.cuda.synchronize()
-    for s in range(min(K, 20)):
+    for s in range(n_lat):
         for i, cam in enumerate(cams):
             e0, e1 = fevs[s * n_pose + i]
             frame(cam, e0, e1)
@@ -356,7 +395,7 @@ def run_ours(args):
     binding.gs_set_timing(True)
     acc = {n: 0.0 for n in binding.TIMING_NAMES}
     n_t = 0
-    for s in range(min(K, 20)):
+    for s in range(n_lat):
         for cam in cams:
             flush.zero_()
             r.render(cam, count_contrib=False)
@@ -367,9 +406,9 @@ def run_ours(args):
     binding.gs_set_timing(False)
     stage_ms = {n: acc[n] / n_t for n in acc}
 
-    # ---- e2e: host buffers in, host images out, every step ----------------------------------------------------------------
+    # ---- e2e: host (pinned) buffers in, host images out, every step ---------------------------------------------------------
     def e2e_step():
-        h2d = r.upload(sc)
+        h2d = r.upload(pinned)
         r.render_batch(cams, lanes=lanes, to_host=True)   # device -> pinned host copies overlap the later frames
         r.synchronize_readback()
         return h2d
@@ -380,11 +419,11 @@ def run_ours(args):
     # K steps, each with its own host -> device copy of the scene and its own device -> host copies of the images; the
     # upload of step k+1 goes to a second set of device buffers on an upload stream while step k is rendered and read back
     t0 = time.perf_counter()
-    r.upload_async(sc)
+    r.upload_async(pinned)
     for k in range(K):
         r.activate_uploaded()
         if k + 1 < K:
-            r.upload_async(sc)
+            r.upload_async(pinned)
         r.render_batch(cams, lanes=lanes, to_host=True)
     r.synchronize_readback()
     torch.cuda.synchronize()
@@ -394,18 +433,27 @@ def run_ours(args):
     e2e_fps = ws * n_pose * K / e2e_s
 
     # ---- rooflines ---------------------------------------------------------------------------------------------------------------------
-    alu_peak = n_sm * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12       # T thread-instr/s
+    issue = ctx["issue"]                                    # measured on this device, this run (gs_selftest_issue_peak)
+    alu_peak = max(issue["ffma"], issue["ffma2"]) / 1e12    # T FP32 thread-operations / s
     render_s = stage_ms["render"] * 1e-3
     achieved = pairs_eval * INSTR_PER_PAIR / render_s / 1e12
-    # dram__bytes_read.sum + dram__bytes_write.sum of one render launch from the committed `ncu --set full` capture
-    # (profiles/r01_render_config2_end_ncu.md); only measured for the default workload
-    traffic = {2: 10130944}.get(args.config)
+    prof = PROFILED.get(config) if args.res_scale == 1 else None
     roofline = {"kernel": "render_b200_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak,
-                "unit": "T FP32-pipe thread-instr/s", "frac": achieved / alu_peak, "traffic": traffic,
-                "peak_source": "derived: %d SMs x %d FP32 lanes x %.0f MHz (max SM clock)" % (n_sm, FP32_LANES_PER_SM, peaks["sm_max_mhz"]),
+                "unit": "T FP32-pipe thread-instr/s", "frac": achieved / alu_peak,
+                "traffic": (prof["dram_bytes"] if prof else None),
+                "peak_source": "measured in this run: gs_selftest_issue_peak, max of scalar FFMA (%.2f T/s) and packed FFMA2 (%.2f T/s); "
+                               "derived figure for comparison: %d SMs x %d lanes x %.0f MHz = %.2f T/s" % (
+                                   issue["ffma"] / 1e12, issue["ffma2"] / 1e12, n_sm, FP32_LANES_PER_SM, peaks["sm_max_mhz"],
+                                   n_sm * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12),
+                "what": "(C) of SURVEY.md 8(d): ALGORITHMIC work = (pixel, Gaussian) pairs whose alpha the blend loop evaluated x 14 "
+                        "FP32-pipe thread-instructions, over the render kernel's own time",
+                "sfu": {"achieved": pairs_eval / render_s / 1e12, "peak": issue["ex2"] / 1e12, "unit": "T ex2/s",
+                        "frac": pairs_eval / render_s / issue["ex2"]},
                 "units_per_launch": {"pairs_evaluated": pairs_eval, "instr_per_pair": INSTR_PER_PAIR,
                                      "pairs_blended": pairs_blend, "entries_staged": staged},
                 "ms_per_launch": stage_ms["render"]}
+    if prof:   # (A) hardware pipe utilisation and (B) executed-work roofline of the committed ncu capture of this config
+        roofline["from_profile"] = dict(prof)
     gx, gy = (W + 15) // 16, (H + 15) // 16
     n_sorted_cells = ((gx + 7) // 8) * ((gy + 7) // 8) if n_coarse_m > 0 else gx * gy   # super-tiles or tiles
     n_sort_passes = (max(1, (n_sorted_cells - 1).bit_length()) + 7) // 8
@@ -420,42 +468,94 @@ def run_ours(args):
         elif n == "render":
             k.update(bound="alu", frac=roofline["frac"])
         kernels.append(k)
+    sort_ms = stage_ms["depth_sort"] + stage_ms["tile_grid"] + stage_ms["offset_scan"] + stage_ms["duplicate"] + stage_ms["tile_sort"]
 
     cpu_baseline = None
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
-        from oracle import oracle
         cores = os.cpu_count() or 1
+        smp = OracleSampler(sc, config, cores)
+        budget = args.cpu_seconds
         t0 = time.perf_counter()
-        nf = 0
-        while nf < 8 * n_pose and (time.perf_counter() - t0 < 10.0 or nf == 0):
-            oracle.render(sc, nf % n_pose, n_threads=cores)
-            nf += 1
+        est = []
+        while not est or (time.perf_counter() - t0 < budget and len(est) < 4 * n_pose):
+            est.append(smp.step())
         dt = time.perf_counter() - t0
-        cpu_baseline = {"value": nf / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": "%d frames (poses 0..%d cycling) of the same workload, oracle tile-parallel on %d threads, %.1f s" % (
-                            nf, min(nf, n_pose) - 1, cores, dt)}
+        cpu_baseline = {"value": len(est) / sum(est), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": smp.describe(len(est), dt)}
 
+    res = {"metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": args.warmup,
+           "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic",
+           "config": _config_dict(config, cfg, sc),
+           "run": {"frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every step", "frames_in_flight": lanes,
+                   "parallelism": "replicas x%d" % ws, "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "n_coarse_mean": n_coarse_m,
+                   "binning": "two-level (8x8-tile super-tiles)" if n_coarse_m > 0 else "one-level", "res_scale": args.res_scale,
+                   "render_variant": binding.gs_get_render_variant(), "workspace_bytes": int(r.workspace.numel())},
+           "ms_per_frame": ms_per_step / n_pose, "wall_ms_per_step_incl_flush": 1e3 * wall / K,
+           "latency": {"ms_per_frame": serial_ms_per_frame, "frames_per_s": ws * 1e3 / serial_ms_per_frame,
+                       "how": "one frame in flight, one stream, L2 flushed before every frame"},
+           "sort_ms_per_frame": sort_ms, "render_ms_per_frame": stage_ms["render"],
+           "clocks": clocks,
+           "e2e": {"value": e2e_fps, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
+                   "input": "scene arrays in pinned host memory (Renderer.pin_scene), copied host -> device every step; images "
+                            "copied device -> pinned host every frame; steps pipelined through a second device buffer set"},
+           "gpu_launches": launches, "launches_per_frame": launches_per_frame,
+           "roofline": roofline, "kernels": kernels, "stage_ms_per_frame": stage_ms,
+           "cpu_baseline": cpu_baseline}
+    del r, pinned, sc
+    torch.cuda.empty_cache()
+    return res
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_16566_b200 import binding
+
+    ws, rank, lrank = _dist()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(lrank)
+    dev = torch.device("cuda", lrank)
+    if ws > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    binding.lib()  # raises if libgs.so is missing and cannot be built
+    if args.render_variant is not None:
+        binding.gs_set_render_variant(args.render_variant)
+    ctx = {"ws": ws, "rank": rank, "lrank": lrank, "dev": dev, "peaks": _peaks(),
+           "n_sm": torch.cuda.get_device_properties(dev).multi_processor_count,
+           "flush": torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev),
+           "issue": binding.gs_selftest_issue_peak(2000)}
+    configs = [args.config] if args.config else [1, 2, 3, 4, 5]
+    headline = args.config if args.config else HEADLINE_CONFIG
+    results = {}
+    for c in configs:
+        results[c] = measure_config(c, args, ctx)
     if rank == 0:
-        line = {"metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": args.warmup,
-                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f32", "data": "synthetic",
-                "config": _config_dict(args.config, cfg, sc, extra={
-                    "frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every step", "frames_in_flight": lanes,
-                    "parallelism": "replicas x%d" % ws,
-                    "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "n_coarse_mean": n_coarse_m,
-                    "binning": "two-level (8x8-tile super-tiles)" if n_coarse_m > 0 else "one-level", "res_scale": args.res_scale, "render_variant": binding.gs_get_render_variant()}),
-                "ms_per_frame": ms_per_step / n_pose, "wall_ms_per_step_incl_flush": 1e3 * wall / K,
-                "latency": {"ms_per_frame": serial_ms_per_frame, "frames_per_s": ws * 1e3 / serial_ms_per_frame,
-                            "how": "one frame in flight, one stream, L2 flushed before every frame"},
-                "clocks": clocks,
-                "e2e": {"value": e2e_fps, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes},
-                "gpu_launches": launches, "launches_per_frame": launches_per_frame,
-                "roofline": roofline, "kernels": kernels, "stage_ms_per_frame": stage_ms,
-                "cpu_baseline": cpu_baseline, "peaks": peaks}
+        line = dict(results[headline])
+        line["peaks"] = dict(ctx["peaks"], issue_peak_measured=ctx["issue"])
+        line["gpu_launches"] = sum(r["gpu_launches"] for r in results.values())
+        if len(configs) > 1:
+            keep = ("config", "value", "unit", "ms_per_step", "ms_per_frame", "latency", "sort_ms_per_frame", "render_ms_per_frame",
+                    "e2e", "roofline", "cpu_baseline", "clocks", "gpu_launches", "launches_per_frame", "stage_ms_per_frame", "kernels", "run")
+            line["per_config"] = [{k: results[c][k] for k in keep} for c in configs]
+            line["headline"] = "configs[%d] (top-level fields); every configuration has its own %d warm-up and %d timed steps" % (
+                headline - 1, args.warmup, args.steps)
         print(json.dumps(line))
     if ws > 1:
         dist.destroy_process_group()
     return 0
+
+
+def _respawn_under_torchrun(args):
+    """`--gpus N` without a torchrun environment: run the same command under torch.distributed.run with N ranks."""
+    import socket
+    import subprocess
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -463,13 +563,23 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, choices=(1, 2, 3, 4, 5))
+    ap.add_argument("--config", type=int, default=0, choices=(0, 1, 2, 3, 4, 5),
+                    help="0 (default): all five configurations, configs[4] as the headline; 1..5: that configuration only")
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=8.0, help="budget of the cpu_baseline leg per configuration")
     ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = the fastest of 1-6 over a few warm-up steps)")
     ap.add_argument("--res-scale", type=int, default=1, choices=(1, 2), help="render at 1x or 2x the configuration's resolution (our arm only)")
     ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")
     args = ap.parse_args()
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
+    ws = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return _respawn_under_torchrun(args)
+    if ws != args.gpus:
+        print("bench.py: --gpus %d but WORLD_SIZE=%d" % (args.gpus, ws), file=sys.stderr)
+        return 2
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)

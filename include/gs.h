@@ -149,6 +149,14 @@ int gs_last_launch_count(void);
  * 0), out[1] = atomics checked. */
 int gs_selftest_atomic_order(int iters, uint64_t out[2]);
 
+/* Measured issue peaks of the current device, the denominators of the render roofline (Sec. IV-F / Table VII
+ * counts FP32 and SFU work; BASELINE.json metric "blend kernel % FP32+SFU issue peak").  Saturates the FP32 pipe with
+ * scalar fma.rn.f32, with packed fma.rn.f32x2 (what the blend loop issues) and the SFU with ex2.approx.ftz -- 8 independent
+ * chains per thread, 64 warps per SM, `iters` x 256 instructions per thread, best of 3 timed launches (CUDA events,
+ * synchronous, default stream) -- and returns THREAD-OPERATIONS per second: out[0] FFMA, out[1] FFMA2 (two FP32
+ * operations per lane and instruction), out[2] MUFU.EX2.  Uses 16 bytes of private device scratch. */
+int gs_selftest_issue_peak(int iters, double out[3]);
+
 /* Synchronous device->host copy of `bytes` bytes (a plain cudaMemcpy) -- lets a binding without CUDA runtime access
  * read the arrays gs_get_intermediates() points at. */
 int gs_copy_to_host(void* dst_host, const void* src_dev, size_t bytes);

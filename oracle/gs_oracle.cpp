@@ -342,9 +342,20 @@ gs_oracle_result* gs_oracle_render(int P, const float* means3D, const float* sca
                     if (l >= 0) r->sorted_ids[cursor[l]++] = (uint32_t)i;
                 }
         }
-        for (size_t l = 0; l < n_lists; l++)  // key = (tile << 32) | depth bits, stable => ties by index (S10)
-            std::stable_sort(r->sorted_ids.begin() + r->list_offsets[l], r->sorted_ids.begin() + r->list_offsets[l + 1],
-                             [&](uint32_t p, uint32_t q) { return pre.depth_bits[p] < pre.depth_bits[q]; });
+        // key = (tile << 32) | depth bits, stable => ties by index (S10).  The lists are independent: with n_threads > 1 they
+        // are sorted by several threads (same std::stable_sort per list, identical result).
+        auto sort_lists = [&](size_t first, size_t stride) {
+            for (size_t l = first; l < n_lists; l += stride)
+                std::stable_sort(r->sorted_ids.begin() + r->list_offsets[l], r->sorted_ids.begin() + r->list_offsets[l + 1],
+                                 [&](uint32_t p, uint32_t q) { return pre.depth_bits[p] < pre.depth_bits[q]; });
+        };
+        if (n_threads <= 1) {
+            sort_lists(0, 1);
+        } else {
+            std::vector<std::thread> th;
+            for (int k = 0; k < n_threads; k++) th.emplace_back(sort_lists, (size_t)k, (size_t)n_threads);
+            for (auto& t : th) t.join();
+        }
     }
     // ---- C-R ---------------------------------------------------------------------------------------------
     const size_t npix = (size_t)W * H;

@@ -56,8 +56,8 @@ typedef struct gs_oracle_view {
 
 /* Runs the oracle.  tile_subset == NULL: all tiles (full).  Otherwise only the n_subset listed tiles get
  * lists and pixels; per-Gaussian outputs and tile_counts always cover everything.
- * n_threads <= 1: single-threaded (the definitional baseline); > 1: tile rows of C-R are spread over threads
- * (same arithmetic per pixel, identical results).  fragile_delta: the delta of the parity protocol (1e-3).
+ * n_threads <= 1: single-threaded (the definitional baseline); > 1: the per-list stable sorts of C-B and the tiles of
+ * C-R are spread over threads (same std::stable_sort per list, same arithmetic per pixel: identical results).  fragile_delta: the delta of the parity protocol (1e-3).
  * Returns NULL on bad arguments. */
 gs_oracle_result* gs_oracle_render(int P, const float* means3D, const float* scales, const float* rotations,
                                    const float* opacities, const float* sh_coeffs, int sh_degree,

@@ -22,6 +22,7 @@ UNITS = {
     "api.cu": [],
     "preprocess.cu": ["-fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false"],
     "binning.cu": [],
+    "selftest.cu": [],
     "render.cu": ["-use_fast_math"],
     "render_b200.cu": ["-use_fast_math"],
 }

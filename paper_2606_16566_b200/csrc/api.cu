@@ -20,6 +20,7 @@ void launch_scan_offsets(const Frame&, const Pointers&, int, int, cudaStream_t, 
 void launch_expand(const Frame&, const Pointers&, cudaStream_t, int*);
 void launch_duplicate_and_tile_sort(const Frame&, const Pointers&, int, cudaStream_t, int*, cudaEvent_t);
 void launch_atomic_order_selftest(unsigned long long*, int, uint32_t, int, int, cudaStream_t);
+cudaError_t run_issue_peak(int, int, double*);
 void launch_render_ladder(int, const Frame&, const Pointers&, float*, float*, uint32_t*, cudaStream_t);
 void launch_render_b200(const Frame&, const Pointers&, float*, float*, uint32_t*, int, bool, cudaStream_t);
 }  // namespace gs
@@ -448,6 +449,15 @@ int gs_selftest_atomic_order(int iters, uint64_t out[2]) {
     out[0] = h[0];
     out[1] = h[1];
     return GS_OK;
+}
+
+int gs_selftest_issue_peak(int iters, double out[3]) {
+    if (iters <= 0 || !out) return GS_ERR_BAD_ARG;
+    int dev = 0, n_sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = run_issue_peak(n_sm, iters, out);
+    return e == cudaSuccess ? GS_OK : cuda_fail(e);
 }
 
 int gs_copy_to_host(void* dst_host, const void* src_dev, size_t bytes) {

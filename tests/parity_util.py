@@ -74,7 +74,11 @@ def compare(r, it, ref, check_lists=True, check_pixels=True):
     ranges = it.tile_ranges.astype(np.uint64)
     assert ranges[0] == 0 and np.array_equal(np.diff(ranges), ref.tile_counts.astype(np.uint64)), "tile ranges differ"
     rep.update(P=int(it.P), n_visible=int(it.n_visible), n_dup=int(it.n_dup))
-    if check_lists:
+    if check_lists and ref.full:   # every list: the concatenation IS the sorted id array (ranges already compared)
+        assert it.sorted_ids.shape == ref.sorted_ids.shape and np.array_equal(it.sorted_ids, ref.sorted_ids), \
+            "sorted id array differs (first at %s)" % (np.flatnonzero(it.sorted_ids != ref.sorted_ids)[:5],)
+        rep["lists_checked"] = int(len(ref.list_tile))
+    elif check_lists:
         n_bad = 0
         for l, t in enumerate(ref.list_tile):
             a = it.sorted_ids[int(ranges[t]):int(ranges[t + 1])]
@@ -110,6 +114,8 @@ def compare(r, it, ref, check_lists=True, check_pixels=True):
     assert d.max() <= TOL_ALL, "max |diff| %.3g > 2/255 at %s" % (d.max(), np.unravel_index(d.argmax(), d.shape))
     assert over.sum() <= (1.0 - FRAC_MOST) * npx, "%d of %d pixels above 2e-3" % (over.sum(), npx)
     assert (over & ~fragile).sum() == 0, "%d NON-fragile pixels above 2e-3" % (over & ~fragile).sum()
+    # the classifier that forgives mismatches must stay what SURVEY.md 8(c) estimates (~3 % of the pixels at delta = 1e-3)
+    assert (fragile & pmask).sum() <= 0.05 * max(npx, 1) + 8, "fragile share %.3f > 5 %%" % ((fragile & pmask).sum() / max(npx, 1))
     rep.update(pixels=npx, fragile_share=float((fragile & pmask).sum()) / max(npx, 1), max_abs_diff=float(d.max()),
                over_2e3=int(over.sum()), p999_abs_diff=float(np.quantile(d[pmask], 0.999)) if npx else 0.0,
                mean_abs_diff=float(d[pmask].mean()) if npx else 0.0)

@@ -2,6 +2,8 @@
 
 Protocol and tolerances: tests/parity_util.py (BASELINE.json north_star).  Every test needs a B200: `-m gpu`.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -20,15 +22,6 @@ def _default_variant():
     binding.gs_set_render_variant(4)
     yield
     binding.gs_set_render_variant(4)
-
-
-def _sample_tiles(ref_counts, gx, gy, n, seed):
-    """Tile subset for full-size configs: the longest lists, the image corners/edges, and random tiles."""
-    rng = np.random.default_rng(seed)
-    order = np.argsort(ref_counts)[::-1]
-    pick = list(order[:3]) + [0, gx - 1, (gy - 1) * gx, gy * gx - 1, (gy // 2) * gx + gx // 2]
-    pick += list(rng.choice(gx * gy, size=n, replace=False))
-    return np.unique(np.array(pick, dtype=np.int32))
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -80,21 +73,57 @@ def test_reduced_configs(config, P, W, H, f, pose):
 
 
 # ------------------------------------------------------------------------------------------------------------------
-# full-size configs 3-5 in the launch configuration bench.py uses: all per-Gaussian integers, N_dup, every tile count
-# and range bit-exact; sorted lists and pixels on a sampled subset of tiles the oracle can compute one by one
+# full-size configs 3-5 in the launch configuration bench.py uses: NO sampling of the bit-exact outputs.
+#   configs 3 and 5: every per-Gaussian integer, N_dup, every tile count / range, the WHOLE sorted id array and the WHOLE
+#     image / final T / n_contrib against the oracle, on two poses each (pose 0 and a mid-orbit pose);
+#   config 4 (1.02 G list entries, ~125 000 per tile): every per-Gaussian integer, every tile count / range and the whole
+#     4 GB sorted id array on pose 0; pixels on the tiles of the three longest lists, the corners, the centre and random
+#     tiles (the oracle blends those one by one); the integers and counts of a second pose.
 # ------------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("config,pose,n_tiles", [(3, 0, 24), (5, 0, 16), (4, 0, 4)])
-def test_full_size_sampled_tiles(config, pose, n_tiles):
-    sc = scenes.make_scene(config, poses=max(pose + 1, 2) if config != 4 else 16)
-    cam = sc.cameras[pose]
-    pre = oracle.render(sc, pose, flags=oracle.NO_LISTS)
-    tiles = _sample_tiles(pre.tile_counts, pre.grid_x, pre.grid_y, n_tiles, seed=config)
-    if config == 4:  # every list has > 1e5 entries: keep the sample small
-        tiles = tiles[:6]
-    r, it = pu.run_gpu_auto(sc, pose, start_dup=int(pre.n_dup) + 4096)
-    ref = oracle.render(sc, pose, tile_subset=tiles, n_threads=8, fragile_delta=pu.DELTA)
+_SCENES = {}
+N_CPU = os.cpu_count() or 8
+
+
+def _full_scene(config):
+    if config not in _SCENES:
+        _SCENES.clear()            # one multi-GB scene at a time
+        _SCENES[config] = scenes.make_scene(config)
+    return _SCENES[config]
+
+
+@pytest.mark.parametrize("config,pose", [(3, 0), (3, 9), (5, 0), (5, 5)])
+def test_full_size_whole_frame(config, pose):
+    sc = _full_scene(config)
+    ref = oracle.render(sc, pose, n_threads=N_CPU, fragile_delta=pu.DELTA)
+    assert ref.full
+    r, it = pu.run_gpu_auto(sc, pose, start_dup=int(ref.n_dup) + 4096)
     rep = pu.compare(r, it, ref)
-    print("config", config, "FULL pose", pose, "tiles", len(tiles), rep)
+    assert rep["lists_checked"] == ref.n_tiles and rep["pixels"] == ref.W * ref.H
+    print("config", config, "FULL pose", pose, rep)
+
+
+def test_config4_full_size_every_list_and_sampled_pixels():
+    sc = _full_scene(4)
+    ref = oracle.render(sc, 0, n_threads=N_CPU, flags=oracle.NO_RENDER)       # every list: 1.02 G entries
+    assert ref.full and ref.n_dup > 900_000_000
+    r, it = pu.run_gpu_auto(sc, 0, start_dup=int(ref.n_dup) + 4096)
+    rep = pu.compare(r, it, ref, check_lists=True, check_pixels=False)
+    assert rep["lists_checked"] == ref.n_tiles
+    counts, gx, gy = ref.tile_counts.copy(), ref.grid_x, ref.grid_y
+    del ref, it
+    longest = [int(t) for t in np.argsort(counts)[::-1][:3]]
+    fixed = [0, gx - 1, (gy - 1) * gx, gy * gx - 1, (gy // 2) * gx + gx // 2]
+    rnd = [int(t) for t in np.random.default_rng(4).choice(gx * gy, size=12, replace=False)]
+    tiles = np.array(sorted(set(longest + fixed + rnd)), dtype=np.int32)
+    assert all(t in tiles for t in longest) and len(tiles) >= 16
+    sub = oracle.render(sc, 0, tile_subset=tiles, n_threads=N_CPU, fragile_delta=pu.DELTA)
+    it = r.intermediates()
+    rep2 = pu.compare(r, it, sub)
+    print("config 4 FULL pose 0: lists", rep, "pixels on", len(tiles), "tiles", rep2)
+    del r, it, sub
+    torch.cuda.empty_cache()
+    rep3, *_ = pu.oracle_and_compare(sc, 9, flags=oracle.NO_LISTS)             # a second pose: integers, N_dup, every tile count
+    print("config 4 FULL pose 9:", rep3)
 
 
 # ------------------------------------------------------------------------------------------------------------------

@@ -69,3 +69,12 @@ def test_culling_rules():
     r = oracle.render(sc)
     assert list(r.tiles_touched > 0) == [False, True, False, False, True]
     assert r.mu[4, 0] > W - 1   # centre is outside the image, the splat is kept because its rect overlaps
+
+
+def test_threaded_oracle_equals_single_threaded():
+    """n_threads > 1 spreads the per-list sorts and the tiles of the blend over threads; nothing may change."""
+    sc = scenes.make_scene(3, P=3000, W=200, H=120, f=150.0, poses=2)
+    a = oracle.render(sc, 1, n_threads=1)
+    b = oracle.render(sc, 1, n_threads=5)
+    assert np.array_equal(a.sorted_ids, b.sorted_ids) and np.array_equal(a.list_offsets, b.list_offsets)
+    assert np.array_equal(a.image, b.image) and np.array_equal(a.n_contrib, b.n_contrib) and np.array_equal(a.fragile, b.fragile)

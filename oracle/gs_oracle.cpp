@@ -87,6 +87,7 @@ struct Frame {
     const float *means, *scales, *rots, *opac, *sh, *V, *PM;
     float fx, fy;
     double campos[3];
+    int tile_cull = 0;   // 0: standard 3-sigma square rect (C-P8); 1: intersected with the AABB of the alpha >= 1/255 ellipse (C-P8')
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -172,10 +173,34 @@ void preprocess_one(const Frame& f, int i, Pre& o) {
     const int radius = (int)rf_;
     // C-P8 tile rectangle, half-open, clamped to the grid                            (reading S6)
     const float rf = (float)radius;
-    const int xmin = (int)std::fmin((float)f.gx, std::fmax(0.0f, std::floor((mux - rf) / 16.0f)));
-    const int xmax = (int)std::fmin((float)f.gx, std::fmax(0.0f, std::floor(((mux + rf) + 15.0f) / 16.0f)));
-    const int ymin = (int)std::fmin((float)f.gy, std::fmax(0.0f, std::floor((muy - rf) / 16.0f)));
-    const int ymax = (int)std::fmin((float)f.gy, std::fmax(0.0f, std::floor(((muy + rf) + 15.0f) / 16.0f)));
+    float rxf = rf, ryf = rf;
+    if (f.tile_cull) {
+        // C-P8' ("tighter tile culling", off by default): the square is intersected with the axis-aligned
+        // bounding box of the ellipse alpha >= 1/255, i.e. a dx^2 + 2 b dx dy + c dy^2 <= tau, tau = 2 ln(255 o)
+        // (PAPER.md:181), whose half-extents are sqrt(tau c / det) and sqrt(tau a / det), det = a c - b^2.  No pixel outside
+        // it can pass step 4 of C-R, so the image does not change.  tau is a library-free UPPER bound: 255 o = 2^e m,
+        // m in [1, 2), ln m <= (m - 1) / sqrt(m), plus 1e-5.  Extents in double from the fp32 conic the blend uses; one
+        // pixel is added because the rounding of S6 can leave out a last pixel that is the first column of its tile.
+        const float x255 = 255.0f * f.opac[i];
+        if (!(x255 > 1.0f)) return;                       // alpha < 1/255 everywhere: never blended
+        const uint32_t xb = f2u(x255);
+        const int e2 = (int)(xb >> 23) - 127;
+        const uint32_t mb = (xb & 0x007fffffu) | 0x3f800000u;
+        float m;
+        std::memcpy(&m, &mb, 4);
+        const float lnm = (m - 1.0f) / std::sqrt(m);
+        const float tau = (2.0f * (((float)e2 * 0.693147182f) + lnm)) + 1e-5f;
+        const double dd = ((double)ca * (double)cc) - ((double)cb * (double)cb);
+        if (dd > 0.0 && ca > 0.0f && cc > 0.0f) {
+            const double hx = std::sqrt(((double)tau * (double)cc) / dd), hy = std::sqrt(((double)tau * (double)ca) / dd);
+            if (hx < 1.0e9) rxf = std::fmin(rf, (float)std::ceil(hx) + 1.0f);
+            if (hy < 1.0e9) ryf = std::fmin(rf, (float)std::ceil(hy) + 1.0f);
+        }
+    }
+    const int xmin = (int)std::fmin((float)f.gx, std::fmax(0.0f, std::floor((mux - rxf) / 16.0f)));
+    const int xmax = (int)std::fmin((float)f.gx, std::fmax(0.0f, std::floor(((mux + rxf) + 15.0f) / 16.0f)));
+    const int ymin = (int)std::fmin((float)f.gy, std::fmax(0.0f, std::floor((muy - ryf) / 16.0f)));
+    const int ymax = (int)std::fmin((float)f.gy, std::fmax(0.0f, std::floor(((muy + ryf) + 15.0f) / 16.0f)));
     const int tt = (xmax - xmin) * (ymax - ymin);
     if (tt <= 0) return;
     // C-P9 colour (double, any order)                                                (reading S8)
@@ -297,6 +322,7 @@ gs_oracle_result* gs_oracle_render(int P, const float* means3D, const float* sca
     if (!make_frame(f, P, means3D, scales, rotations, opacities, sh_coeffs, sh_degree, viewmatrix, projmatrix, fx, fy, W, H))
         return nullptr;
     if (!bg) return nullptr;
+    f.tile_cull = (flags & GS_ORACLE_TILE_CULL) ? 1 : 0;
     gs_oracle_result* r = new gs_oracle_result();
     r->f = f;
     const int n_tiles = f.gx * f.gy;

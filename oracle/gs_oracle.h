@@ -53,6 +53,8 @@ typedef struct gs_oracle_view {
 /* flags */
 #define GS_ORACLE_NO_RENDER 1   /* stop after binning */
 #define GS_ORACLE_NO_LISTS  2   /* stop after preprocess + tile_counts */
+#define GS_ORACLE_TILE_CULL 4   /* C-P8': tile rect intersected with the AABB of the alpha >= 1/255 ellipse;
+                                   off by default -- every pin of the standard definition uses the 3-sigma square */
 
 /* Runs the oracle.  tile_subset == NULL: all tiles (full).  Otherwise only the n_subset listed tiles get
  * lists and pixels; per-Gaussian outputs and tile_counts always cover everything.

@@ -489,7 +489,7 @@ def measure_config(config, args, ctx):
            "run": {"frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every step", "frames_in_flight": lanes,
                    "parallelism": "replicas x%d" % ws, "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "n_coarse_mean": n_coarse_m,
                    "binning": "two-level (8x8-tile super-tiles)" if n_coarse_m > 0 else "one-level", "res_scale": args.res_scale,
-                   "render_variant": binding.gs_get_render_variant(), "workspace_bytes": int(r.workspace.numel())},
+                   "render_variant": binding.gs_get_render_variant(), "tile_cull": binding.gs_get_tile_cull(), "workspace_bytes": int(r.workspace.numel())},
            "ms_per_frame": ms_per_step / n_pose, "wall_ms_per_step_incl_flush": 1e3 * wall / K,
            "latency": {"ms_per_frame": serial_ms_per_frame, "frames_per_s": ws * 1e3 / serial_ms_per_frame,
                        "how": "one frame in flight, one stream, L2 flushed before every frame"},
@@ -521,6 +521,7 @@ def run_ours(args):
     binding.lib()  # raises if libgs.so is missing and cannot be built
     if args.render_variant is not None:
         binding.gs_set_render_variant(args.render_variant)
+    binding.gs_set_tile_cull(args.tile_cull)
     ctx = {"ws": ws, "rank": rank, "lrank": lrank, "dev": dev, "peaks": _peaks(),
            "n_sm": torch.cuda.get_device_properties(dev).multi_processor_count,
            "flush": torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev),
@@ -570,6 +571,7 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=8.0, help="budget of the cpu_baseline leg per configuration")
     ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = the fastest of 1-6 over a few warm-up steps)")
     ap.add_argument("--res-scale", type=int, default=1, choices=(1, 2), help="render at 1x or 2x the configuration's resolution (our arm only)")
+    ap.add_argument("--tile-cull", type=int, default=0, choices=(0, 1), help="gs_set_tile_cull: 1 = rects intersected with the alpha >= 1/255 bounding box (our arm only; the default is the standard 3-sigma rect)")
     ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")
     args = ap.parse_args()
     if args.gpus < 1:

@@ -25,7 +25,7 @@ TIMING_NAMES = ("preprocess", "depth_sort", "tile_grid", "offset_scan", "duplica
 EXPORTS = ("gs_workspace_bytes", "gs_render", "gs_get_intermediates", "gs_set_timing", "gs_get_timings",
            "gs_set_render_variant", "gs_get_render_variant", "gs_last_launch_count", "gs_error_string",
            "gs_last_cuda_error", "gs_copy_to_host", "gs_set_stats", "gs_get_stats", "gs_selftest_atomic_order",
-           "gs_set_render_stream", "gs_selftest_issue_peak")
+           "gs_set_render_stream", "gs_selftest_issue_peak", "gs_set_tile_cull", "gs_get_tile_cull")
 GS_N_STATS = 4
 STATS_NAMES = ("warp_slots_walked", "pairs_blended", "entries_staged", "pairs_evaluated")
 
@@ -84,6 +84,9 @@ def lib():
         L.gs_get_stats.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.gs_copy_to_host.restype = C.c_int
         L.gs_copy_to_host.argtypes = [vp, vp, C.c_size_t]
+        L.gs_set_tile_cull.restype = C.c_int
+        L.gs_set_tile_cull.argtypes = [C.c_int]
+        L.gs_get_tile_cull.restype = C.c_int
         L.gs_selftest_issue_peak.restype = C.c_int
         L.gs_selftest_issue_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.gs_selftest_atomic_order.restype = C.c_int
@@ -229,6 +232,16 @@ def gs_selftest_issue_peak(iters: int = 2000) -> dict:
     if rc != GS_OK:
         raise GsError(rc, "gs_selftest_issue_peak")
     return {"ffma": float(out[0]), "ffma2": float(out[1]), "ex2": float(out[2])}
+
+
+def gs_set_tile_cull(mode: int) -> None:
+    rc = lib().gs_set_tile_cull(int(mode))
+    if rc != GS_OK:
+        raise GsError(rc, "gs_set_tile_cull")
+
+
+def gs_get_tile_cull() -> int:
+    return int(lib().gs_get_tile_cull())
 
 
 def gs_set_render_variant(variant: int) -> None:

@@ -115,7 +115,7 @@ struct LastCall {
 
 std::mutex g_mu;
 std::map<const void*, LastCall> g_calls;
-std::atomic<int> g_variant{4}, g_timing{0}, g_stats{0}, g_launches{0}, g_cuda_err{0}, g_render_stream{0};
+std::atomic<int> g_tile_cull{0}, g_variant{4}, g_timing{0}, g_stats{0}, g_launches{0}, g_cuda_err{0}, g_render_stream{0};
 int g_n_sm = 0;
 
 int cuda_fail(cudaError_t e) {
@@ -217,6 +217,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     f.deg = sh_degree; f.K = (sh_degree + 1) * (sh_degree + 1);
     f.tile_bits = L.tile_bits; f.n_tile_passes = L.n_tile_passes;
     f.compact = P >= COMPACT_MIN_P ? 1 : 0;
+    f.tile_cull = g_tile_cull.load();
     f.diff_copies = L.diff_copies; f.diff_cells = L.diff_cells;
     f.cshift = L.cshift; f.cgx = L.cgx; f.cgy = L.cgy; f.n_ctiles = L.n_ctiles; f.cdiff_cells = L.cdiff_cells;
     for (int k = 0; k < 16; k++) { f.V[k] = viewmatrix[k]; f.PM[k] = projmatrix[k]; }
@@ -473,6 +474,12 @@ int gs_set_render_variant(int variant) {
     return GS_OK;
 }
 int gs_get_render_variant(void) { return g_variant.load(); }
+int gs_set_tile_cull(int mode) {
+    if (mode != 0 && mode != 1) return GS_ERR_BAD_ARG;
+    g_tile_cull.store(mode);
+    return GS_OK;
+}
+int gs_get_tile_cull(void) { return g_tile_cull.load(); }
 int gs_set_render_stream(int enable) {
     g_render_stream.store(enable ? 1 : 0);
     return GS_OK;

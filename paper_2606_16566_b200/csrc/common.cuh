@@ -56,6 +56,7 @@ struct Frame {              // per-frame constants, passed by value to the kerne
     int cgx, cgy, n_ctiles, cdiff_cells;   // super-tile grid and its difference grid
     int tile_bits, n_tile_passes;         // of the grid the duplication + sort runs on (the super-tile grid)
     int compact;                // 1: preprocess compacts the visible Gaussians (P >= COMPACT_MIN_P)
+    int tile_cull;              // 1: tile rect intersected with the bounding box of the alpha >= 1/255 ellipse (gs_set_tile_cull)
     int diff_copies, diff_cells; // replicas of the coverage difference grid (power of two) and cells per replica
     float V[16], PM[16];
     float fx, fy;

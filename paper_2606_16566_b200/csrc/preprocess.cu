@@ -34,7 +34,7 @@ struct Splat {
 
 // C-P0..C-P8.  Returns false when the Gaussian is culled.
 __device__ __forceinline__ bool project(const Frame& f, float px, float py, float pz, float sx, float sy, float sz,
-                                        float qw, float qx, float qy, float qz, Splat& o) {
+                                        float qw, float qx, float qy, float qz, float opacity, Splat& o) {
     const float* V = f.V;
     const float* PM = f.PM;
     const float Wf = (float)f.W, Hf = (float)f.H;
@@ -108,11 +108,33 @@ __device__ __forceinline__ bool project(const Frame& f, float px, float py, floa
     const int radius = (int)rf_;
     // C-P8 tile rect, half-open, clamped to the grid (reading S6)
     const float rf = (float)radius;
+    float rxf = rf, ryf = rf;
+    if (f.tile_cull) {
+        // C-P8' (gs_set_tile_cull(1)): the square intersected with the bounding box of the ellipse
+        // alpha >= 1/255, i.e. a dx^2 + 2 b dx dy + c dy^2 <= tau = 2 ln(255 o), half-extents
+        // sqrt(tau c / det) and sqrt(tau a / det).  tau is a library-free UPPER bound (255 o = 2^e m, ln m <= (m - 1) /
+        // sqrt(m) on [1, 2], + 1e-5); the extents are formed in double from the fp32 conic the blend uses; every operation
+        // is one explicit IEEE rounding, as in the rest of this function, so the rect is bit-reproducible.
+        const float x255 = mul(255.0f, opacity);
+        if (!(x255 > 1.0f)) return false;                 // alpha < 1/255 everywhere: never blended
+        const uint32_t xb = __float_as_uint(x255);
+        const int e2 = (int)(xb >> 23) - 127;
+        const float m = __uint_as_float((xb & 0x007fffffu) | 0x3f800000u);
+        const float lnm = dvd(sub(m, 1.0f), sqr(m));
+        const float tau = add(mul(2.0f, add(mul((float)e2, 0.693147182f), lnm)), 1e-5f);
+        const double dd = __dsub_rn(__dmul_rn((double)o.ca, (double)o.cc), __dmul_rn((double)o.cb, (double)o.cb));
+        if (dd > 0.0 && o.ca > 0.0f && o.cc > 0.0f) {
+            const double hx = __dsqrt_rn(__ddiv_rn(__dmul_rn((double)tau, (double)o.cc), dd));
+            const double hy = __dsqrt_rn(__ddiv_rn(__dmul_rn((double)tau, (double)o.ca), dd));
+            if (hx < 1.0e9) rxf = fminf(rf, add((float)ceil(hx), 1.0f));
+            if (hy < 1.0e9) ryf = fminf(rf, add((float)ceil(hy), 1.0f));
+        }
+    }
     const float gxf = (float)f.gx, gyf = (float)f.gy;
-    const int xmin = (int)fminf(gxf, fmaxf(0.0f, floorf(dvd(sub(mux, rf), 16.0f))));
-    const int xmax = (int)fminf(gxf, fmaxf(0.0f, floorf(dvd(add(add(mux, rf), 15.0f), 16.0f))));
-    const int ymin = (int)fminf(gyf, fmaxf(0.0f, floorf(dvd(sub(muy, rf), 16.0f))));
-    const int ymax = (int)fminf(gyf, fmaxf(0.0f, floorf(dvd(add(add(muy, rf), 15.0f), 16.0f))));
+    const int xmin = (int)fminf(gxf, fmaxf(0.0f, floorf(dvd(sub(mux, rxf), 16.0f))));
+    const int xmax = (int)fminf(gxf, fmaxf(0.0f, floorf(dvd(add(add(mux, rxf), 15.0f), 16.0f))));
+    const int ymin = (int)fminf(gyf, fmaxf(0.0f, floorf(dvd(sub(muy, ryf), 16.0f))));
+    const int ymax = (int)fminf(gyf, fmaxf(0.0f, floorf(dvd(add(add(muy, ryf), 15.0f), 16.0f))));
     if ((xmax - xmin) * (ymax - ymin) <= 0) return false;
     o.mux = mux; o.muy = muy; o.depth = pc2; o.radius = radius;
     o.xmin = xmin; o.ymin = ymin; o.xmax = xmax; o.ymax = ymax;
@@ -218,7 +240,7 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             px = __ldg(means + 3 * (size_t)i); py = __ldg(means + 3 * (size_t)i + 1); pz = __ldg(means + 3 * (size_t)i + 2);
             const float sx = __ldg(scales + 3 * (size_t)i), sy = __ldg(scales + 3 * (size_t)i + 1), sz = __ldg(scales + 3 * (size_t)i + 2);
             const float4 q = __ldcs(reinterpret_cast<const float4*>(rots) + i);
-            vis = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, s);
+            vis = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, f.tile_cull ? __ldg(opac + i) : 1.0f, s);
         }
         const uint32_t cnt = __popc(__ballot_sync(0xffffffffu, vis));
         if (lane == 0 && cnt) atomicAdd(&s_nvis, cnt);
@@ -358,7 +380,7 @@ preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ me
                     const float sx = __ldg(scales + 3 * (size_t)i), sy = __ldg(scales + 3 * (size_t)i + 1), sz = __ldg(scales + 3 * (size_t)i + 2);
                     const float4 q = __ldcs(reinterpret_cast<const float4*>(rots) + i);
                     Splat t;
-                    vis[h] = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, t);
+                    vis[h] = project(f, px, py, pz, sx, sy, sz, q.x, q.y, q.z, q.w, f.tile_cull ? __ldg(opac + i) : 1.0f, t);
                     uint4 pg = zero4;
                     if (vis[h]) {
                         pg.x = (uint32_t)t.xmin | ((uint32_t)t.ymin << 16);

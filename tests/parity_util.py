@@ -123,8 +123,15 @@ def compare(r, it, ref, check_lists=True, check_pixels=True):
     return rep
 
 
-def oracle_and_compare(scene, cam_index=0, tile_subset=None, n_threads=8, variant=None, count_contrib=True, flags=0):
-    r, it = run_gpu_auto(scene, cam_index, variant=variant, count_contrib=count_contrib)
+def oracle_and_compare(scene, cam_index=0, tile_subset=None, n_threads=8, variant=None, count_contrib=True, flags=0, tile_cull=False):
+    """tile_cull: both sides in the tighter-rect mode (gs_set_tile_cull(1) / oracle flag TILE_CULL); reset to 0 afterwards."""
+    binding.gs_set_tile_cull(1 if tile_cull else 0)
+    try:
+        r, it = run_gpu_auto(scene, cam_index, variant=variant, count_contrib=count_contrib)
+    finally:
+        binding.gs_set_tile_cull(0)
+    if tile_cull:
+        flags |= oracle.TILE_CULL
     ref = oracle.render(scene, cam_index, tile_subset=tile_subset, n_threads=n_threads, flags=flags, fragile_delta=DELTA)
     rep = compare(r, it, ref, check_lists=not (flags & oracle.NO_LISTS),
                   check_pixels=not (flags & (oracle.NO_LISTS | oracle.NO_RENDER)))

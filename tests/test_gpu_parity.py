@@ -20,8 +20,10 @@ pytestmark = pytest.mark.gpu
 @pytest.fixture(autouse=True)
 def _default_variant():
     binding.gs_set_render_variant(4)
+    binding.gs_set_tile_cull(0)
     yield
     binding.gs_set_render_variant(4)
+    binding.gs_set_tile_cull(0)
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -473,3 +475,49 @@ def test_upload_restages_the_scene_on_every_call():
         assert torch.equal(r.out_rgb, want[k & 1]), "call %d" % k
     with pytest.raises(ValueError):
         r.upload(scenes.make_scene(2, P=10_000, W=320, H=240, f=400.0))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# tighter tile culling (gs_set_tile_cull(1) / oracle flag TILE_CULL): rects, N_dup, counts, ranges and
+# the sorted lists bit-exact against the oracle in the same mode; the image identical to the standard mode's
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,kw,pose", [
+    (1, {}, 0), (2, {}, 0), (2, {}, 5),
+    (3, dict(P=120_000, W=637, H=419, f=500.0), 7), (4, dict(P=60_000, W=963, H=541, f=750.0), 5),
+    (5, dict(P=400_000, W=1283, H=727, f=1000.0), 3)])
+def test_tile_cull_mode_matches_the_oracle_in_the_same_mode(config, kw, pose):
+    sc = scenes.make_scene(config, **kw)
+    rep, r, it, ref = pu.oracle_and_compare(sc, pose, tile_cull=True)
+    std = oracle.render(sc, pose, flags=oracle.NO_LISTS)
+    assert ref.n_dup < std.n_dup
+    print("config", config, "tile cull: N_dup %d -> %d (%.2f)" % (std.n_dup, ref.n_dup, ref.n_dup / std.n_dup), rep)
+
+
+@pytest.mark.parametrize("config,pose", [(3, 4), (5, 2)])
+def test_tile_cull_mode_full_size(config, pose):
+    sc = _full_scene(config)
+    binding.gs_set_tile_cull(1)
+    ref = oracle.render(sc, pose, n_threads=N_CPU, fragile_delta=pu.DELTA, flags=oracle.TILE_CULL)
+    r, it = pu.run_gpu_auto(sc, pose, start_dup=int(ref.n_dup) + 4096)
+    binding.gs_set_tile_cull(0)
+    rep = pu.compare(r, it, ref)
+    print("config", config, "FULL, tile cull, pose", pose, rep)
+
+
+def test_tile_cull_mode_leaves_the_image_unchanged():
+    """No pixel outside the tighter rect can be blended (alpha < 1/255 there), so the entries it removes contributed
+    exactly nothing: same contributor counts, and the same image and final T up to the rounding of the kernel's stop
+    repair (two entries are blended per iteration and a stopping pixel takes its pair back: which entries share a pair
+    changes with the list), from 30 % fewer list entries.  (In the oracle the two modes are bit-identical.)"""
+    sc = scenes.make_scene(2)
+    out = []
+    for mode in (0, 1):
+        binding.gs_set_tile_cull(mode)
+        r, it = pu.run_gpu_auto(sc, 3)
+        out.append((r.out_rgb.clone(), r.out_final_T.clone(), r.out_n_contrib.clone(), it.n_dup))
+    binding.gs_set_tile_cull(0)
+    assert out[1][3] < 0.8 * out[0][3]
+    assert torch.equal(out[0][2], out[1][2])
+    assert float((out[0][0] - out[1][0]).abs().max()) < 2e-6 and float((out[0][1] - out[1][1]).abs().max()) < 2e-6
+    with pytest.raises(binding.GsError):
+        binding.gs_set_tile_cull(2)

@@ -15,7 +15,10 @@
  *     kernels run on a library-owned side stream, forked from and joined back into `cuda_stream` with events.
  *     gs_render() returns after enqueueing; it performs NO host synchronisation unless timing is enabled.
  *   - Return value: 0 (GS_OK) or a negative error code; nothing is printed, thrown or exit()ed.
- *   - Not thread-safe per workspace; distinct workspaces on distinct streams may be used concurrently.
+ *   - Not thread-safe per workspace; distinct workspaces on distinct streams may be used concurrently (per-workspace
+ *     switches: gs_set_workspace_option).  The workspace must live on the CURRENT device (GS_ERR_BAD_ARG otherwise); the
+ *     first call on a device runs a short synchronous self-test (gs_set_rank_mode).  gs_release() frees what the library
+ *     keeps per workspace address.
  */
 #ifndef GS_H
 #define GS_H
@@ -109,11 +112,11 @@ int gs_get_timings(const void* workspace, float ms[GS_N_TIMINGS]);
  *   1 = + tile-local hoisting (Eq. 7-10)
  *   2 = + warp-level culling (Eq. 13-21)
  *   3 = + warp-coherent blending (Eq. 22, branch-free)            -- the paper's full method
- *   4 = B200 design (default): 2 pixels/thread, packed f32x2, per-warp ballot compaction, prefetched staging
- *   5 = experimental: variant 4's blend loop in warp-specialised persistent CTAs (producer / consumer warps, mbarrier ring)
+ *   4 = B200 design (default): 2 pixels/thread, packed f32x2, per-warp ballot compaction, cp.async-gathered staging
+ *   5 = (removed: the warp-specialised experiment of round 1; GS_ERR_BAD_ARG)
  *   6 = precision switch of PAPER.md Table V: variant 3 with the polynomial in GLOBAL pixel coordinates and fp32
  *       coefficients (Eq. 11).  For measuring the error the tile-local form removes; NOT within the parity tolerance.
- * Returns GS_ERR_BAD_ARG for an unknown variant.  Process-wide. */
+ * Returns GS_ERR_BAD_ARG for an unknown variant.  Process-wide default (see gs_set_workspace_option). */
 int gs_set_render_variant(int variant);
 int gs_get_render_variant(void);
 
@@ -148,6 +151,32 @@ int gs_set_render_stream(int enable);
 #define GS_N_STATS 4
 int gs_set_stats(int enable);
 int gs_get_stats(const void* workspace, uint64_t out[GS_N_STATS]);
+
+/* Per-workspace switches.  The setters above are process-wide DEFAULTS; a value set here applies to the gs_render() calls on
+ * this workspace only and wins over the default, so that two renderers (or a timed / statistics render next to a batch in
+ * another thread) cannot change each other's launch path.  value -1 = follow the process-wide switch again.  May be called
+ * before the first gs_render() on the workspace.  GS_ERR_BAD_ARG for an unknown option or value. */
+#define GS_OPT_RENDER_VARIANT 0   /* as gs_set_render_variant */
+#define GS_OPT_TILE_CULL 1        /* as gs_set_tile_cull      */
+#define GS_OPT_TIMING 2           /* as gs_set_timing         */
+#define GS_OPT_STATS 3            /* as gs_set_stats          */
+#define GS_OPT_RENDER_STREAM 4    /* as gs_set_render_stream  */
+#define GS_N_OPTIONS 5
+int gs_set_workspace_option(const void* workspace, int option, int value);
+
+/* Releases what the library keeps for a workspace address: its side stream, its render stream, their events and the
+ * record of the last call (gs_get_intermediates / gs_get_timings / gs_get_stats then fail until the next gs_render).
+ * Synchronises those streams first.  Call it before freeing the workspace; GS_OK also when nothing was kept. */
+int gs_release(const void* workspace);
+
+/* Ranking of the radix passes (csrc/binning.cu).  0: one shared-memory atomicAdd per key, whose returned value is the
+ * stable rank PROVIDED the hardware serves same-address lanes in lane order (true on sm_100, not a PTX guarantee);
+ * 1: ballot multi-split, documented semantics only (8 ballots per key round).  -1 (default): decided per device by
+ * gs_selftest_atomic_order(), run once on the first gs_render() on that device -- if it ever reports a violation the
+ * library ranks with ballots instead of returning unstable lists.  gs_get_rank_mode() returns the mode in force on the
+ * current device (running the self-test if it has not run yet), or a negative error code. */
+int gs_set_rank_mode(int mode);
+int gs_get_rank_mode(void);
 
 /* Number of kernel launches (ours; memsets not counted) enqueued by the last gs_render() in this process. */
 int gs_last_launch_count(void);

@@ -25,7 +25,9 @@ TIMING_NAMES = ("preprocess", "depth_sort", "tile_grid", "offset_scan", "duplica
 EXPORTS = ("gs_workspace_bytes", "gs_render", "gs_get_intermediates", "gs_set_timing", "gs_get_timings",
            "gs_set_render_variant", "gs_get_render_variant", "gs_last_launch_count", "gs_error_string",
            "gs_last_cuda_error", "gs_copy_to_host", "gs_set_stats", "gs_get_stats", "gs_selftest_atomic_order",
-           "gs_set_render_stream", "gs_selftest_issue_peak", "gs_set_tile_cull", "gs_get_tile_cull")
+           "gs_set_render_stream", "gs_selftest_issue_peak", "gs_set_tile_cull", "gs_get_tile_cull",
+           "gs_set_workspace_option", "gs_release", "gs_set_rank_mode", "gs_get_rank_mode")
+GS_OPT_RENDER_VARIANT, GS_OPT_TILE_CULL, GS_OPT_TIMING, GS_OPT_STATS, GS_OPT_RENDER_STREAM = range(5)
 GS_N_STATS = 4
 STATS_NAMES = ("warp_slots_walked", "pairs_blended", "entries_staged", "pairs_evaluated")
 
@@ -84,6 +86,13 @@ def lib():
         L.gs_get_stats.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.gs_copy_to_host.restype = C.c_int
         L.gs_copy_to_host.argtypes = [vp, vp, C.c_size_t]
+        L.gs_set_workspace_option.restype = C.c_int
+        L.gs_set_workspace_option.argtypes = [vp, C.c_int, C.c_int]
+        L.gs_release.restype = C.c_int
+        L.gs_release.argtypes = [vp]
+        L.gs_set_rank_mode.restype = C.c_int
+        L.gs_set_rank_mode.argtypes = [C.c_int]
+        L.gs_get_rank_mode.restype = C.c_int
         L.gs_set_tile_cull.restype = C.c_int
         L.gs_set_tile_cull.argtypes = [C.c_int]
         L.gs_get_tile_cull.restype = C.c_int
@@ -232,6 +241,32 @@ def gs_selftest_issue_peak(iters: int = 2000) -> dict:
     if rc != GS_OK:
         raise GsError(rc, "gs_selftest_issue_peak")
     return {"ffma": float(out[0]), "ffma2": float(out[1]), "ex2": float(out[2])}
+
+
+def gs_set_workspace_option(workspace, option: int, value: int) -> None:
+    """Per-workspace switch (include/gs.h): wins over the process-wide setter for calls on this workspace; -1 = follow it."""
+    rc = lib().gs_set_workspace_option(C.c_void_p(workspace.data_ptr()), int(option), int(value))
+    if rc != GS_OK:
+        raise GsError(rc, "gs_set_workspace_option")
+
+
+def gs_release(workspace) -> None:
+    rc = lib().gs_release(C.c_void_p(workspace.data_ptr()))
+    if rc != GS_OK:
+        raise GsError(rc, "gs_release")
+
+
+def gs_set_rank_mode(mode: int) -> None:
+    rc = lib().gs_set_rank_mode(int(mode))
+    if rc != GS_OK:
+        raise GsError(rc, "gs_set_rank_mode")
+
+
+def gs_get_rank_mode() -> int:
+    rc = int(lib().gs_get_rank_mode())
+    if rc < 0:
+        raise GsError(rc, "gs_get_rank_mode")
+    return rc
 
 
 def gs_set_tile_cull(mode: int) -> None:

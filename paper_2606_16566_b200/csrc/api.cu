@@ -11,7 +11,7 @@
 #include "common.cuh"
 
 namespace gs {
-int g_use_pdl = 1;
+thread_local int g_use_pdl = 1;   // set by gs_render on the calling thread for the launches it makes
 void launch_preprocess(const Frame&, const Pointers&, const float*, const float*, const float*, const float*, const float*,
                        int, cudaStream_t);
 void launch_depth_sort(const Frame&, const Pointers&, int, cudaStream_t, int*);
@@ -99,7 +99,13 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     return true;
 }
 
+struct WsOptions {   // per-workspace overrides of the process-wide switches; -1 = follow the process-wide value
+    int v[GS_N_OPTIONS] = {-1, -1, -1, -1, -1};
+};
+
 struct LastCall {
+    WsOptions opt;
+    int device = -1;
     Layout L;
     Frame f;
     unsigned long long max_dup = 0;
@@ -116,11 +122,61 @@ struct LastCall {
 std::mutex g_mu;
 std::map<const void*, LastCall> g_calls;
 std::atomic<int> g_tile_cull{0}, g_variant{4}, g_timing{0}, g_stats{0}, g_launches{0}, g_cuda_err{0}, g_render_stream{0};
-int g_n_sm = 0;
+std::atomic<int> g_rank_mode{-1};   // -1: decided per device by the self-test, 0: shared-atomic ranking, 1: ballot ranking
+
+struct DevInfo {
+    int n_sm = 0;
+    int rank_auto = -1;   // result of the atomic-order self-test on this device: 0 = the atomics rank stably, 1 = use ballots
+};
+std::map<int, DevInfo> g_devs;   // under g_mu
 
 int cuda_fail(cudaError_t e) {
     g_cuda_err.store((int)e);
+    (void)cudaGetLastError();   // clear the sticky-free error state for the next call
     return GS_ERR_CUDA;
+}
+#define GS_CK(call) do { const cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
+
+void destroy_call_resources(LastCall& lc) {
+    if (lc.have_events)
+        for (auto& e : lc.ev) if (e) { cudaEventDestroy(e); e = nullptr; }
+    lc.have_events = false;
+    if (lc.ev_fork) cudaEventDestroy(lc.ev_fork);
+    if (lc.ev_join) cudaEventDestroy(lc.ev_join);
+    if (lc.ev_r0) cudaEventDestroy(lc.ev_r0);
+    if (lc.ev_r1) cudaEventDestroy(lc.ev_r1);
+    if (lc.side) cudaStreamDestroy(lc.side);
+    if (lc.rstream) cudaStreamDestroy(lc.rstream);
+    lc.ev_fork = lc.ev_join = lc.ev_r0 = lc.ev_r1 = nullptr;
+    lc.side = lc.rstream = nullptr;
+}
+
+// The device the workspace lives on must be the current one (streams and events are created there); returns its SM count
+// and the ranking mode of the radix passes (the self-test of the shared-atomic order runs once per device, on first use).
+int device_info(const void* workspace, int& dev_out, DevInfo& info_out) {
+    cudaPointerAttributes at;
+    GS_CK(cudaPointerGetAttributes(&at, workspace));
+    int cur = 0;
+    GS_CK(cudaGetDevice(&cur));
+    if (at.type != cudaMemoryTypeDevice || at.device != cur) return GS_ERR_BAD_ARG;
+    dev_out = cur;
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        auto it = g_devs.find(cur);
+        if (it != g_devs.end() && it->second.rank_auto >= 0) { info_out = it->second; return GS_OK; }
+    }
+    DevInfo d;
+    GS_CK(cudaDeviceGetAttribute(&d.n_sm, cudaDevAttrMultiProcessorCount, cur));
+    uint64_t res[2] = {0, 0};
+    const int rc = gs_selftest_atomic_order(2, res);   // ~10^7 atomics, a few hundred microseconds; synchronous, once per device
+    if (rc != GS_OK) return rc;
+    d.rank_auto = res[0] == 0 ? 0 : 1;
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        g_devs[cur] = d;
+    }
+    info_out = d;
+    return GS_OK;
 }
 
 Pointers carve(void* ws, const Layout& L) {
@@ -205,19 +261,20 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     if (!fit_max_dup(P, W, H, workspace_bytes, max_dup)) return GS_ERR_WORKSPACE;
     make_layout(P, W, H, max_dup, L);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    if (g_n_sm == 0) {
-        int dev = 0, n = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return cuda_fail(e);
-        g_n_sm = n;
+    int dev = 0;
+    DevInfo dinfo;
+    {
+        const int rc = device_info(workspace, dev, dinfo);   // the workspace must live on the current device
+        if (rc != GS_OK) return rc;
     }
+    const int g_n_sm = dinfo.n_sm;
+    const int rank_mode = g_rank_mode.load() >= 0 ? g_rank_mode.load() : dinfo.rank_auto;
     Frame f;
     f.P = P; f.W = W; f.H = H; f.gx = L.gx; f.gy = L.gy; f.n_tiles = L.n_tiles;
     f.deg = sh_degree; f.K = (sh_degree + 1) * (sh_degree + 1);
     f.tile_bits = L.tile_bits; f.n_tile_passes = L.n_tile_passes;
     f.compact = P >= COMPACT_MIN_P ? 1 : 0;
-    f.tile_cull = g_tile_cull.load();
+    f.tile_cull = 0; f.rank_mode = 0;   // set below, from the options of this call
     f.diff_copies = L.diff_copies; f.diff_cells = L.diff_cells;
     f.cshift = L.cshift; f.cgx = L.cgx; f.cgy = L.cgy; f.n_ctiles = L.n_ctiles; f.cdiff_cells = L.cdiff_cells;
     for (int k = 0; k < 16; k++) { f.V[k] = viewmatrix[k]; f.PM[k] = projmatrix[k]; }
@@ -235,22 +292,42 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     Pointers pc = p;
     pc.ctrl = p.cctrl; pc.diff = p.cdiff; pc.ranges = p.cranges; pc.desc = nullptr; pc.ids = p.cids;
 
-    const bool timed = g_timing.load() != 0;
     LastCall* lc;
     {
         std::lock_guard<std::mutex> g(g_mu);
         lc = &g_calls[workspace];
     }
+    if (lc->device >= 0 && lc->device != dev) destroy_call_resources(*lc);   // the address now belongs to another device
+    lc->device = dev;
+    // the switches of THIS call: the workspace's own value where one was set (gs_set_workspace_option), else the process-wide one
+    auto opt = [&](int k, int process_wide) { return lc->opt.v[k] >= 0 ? lc->opt.v[k] : process_wide; };
+    const int variant = opt(GS_OPT_RENDER_VARIANT, g_variant.load());
+    const bool timed = opt(GS_OPT_TIMING, g_timing.load()) != 0;
+    const bool stats = opt(GS_OPT_STATS, g_stats.load()) != 0;
+    const bool render_stream = opt(GS_OPT_RENDER_STREAM, g_render_stream.load()) != 0;
+    f.tile_cull = opt(GS_OPT_TILE_CULL, g_tile_cull.load());
+    f.rank_mode = rank_mode;
+    fc.tile_cull = f.tile_cull; fc.rank_mode = rank_mode;
     if (timed && !lc->have_events) {
-        for (auto& e : lc->ev)
-            if (cudaEventCreate(&e) != cudaSuccess) return cuda_fail(cudaGetLastError());
         lc->have_events = true;
+        for (auto& e : lc->ev) {
+            const cudaError_t ce = cudaEventCreate(&e);
+            if (ce != cudaSuccess) { destroy_call_resources(*lc); return cuda_fail(ce); }
+        }
     }
     if (!lc->side) {
-        if (cudaStreamCreateWithFlags(&lc->side, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaEventCreateWithFlags(&lc->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&lc->ev_join, cudaEventDisableTiming) != cudaSuccess)
-            return cuda_fail(cudaGetLastError());
+        cudaError_t ce = cudaStreamCreateWithFlags(&lc->side, cudaStreamNonBlocking);
+        if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&lc->ev_fork, cudaEventDisableTiming);
+        if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&lc->ev_join, cudaEventDisableTiming);
+        if (ce != cudaSuccess) { destroy_call_resources(*lc); return cuda_fail(ce); }
+    }
+    if (render_stream && !timed && !lc->rstream) {
+        int lo = 0, hi = 0;
+        cudaError_t ce = cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        if (ce == cudaSuccess) ce = cudaStreamCreateWithPriority(&lc->rstream, cudaStreamNonBlocking, lo);
+        if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&lc->ev_r0, cudaEventDisableTiming);
+        if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&lc->ev_r1, cudaEventDisableTiming);
+        if (ce != cudaSuccess) { destroy_call_resources(*lc); return cuda_fail(ce); }
     }
     lc->L = L; lc->f = f; lc->max_dup = max_dup; lc->stream = st; lc->valid = true; lc->timed = timed;
 #ifdef GS_DEBUG_SYNC   // development builds only: synchronise and report after every stage (never defined in libgs.so)
@@ -260,16 +337,16 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
         if (timed) cudaEventRecord(lc->ev[k], st);
     };
 #else
-    auto mark = [&](int k) { if (timed) cudaEventRecord(lc->ev[k], st); };
+    cudaError_t mark_err = cudaSuccess;
+    auto mark = [&](int k) {
+        if (timed && mark_err == cudaSuccess) mark_err = cudaEventRecord(lc->ev[k], st);
+    };
 #endif
 
     // PDL hides launch latency between the 11 kernels of a small frame; large frames (kernels of 100+ us) gain nothing
-    // and lose a little to early-resident dependents, so they launch plainly.  GS_PDL=0/1 overrides (experiments).
-    {
-        static const char* env = getenv("GS_PDL");
-        g_use_pdl = env ? (env[0] == '1') : (P <= (1 << 21) && max_dup <= (1ull << 25));
-        if (timed) g_use_pdl = 0;
-    }
+    // and lose a little to early-resident dependents, so they launch plainly.  Thread-local: the launches below are made
+    // by this thread.
+    g_use_pdl = (!timed && P <= (1 << 21) && max_dup <= (1ull << 25)) ? 1 : 0;
     int launches = 0;
     mark(0);
     cudaError_t e = cudaMemsetAsync(workspace, 0, L.zero_end, st);
@@ -284,11 +361,11 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     // serialised on the caller's stream so that every per-stage time is that stage alone.
     const bool two_level = L.two_level;
     if (!timed) {
-        cudaEventRecord(lc->ev_fork, st);
-        cudaStreamWaitEvent(lc->side, lc->ev_fork, 0);
+        GS_CK(cudaEventRecord(lc->ev_fork, st));
+        GS_CK(cudaStreamWaitEvent(lc->side, lc->ev_fork, 0));
         launch_tile_grid(f, p, out_tile_counts, nullptr, lc->side, &launches);
         if (two_level) launch_tile_grid(fc, pc, p.ccounts, p.ctrl, lc->side, &launches);
-        cudaEventRecord(lc->ev_join, lc->side);
+        GS_CK(cudaEventRecord(lc->ev_join, lc->side));
     }
     launch_depth_sort(f, p, g_n_sm, st, &launches);          // (3a) LSD passes over the depth bits, pre-duplication
     mark(2);
@@ -296,7 +373,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
         launch_tile_grid(f, p, out_tile_counts, nullptr, st, &launches);
         if (two_level) launch_tile_grid(fc, pc, p.ccounts, p.ctrl, st, &launches);
     } else {
-        cudaStreamWaitEvent(st, lc->ev_join, 0);
+        GS_CK(cudaStreamWaitEvent(st, lc->ev_join, 0));
     }
     mark(3);
     if (two_level) {
@@ -310,30 +387,22 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
         launch_duplicate_and_tile_sort(f, p, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b)
     }
     mark(6);
-    const int variant = g_variant.load();                      // (4) render
-    const bool render_stream = g_render_stream.load() != 0;
-    cudaStream_t rs = st;
+    cudaStream_t rs = st;                                      // (4) render
     if (render_stream && !timed) {
-        if (!lc->rstream) {
-            int lo = 0, hi = 0;
-            cudaDeviceGetStreamPriorityRange(&lo, &hi);
-            cudaStreamCreateWithPriority(&lc->rstream, cudaStreamNonBlocking, lo);
-            cudaEventCreateWithFlags(&lc->ev_r0, cudaEventDisableTiming);
-            cudaEventCreateWithFlags(&lc->ev_r1, cudaEventDisableTiming);
-        }
         rs = lc->rstream;
-        cudaEventRecord(lc->ev_r0, st);
-        cudaStreamWaitEvent(rs, lc->ev_r0, 0);
+        GS_CK(cudaEventRecord(lc->ev_r0, st));
+        GS_CK(cudaStreamWaitEvent(rs, lc->ev_r0, 0));
     }
-    if (variant == 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, g_stats.load() != 0, rs);
+    if (variant == 4) launch_render_b200(f, p, out_rgb, out_final_T, out_n_contrib, g_n_sm, stats, rs);
     else launch_render_ladder(variant, f, p, out_rgb, out_final_T, out_n_contrib, rs);
     if (rs != st) {
-        cudaEventRecord(lc->ev_r1, rs);
-        cudaStreamWaitEvent(st, lc->ev_r1, 0);
+        GS_CK(cudaEventRecord(lc->ev_r1, rs));
+        GS_CK(cudaStreamWaitEvent(st, lc->ev_r1, 0));
     }
     launches++;
     mark(7);
     g_launches.store(launches);
+    if (mark_err != cudaSuccess) return cuda_fail(mark_err);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     if (timed) {
@@ -484,6 +553,60 @@ int gs_set_render_stream(int enable) {
     g_render_stream.store(enable ? 1 : 0);
     return GS_OK;
 }
+int gs_set_workspace_option(const void* workspace, int option, int value) {
+    if (!workspace || option < 0 || option >= GS_N_OPTIONS || value < -1) return GS_ERR_BAD_ARG;
+    if (option == GS_OPT_RENDER_VARIANT && (value > 6 || value == 5)) return GS_ERR_BAD_ARG;
+    if (option != GS_OPT_RENDER_VARIANT && value > 1) return GS_ERR_BAD_ARG;
+    std::lock_guard<std::mutex> g(g_mu);
+    g_calls[workspace].opt.v[option] = value;
+    return GS_OK;
+}
+
+int gs_release(const void* workspace) {
+    if (!workspace) return GS_ERR_BAD_ARG;
+    LastCall lc;
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        auto it = g_calls.find(workspace);
+        if (it == g_calls.end()) return GS_OK;
+        lc = it->second;
+        g_calls.erase(it);
+    }
+    cudaError_t e = cudaSuccess;
+    if (lc.side) e = cudaStreamSynchronize(lc.side);
+    if (lc.rstream && e == cudaSuccess) e = cudaStreamSynchronize(lc.rstream);
+    destroy_call_resources(lc);
+    return e == cudaSuccess ? GS_OK : cuda_fail(e);
+}
+
+int gs_set_rank_mode(int mode) {
+    if (mode < -1 || mode > 1) return GS_ERR_BAD_ARG;
+    g_rank_mode.store(mode);
+    return GS_OK;
+}
+
+int gs_get_rank_mode(void) {
+    const int forced = g_rank_mode.load();
+    if (forced >= 0) return forced;
+    int cur = 0;
+    if (cudaGetDevice(&cur) != cudaSuccess) return cuda_fail(cudaGetLastError());
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        auto it = g_devs.find(cur);
+        if (it != g_devs.end() && it->second.rank_auto >= 0) return it->second.rank_auto;
+    }
+    DevInfo d;
+    cudaError_t e = cudaDeviceGetAttribute(&d.n_sm, cudaDevAttrMultiProcessorCount, cur);
+    if (e != cudaSuccess) return cuda_fail(e);
+    uint64_t res[2] = {0, 0};
+    const int rc = gs_selftest_atomic_order(2, res);
+    if (rc != GS_OK) return rc;
+    d.rank_auto = res[0] == 0 ? 0 : 1;
+    std::lock_guard<std::mutex> g(g_mu);
+    g_devs[cur] = d;
+    return d.rank_auto;
+}
+
 int gs_last_launch_count(void) { return g_launches.load(); }
 int gs_last_cuda_error(void) { return g_cuda_err.load(); }
 

@@ -46,13 +46,41 @@ struct SortSmem {
 // exclusive scan of the global digit histogram.  digit(key) -> 0..255; store(pos, key) writes one output element.
 template <int ITEMS, typename K, typename DigitF, typename StoreF>
 __device__ __forceinline__ void radix_tile(SortSmem<ITEMS, K>& sm, K (&key)[ITEMS], const int tile, const uint32_t tile_n,
-                                           unsigned long long* __restrict__ status, DigitF digit, StoreF store) {
+                                           unsigned long long* __restrict__ status, const int rank_mode, DigitF digit, StoreF store) {
     constexpr int NW = SORT_THREADS / 32;
     constexpr int TILE_N = SORT_THREADS * ITEMS;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const uint32_t wbase = w * (32 * ITEMS) + lane;
     uint32_t rk2[ITEMS / 2];  // two 16-bit ranks per register (a warp holds 32 * ITEMS <= 512 keys)
-    if (tile_n == TILE_N) {
+    if (rank_mode != 0) {
+        // Ranking with documented semantics only (gs_set_rank_mode(1), or chosen by the device self-test): the lanes of a
+        // round that hold the same digit find each other with 8 ballots (multi-split), rank = the warp's running count of
+        // the digit + the number of such lanes below this one; the lowest of them advances the count.  ~10x the issue
+        // cost of the atomic form (profiles/r01_microbench.md), same result.
+        const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+        for (int j = 0; j < ITEMS; j++) {
+            const bool valid = wbase + j * 32 < tile_n;
+            const uint32_t d = digit(key[j]);
+            unsigned peers = __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+            for (int b = 0; b < 8; b++) {
+                const unsigned bb = __ballot_sync(0xffffffffu, (d >> b) & 1u);
+                peers &= ((d >> b) & 1u) ? bb : ~bb;
+            }
+            if (!valid) peers = 0u;
+            const int leader = peers ? __ffs(peers) - 1 : 0;
+            uint32_t base = 0;
+            if (valid && lane == leader) {
+                base = sm.hist[w][d];
+                sm.hist[w][d] = base + __popc(peers);
+            }
+            __syncwarp();
+            base = __shfl_sync(0xffffffffu, base, leader);
+            const uint32_t r = valid ? base + __popc(peers & lt) : 0u;
+            if (j & 1) rk2[j / 2] |= r << 16; else rk2[j / 2] = r;
+        }
+    } else if (tile_n == TILE_N) {
 #pragma unroll
         for (int j = 0; j < ITEMS; j += 2) {
             const uint32_t ra = atomicAdd(&sm.hist[w][digit(key[j])], 1u);
@@ -145,7 +173,7 @@ template <int ITEMS, int MODE>
 __global__ void __launch_bounds__(SORT_THREADS, 4)
 radix_pass_kernel(const void* __restrict__ in_v, void* __restrict__ out_v, const unsigned long long* __restrict__ n_ptr,
                   int shift, const uint32_t* __restrict__ ghist, unsigned long long* __restrict__ status,
-                  uint32_t* __restrict__ tile_counter) {
+                  uint32_t* __restrict__ tile_counter, const int rank_mode) {
     using K = typename std::conditional<MODE == 2, uint32_t, unsigned long long>::type;
     constexpr int TILE_N = SORT_THREADS * ITEMS;
     __shared__ SortSmem<ITEMS, K> sm;
@@ -186,7 +214,7 @@ radix_pass_kernel(const void* __restrict__ in_v, void* __restrict__ out_v, const
 #pragma unroll
             for (int j = 0; j < ITEMS; j++) key[j] = (wbase + j * 32 < tile_n) ? in[tile_base + wbase + j * 32] : (K)0;
         }
-        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, digit, store);
+        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, rank_mode, digit, store);
     }
 }
 
@@ -541,7 +569,7 @@ dup_pass_kernel(const Frame f, const Pointers p, void* __restrict__ out_v, const
         const uint32_t wbase = w * (32 * ITEMS) + lane;
 #pragma unroll
         for (int j = 0; j < ITEMS; j++) key[j] = (wbase + j * 32 < tile_n) ? sm.sorted[wbase + j * 32] : (K)0;
-        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, digit, store);   // first barrier inside precedes its stores
+        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, f.rank_mode, digit, store);   // first barrier inside precedes its stores
     }
 }
 
@@ -630,14 +658,14 @@ static int imin(long long a, long long b) { return (int)(a < b ? a : b); }
 template <int MODE>
 static void launch_pass(int items, int n_sm, unsigned long long capacity, const void* in, void* out,
                         const unsigned long long* n_ptr, int shift, const uint32_t* ghist, unsigned long long* status,
-                        uint32_t* tile_counter, cudaStream_t st) {
+                        uint32_t* tile_counter, cudaStream_t st, int rank_mode) {
     const long long tile_n = (long long)SORT_THREADS * items;
     const long long cap_tiles = ((long long)capacity + tile_n - 1) / tile_n;
     const int grid = imin(cap_tiles > 0 ? cap_tiles : 1, (long long)n_sm * 4);
     if (items == 16)
-        launch_pdl(radix_pass_kernel<16, MODE>, dim3(grid), dim3(SORT_THREADS), st, in, out, n_ptr, shift, ghist, status, tile_counter);
+        launch_pdl(radix_pass_kernel<16, MODE>, dim3(grid), dim3(SORT_THREADS), st, in, out, n_ptr, shift, ghist, status, tile_counter, rank_mode);
     else
-        launch_pdl(radix_pass_kernel<4, MODE>, dim3(grid), dim3(SORT_THREADS), st, in, out, n_ptr, shift, ghist, status, tile_counter);
+        launch_pdl(radix_pass_kernel<4, MODE>, dim3(grid), dim3(SORT_THREADS), st, in, out, n_ptr, shift, ghist, status, tile_counter, rank_mode);
 }
 
 void launch_depth_sort(const Frame& f, const Pointers& p, int n_sm, cudaStream_t st, int* launches) {
@@ -646,7 +674,7 @@ void launch_depth_sort(const Frame& f, const Pointers& p, int n_sm, cudaStream_t
     for (int pass = 0; pass < MAX_SORT_PASSES_DEPTH; pass++) {
         launch_pass<0>(items, n_sm, (unsigned long long)f.P, bufs[pass & 1], bufs[(pass + 1) & 1], &p.ctrl->n_sort,
                        32 + 8 * pass, p.ctrl->depth_hist[pass], p.st_depth + (size_t)pass * p.n_depth_tiles * 256,
-                       &p.ctrl->tile_counter[TC_DEPTH0 + pass], st);
+                       &p.ctrl->tile_counter[TC_DEPTH0 + pass], st, f.rank_mode);
         (*launches)++;
     }
 }
@@ -701,13 +729,13 @@ void launch_duplicate_and_tile_sort(const Frame& f, const Pointers& p, int n_sm,
         if (ev_after_duplicate) cudaEventRecord(ev_after_duplicate, st);
         if (f.n_tile_passes == 1)
             launch_pass<1>(items, n_sm, f.max_dup, p.entB, p.ids, &p.ctrl->n_dup_eff, 32, p.ctrl->tile_hist[0], p.st_tile,
-                           &p.ctrl->tile_counter[TC_TILE0], st);
+                           &p.ctrl->tile_counter[TC_TILE0], st, f.rank_mode);
         else if (packed)
             launch_pass<3>(items, n_sm, f.max_dup, p.entB, p.entA, &p.ctrl->n_dup_eff, 32, p.ctrl->tile_hist[0], p.st_tile,
-                           &p.ctrl->tile_counter[TC_TILE0], st);
+                           &p.ctrl->tile_counter[TC_TILE0], st, f.rank_mode);
         else {   // three passes: entB -> entA -> entB -> ids
             launch_pass<0>(items, n_sm, f.max_dup, p.entB, p.entA, &p.ctrl->n_dup_eff, 32, p.ctrl->tile_hist[0], p.st_tile,
-                           &p.ctrl->tile_counter[TC_TILE0], st);
+                           &p.ctrl->tile_counter[TC_TILE0], st, f.rank_mode);
         }
         (*launches)++;
     }
@@ -717,13 +745,13 @@ void launch_duplicate_and_tile_sort(const Frame& f, const Pointers& p, int n_sm,
         const void* in = bufs[(pass - 1) & 1];
         if (packed)
             launch_pass<2>(items, n_sm, f.max_dup, in, p.ids, &p.ctrl->n_dup_eff, 0, p.ctrl->tile_hist[pass], status,
-                           &p.ctrl->tile_counter[TC_TILE0 + pass], st);
+                           &p.ctrl->tile_counter[TC_TILE0 + pass], st, f.rank_mode);
         else if (last)
             launch_pass<1>(items, n_sm, f.max_dup, in, p.ids, &p.ctrl->n_dup_eff, 32 + 8 * pass, p.ctrl->tile_hist[pass], status,
-                           &p.ctrl->tile_counter[TC_TILE0 + pass], st);
+                           &p.ctrl->tile_counter[TC_TILE0 + pass], st, f.rank_mode);
         else
             launch_pass<0>(items, n_sm, f.max_dup, in, bufs[pass & 1], &p.ctrl->n_dup_eff, 32 + 8 * pass, p.ctrl->tile_hist[pass],
-                           status, &p.ctrl->tile_counter[TC_TILE0 + pass], st);
+                           status, &p.ctrl->tile_counter[TC_TILE0 + pass], st, f.rank_mode);
         (*launches)++;
     }
 }

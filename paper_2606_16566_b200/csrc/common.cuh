@@ -56,6 +56,7 @@ struct Frame {              // per-frame constants, passed by value to the kerne
     int cgx, cgy, n_ctiles, cdiff_cells;   // super-tile grid and its difference grid
     int tile_bits, n_tile_passes;         // of the grid the duplication + sort runs on (the super-tile grid)
     int compact;                // 1: preprocess compacts the visible Gaussians (P >= COMPACT_MIN_P)
+    int rank_mode;              // radix passes: 0 = rank by shared-memory atomics, 1 = by ballots (gs_set_rank_mode)
     int tile_cull;              // 1: tile rect intersected with the bounding box of the alpha >= 1/255 ellipse (gs_set_tile_cull)
     int diff_copies, diff_cells; // replicas of the coverage difference grid (power of two) and cells per replica
     float V[16], PM[16];
@@ -101,7 +102,7 @@ __device__ __forceinline__ void griddep_sync() {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
-extern int g_use_pdl;   // api.cu: 1 = launch with the programmatic-serialization attribute (set per frame)
+extern thread_local int g_use_pdl;   // api.cu: 1 = launch with the programmatic-serialization attribute (set per frame, by the calling thread)
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, Args&&... args) {
     cudaLaunchConfig_t cfg = {};

@@ -134,6 +134,9 @@ class Renderer:
 
     def render(self, cam, stream=None, count_contrib: bool = True, out_rgb=None) -> None:
         s = self.scene
+        if self._lanes and self._lanes[0]["render_stream"]:   # render_batch left lane 0 (this workspace) on the render stream
+            binding.gs_set_workspace_option(self.workspace, binding.GS_OPT_RENDER_STREAM, 0)
+            self._lanes[0]["render_stream"] = False
         binding.gs_render(s["means3D"], s["scales"], s["rotations"], s["opacities"], s["sh"], s["sh_degree"],
                           cam.viewmatrix, cam.projmatrix, cam.fx, cam.fy, cam.W, cam.H, s["bg"],
                           self.out_rgb if out_rgb is None else out_rgb,
@@ -179,7 +182,7 @@ class Renderer:
                       out_rgb=self.out_rgb if first else torch.empty_like(self.out_rgb),
                       out_final_T=self.out_final_T if first else torch.empty_like(self.out_final_T),
                       out_tile_counts=self.out_tile_counts if first else torch.empty_like(self.out_tile_counts),
-                      done=torch.cuda.Event(), copied=torch.cuda.Event(), copy_pending=False)
+                      done=torch.cuda.Event(), copied=torch.cuda.Event(), copy_pending=False, render_stream=False)
             self._lanes.append(ln)
         return self._lanes[k]
 
@@ -203,8 +206,7 @@ class Renderer:
         fork = torch.cuda.Event()
         fork.record(main)
         # several frames in flight: binning kernels on the lanes' high-priority streams, render kernels on the library's
-        # lowest-priority stream of each workspace (include/gs.h: gs_set_render_stream)
-        binding.gs_set_render_stream(lanes > 1)
+        # lowest-priority stream of each workspace (include/gs.h: gs_set_render_stream, set per workspace)
         host = None
         if to_host:
             if self._host_rgb is None or self._host_rgb.shape[0] < n:
@@ -222,6 +224,9 @@ class Renderer:
                 st.wait_event(ln["copied"])          # the image of frame i - lanes has left this lane's buffer
                 ln["copy_pending"] = False
             img = ln["out_rgb"] if out_rgb is None else out_rgb[i]
+            if ln["render_stream"] != (lanes > 1):     # a per-workspace switch: other renderers and threads are not affected
+                binding.gs_set_workspace_option(ln["workspace"], binding.GS_OPT_RENDER_STREAM, 1 if lanes > 1 else 0)
+                ln["render_stream"] = lanes > 1
             binding.gs_render(s["means3D"], s["scales"], s["rotations"], s["opacities"], s["sh"], s["sh_degree"],
                               cam.viewmatrix, cam.projmatrix, cam.fx, cam.fy, cam.W, cam.H, s["bg"], img,
                               ln["out_final_T"], ln["out_tile_counts"], None, ln["workspace"], st)
@@ -233,7 +238,6 @@ class Renderer:
                     host[i].copy_(img, non_blocking=True)
                 ln["copied"].record(cs)
                 ln["copy_pending"] = True
-        binding.gs_set_render_stream(False)
         for k in range(lanes):
             main.wait_event(self._lanes[k]["done"])
         if to_host:
@@ -243,6 +247,20 @@ class Renderer:
             for k in range(lanes):
                 self._lanes[k]["copy_pending"] = False
         return host
+
+    def close(self) -> None:
+        """Releases what the library keeps for this renderer's workspaces (streams, events); the tensors go with the object."""
+        wss = [self.workspace] + [ln["workspace"] for ln in (self._lanes or [])[1:]]
+        for ws in wss:
+            if ws is not None:
+                binding.gs_release(ws)
+        self._lanes = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
     def synchronize_readback(self) -> None:
         if self._ring is not None:

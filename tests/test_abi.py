@@ -47,6 +47,17 @@ def test_workspace_bytes_and_error_strings_host_only():
         assert binding.gs_error_string(code) not in ("ok", "unknown error")
     assert L.gs_set_render_variant(9) == binding.GS_ERR_BAD_ARG
     assert L.gs_set_render_variant(4) == 0 and binding.gs_get_render_variant() == 4
+    assert L.gs_set_render_variant(5) == binding.GS_ERR_BAD_ARG          # the removed warp-specialised experiment
+    # host-only argument checks of the round-2 entry points
+    assert L.gs_set_rank_mode(2) == binding.GS_ERR_BAD_ARG and L.gs_set_rank_mode(-1) == 0
+    assert L.gs_set_tile_cull(7) == binding.GS_ERR_BAD_ARG and L.gs_set_tile_cull(0) == 0
+    fake = ctypes.c_void_p(0x1000)
+    assert L.gs_set_workspace_option(fake, 9, 0) == binding.GS_ERR_BAD_ARG
+    assert L.gs_set_workspace_option(fake, binding.GS_OPT_RENDER_VARIANT, 5) == binding.GS_ERR_BAD_ARG
+    assert L.gs_set_workspace_option(fake, binding.GS_OPT_TILE_CULL, 2) == binding.GS_ERR_BAD_ARG
+    assert L.gs_set_workspace_option(None, 0, 0) == binding.GS_ERR_BAD_ARG
+    assert L.gs_set_workspace_option(fake, binding.GS_OPT_STATS, 1) == 0 and L.gs_release(fake) == 0   # nothing CUDA was created
+    assert L.gs_release(fake) == 0 and L.gs_release(None) == binding.GS_ERR_BAD_ARG
 
 
 def test_product_does_not_import_oracle():

@@ -521,3 +521,51 @@ def test_tile_cull_mode_leaves_the_image_unchanged():
     assert float((out[0][0] - out[1][0]).abs().max()) < 2e-6 and float((out[0][1] - out[1][1]).abs().max()) < 2e-6
     with pytest.raises(binding.GsError):
         binding.gs_set_tile_cull(2)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# boundary: ranking fallback, per-workspace switches, release
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,kw,pose", [(1, {}, 0), (2, {}, 2), (5, dict(P=1_100_000, W=1283, H=727, f=1000.0), 1)])
+def test_ballot_ranking_fallback_gives_the_same_lists(config, kw, pose):
+    """gs_set_rank_mode(1): the radix passes rank with ballots (documented semantics only) instead of the shared-memory
+    atomic whose lane order is a hardware property; every list must stay bit-exact (one-level and two-level binning)."""
+    assert binding.gs_get_rank_mode() == 0          # the self-test found the atomic ranking stable on this device
+    sc = scenes.make_scene(config, **kw)
+    binding.gs_set_rank_mode(1)
+    try:
+        assert binding.gs_get_rank_mode() == 1
+        rep, r, it, ref = pu.oracle_and_compare(sc, pose)
+        if config == 5:
+            r2 = pu.run_gpu(sc, pose, max_dup=9 << 20)       # two-level binning
+            it2 = r2.intermediates()
+            assert it2.n_coarse > 0 and np.array_equal(it2.sorted_ids, it.sorted_ids)
+    finally:
+        binding.gs_set_rank_mode(-1)
+    print("ballot ranking, config", config, rep)
+
+
+def test_workspace_options_are_per_workspace_and_release_forgets_the_workspace():
+    sc = scenes.make_scene(2, P=20_000, W=320, H=240, f=400.0)
+    ra = Renderer(sc.P, 320, 240, 1 << 20, device="cuda:0")
+    rb = Renderer(sc.P, 320, 240, 1 << 20, device="cuda:0")
+    ra.upload(sc); rb.upload(sc)
+    binding.gs_set_workspace_option(ra.workspace, binding.GS_OPT_TILE_CULL, 1)       # only renderer a
+    binding.gs_set_workspace_option(rb.workspace, binding.GS_OPT_STATS, 1)           # only renderer b
+    ra.render(sc.cameras[0]); rb.render(sc.cameras[0])
+    torch.cuda.synchronize()
+    ia, ib = ra.intermediates(copy=()), rb.intermediates(copy=())
+    assert ia.n_dup < ib.n_dup and ib.n_dup == oracle.render(sc, 0, flags=oracle.NO_LISTS).n_dup
+    assert binding.gs_get_stats(rb.workspace)["pairs_evaluated"] > 0 and binding.gs_get_stats(ra.workspace)["pairs_evaluated"] == 0
+    assert binding.gs_get_tile_cull() == 0                                           # the process-wide switch never moved
+    binding.gs_set_workspace_option(ra.workspace, binding.GS_OPT_TILE_CULL, -1)      # back to the process-wide value
+    ra.render(sc.cameras[0])
+    assert ra.intermediates(copy=()).n_dup == ib.n_dup
+    assert torch.equal(ra.out_rgb, rb.out_rgb)
+    binding.gs_release(ra.workspace)
+    with pytest.raises(binding.GsError):
+        ra.intermediates(copy=())                                                    # nothing is kept for a released workspace
+    ra.render(sc.cameras[1])                                                         # and it can simply be used again
+    rb.render(sc.cameras[1])
+    assert torch.equal(ra.out_rgb, rb.out_rgb)
+    ra.close(); rb.close()

@@ -278,7 +278,8 @@ def measure_config(config, args, ctx):
 
     # ---- size the workspace: largest N_dup over the poses (+5 %) -----------------------------------------------------
     max_dup, need = 1 << 21, 0
-    r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True)
+    graph = None if args.graph < 0 else bool(args.graph)
+    r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True, graph=graph)
     r.upload(pinned)
     overflowed = False
     for cam in cams:
@@ -293,7 +294,7 @@ def measure_config(config, args, ctx):
         del r
         torch.cuda.empty_cache()
         max_dup = int(need * 1.05) + 4096
-        r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True)
+        r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True, graph=graph)
         r.upload(pinned)
     # ---- statistics pass (untimed): units of the rooflines -------------------------------------------------------------
     binding.gs_set_stats(True)
@@ -489,7 +490,7 @@ def measure_config(config, args, ctx):
            "run": {"frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every step", "frames_in_flight": lanes,
                    "parallelism": "replicas x%d" % ws, "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "n_coarse_mean": n_coarse_m,
                    "binning": "two-level (8x8-tile super-tiles)" if n_coarse_m > 0 else "one-level", "res_scale": args.res_scale,
-                   "render_variant": binding.gs_get_render_variant(), "tile_cull": binding.gs_get_tile_cull(), "workspace_bytes": int(r.workspace.numel())},
+                   "render_variant": binding.gs_get_render_variant(), "tile_cull": binding.gs_get_tile_cull(), "cuda_graph": bool(r.graph), "workspace_bytes": int(r.workspace.numel())},
            "ms_per_frame": ms_per_step / n_pose, "wall_ms_per_step_incl_flush": 1e3 * wall / K,
            "latency": {"ms_per_frame": serial_ms_per_frame, "frames_per_s": ws * 1e3 / serial_ms_per_frame,
                        "how": "one frame in flight, one stream, L2 flushed before every frame"},
@@ -529,8 +530,11 @@ def run_ours(args):
     configs = [args.config] if args.config else [1, 2, 3, 4, 5]
     headline = args.config if args.config else HEADLINE_CONFIG
     results = {}
+    # everything runs on an ordinary (capturable) stream: the legacy default stream cannot replay CUDA graphs (gs_set_graph)
+    main_stream = torch.cuda.Stream(device=dev)
     for c in configs:
-        results[c] = measure_config(c, args, ctx)
+        with torch.cuda.stream(main_stream):
+            results[c] = measure_config(c, args, ctx)
     if rank == 0:
         line = dict(results[headline])
         line["peaks"] = dict(ctx["peaks"], issue_peak_measured=ctx["issue"])
@@ -572,6 +576,7 @@ def main():
     ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = the fastest of 1-6 over a few warm-up steps)")
     ap.add_argument("--res-scale", type=int, default=1, choices=(1, 2), help="render at 1x or 2x the configuration's resolution (our arm only)")
     ap.add_argument("--tile-cull", type=int, default=0, choices=(0, 1), help="gs_set_tile_cull: 1 = rects intersected with the alpha >= 1/255 bounding box (our arm only; the default is the standard 3-sigma rect)")
+    ap.add_argument("--graph", type=int, default=-1, choices=(-1, 0, 1), help="CUDA graph replay of the frame (gs_set_graph): -1 = the Renderer's default (on up to 2^21 Gaussians), 0 off, 1 on")
     ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")
     args = ap.parse_args()
     if args.gpus < 1:

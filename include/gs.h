@@ -152,6 +152,15 @@ int gs_set_render_stream(int enable);
 int gs_set_stats(int enable);
 int gs_get_stats(const void* workspace, uint64_t out[GS_N_STATS]);
 
+/* CUDA graph replay (small frames are launch-chain-bound).  With gs_set_graph(1) the launch sequence of
+ * a frame -- the workspace memset, the 10-12 kernels, the fork / join of the side and render streams -- is captured ONCE
+ * per workspace and (P, W, H, SH degree, capacity, switches) and replayed with one cudaGraphLaunch; before every replay
+ * the three kernel nodes whose arguments change (camera in preprocess and render, the caller's input / output pointers)
+ * are updated with cudaGraphExecKernelNodeSetParams.  Same kernels, same results.  Ignored (plain launches) while timing
+ * is enabled, for render variants other than 4 and on the legacy / per-thread default streams, which cannot be captured.
+ * Process-wide default, off; per workspace: GS_OPT_GRAPH. */
+int gs_set_graph(int enable);
+
 /* Per-workspace switches.  The setters above are process-wide DEFAULTS; a value set here applies to the gs_render() calls on
  * this workspace only and wins over the default, so that two renderers (or a timed / statistics render next to a batch in
  * another thread) cannot change each other's launch path.  value -1 = follow the process-wide switch again.  May be called
@@ -161,7 +170,8 @@ int gs_get_stats(const void* workspace, uint64_t out[GS_N_STATS]);
 #define GS_OPT_TIMING 2           /* as gs_set_timing         */
 #define GS_OPT_STATS 3            /* as gs_set_stats          */
 #define GS_OPT_RENDER_STREAM 4    /* as gs_set_render_stream  */
-#define GS_N_OPTIONS 5
+#define GS_OPT_GRAPH 5            /* as gs_set_graph          */
+#define GS_N_OPTIONS 6
 int gs_set_workspace_option(const void* workspace, int option, int value);
 
 /* Releases what the library keeps for a workspace address: its side stream, its render stream, their events and the

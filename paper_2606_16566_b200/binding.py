@@ -26,8 +26,8 @@ EXPORTS = ("gs_workspace_bytes", "gs_render", "gs_get_intermediates", "gs_set_ti
            "gs_set_render_variant", "gs_get_render_variant", "gs_last_launch_count", "gs_error_string",
            "gs_last_cuda_error", "gs_copy_to_host", "gs_set_stats", "gs_get_stats", "gs_selftest_atomic_order",
            "gs_set_render_stream", "gs_selftest_issue_peak", "gs_set_tile_cull", "gs_get_tile_cull",
-           "gs_set_workspace_option", "gs_release", "gs_set_rank_mode", "gs_get_rank_mode")
-GS_OPT_RENDER_VARIANT, GS_OPT_TILE_CULL, GS_OPT_TIMING, GS_OPT_STATS, GS_OPT_RENDER_STREAM = range(5)
+           "gs_set_workspace_option", "gs_release", "gs_set_rank_mode", "gs_get_rank_mode", "gs_set_graph")
+GS_OPT_RENDER_VARIANT, GS_OPT_TILE_CULL, GS_OPT_TIMING, GS_OPT_STATS, GS_OPT_RENDER_STREAM, GS_OPT_GRAPH = range(6)
 GS_N_STATS = 4
 STATS_NAMES = ("warp_slots_walked", "pairs_blended", "entries_staged", "pairs_evaluated")
 
@@ -88,6 +88,8 @@ def lib():
         L.gs_copy_to_host.argtypes = [vp, vp, C.c_size_t]
         L.gs_set_workspace_option.restype = C.c_int
         L.gs_set_workspace_option.argtypes = [vp, C.c_int, C.c_int]
+        L.gs_set_graph.restype = C.c_int
+        L.gs_set_graph.argtypes = [C.c_int]
         L.gs_release.restype = C.c_int
         L.gs_release.argtypes = [vp]
         L.gs_set_rank_mode.restype = C.c_int
@@ -254,6 +256,10 @@ def gs_release(workspace) -> None:
     rc = lib().gs_release(C.c_void_p(workspace.data_ptr()))
     if rc != GS_OK:
         raise GsError(rc, "gs_release")
+
+
+def gs_set_graph(enable: bool) -> None:
+    lib().gs_set_graph(1 if enable else 0)
 
 
 def gs_set_rank_mode(mode: int) -> None:

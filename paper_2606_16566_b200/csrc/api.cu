@@ -5,12 +5,15 @@
 #include <atomic>
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
 #include <map>
 #include <mutex>
+#include <vector>
 
 #include "common.cuh"
 
 namespace gs {
+thread_local CaptureLog g_caplog;
 thread_local int g_use_pdl = 1;   // set by gs_render on the calling thread for the launches it makes
 void launch_preprocess(const Frame&, const Pointers&, const float*, const float*, const float*, const float*, const float*,
                        int, cudaStream_t);
@@ -100,7 +103,7 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
 }
 
 struct WsOptions {   // per-workspace overrides of the process-wide switches; -1 = follow the process-wide value
-    int v[GS_N_OPTIONS] = {-1, -1, -1, -1, -1};
+    int v[GS_N_OPTIONS] = {-1, -1, -1, -1, -1, -1};
 };
 
 struct LastCall {
@@ -117,11 +120,21 @@ struct LastCall {
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     cudaStream_t rstream = nullptr;       // gs_set_render_stream(1): the render kernel runs on this lowest-priority stream
     cudaEvent_t ev_r0 = nullptr, ev_r1 = nullptr;
+    // gs_set_graph(1): the launch sequence of a frame, captured once per (shape, capacity, switches) and replayed; the three
+    // kernel nodes whose arguments change from frame to frame (camera, caller pointers) are updated before every launch
+    struct GNode { cudaGraphNode_t node = nullptr; cudaKernelNodeParams kp = {}; std::vector<void*> args; };
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t gexec = nullptr, gexec2 = nullptr;   // two instances, used alternately: the one being updated is never the one just launched
+    int gflip = 0;
+    GNode g_pre, g_grid, g_render;
+    long long gkey[12] = {};
+    int g_launches = 0;
 };
 
 std::mutex g_mu;
 std::map<const void*, LastCall> g_calls;
 std::atomic<int> g_tile_cull{0}, g_variant{4}, g_timing{0}, g_stats{0}, g_launches{0}, g_cuda_err{0}, g_render_stream{0};
+std::atomic<int> g_graph{0};
 std::atomic<int> g_rank_mode{-1};   // -1: decided per device by the self-test, 0: shared-atomic ranking, 1: ballot ranking
 
 struct DevInfo {
@@ -149,6 +162,11 @@ void destroy_call_resources(LastCall& lc) {
     if (lc.rstream) cudaStreamDestroy(lc.rstream);
     lc.ev_fork = lc.ev_join = lc.ev_r0 = lc.ev_r1 = nullptr;
     lc.side = lc.rstream = nullptr;
+    if (lc.gexec) cudaGraphExecDestroy(lc.gexec);
+    if (lc.gexec2) cudaGraphExecDestroy(lc.gexec2);
+    lc.gexec2 = nullptr;
+    if (lc.graph) cudaGraphDestroy(lc.graph);
+    lc.gexec = nullptr; lc.graph = nullptr;
 }
 
 // The device the workspace lives on must be the current one (streams and events are created there); returns its SM count
@@ -348,6 +366,8 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     // by this thread.
     g_use_pdl = (!timed && P <= (1 << 21) && max_dup <= (1ull << 25)) ? 1 : 0;
     int launches = 0;
+    auto enqueue = [&]() -> int {   // the launch sequence of one frame on `st` (+ the library's side / render streams)
+    launches = 0;
     mark(0);
     cudaError_t e = cudaMemsetAsync(workspace, 0, L.zero_end, st);
     if (e != cudaSuccess) return cuda_fail(e);
@@ -401,6 +421,80 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     }
     launches++;
     mark(7);
+    return GS_OK;
+    };   // enqueue
+
+    const bool special_stream = st == nullptr || st == cudaStreamLegacy || st == cudaStreamPerThread;   // cannot be captured
+    const bool use_graph = opt(GS_OPT_GRAPH, g_graph.load()) != 0 && !timed && variant == 4 && !special_stream;
+    cudaError_t e = cudaSuccess;
+    if (!use_graph) {
+        const int rc = enqueue();
+        if (rc != GS_OK) return rc;
+    } else {
+        const long long key[12] = {P, W, H, sh_degree, (long long)max_dup, f.tile_cull, rank_mode, stats ? 1 : 0, render_stream ? 1 : 0,
+                                   out_n_contrib ? 1 : 0, (long long)workspace_bytes, g_use_pdl};
+        bool fresh = false;
+        if (!lc->gexec || memcmp(key, lc->gkey, sizeof(key)) != 0) {
+            if (lc->gexec) { cudaGraphExecDestroy(lc->gexec); lc->gexec = nullptr; }
+            if (lc->gexec2) { cudaGraphExecDestroy(lc->gexec2); lc->gexec2 = nullptr; }
+            if (lc->graph) { cudaGraphDestroy(lc->graph); lc->graph = nullptr; }
+            g_caplog = CaptureLog();
+            GS_CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+            const int rc = enqueue();
+            cudaGraph_t g = nullptr;
+            const cudaError_t ce = cudaStreamEndCapture(st, &g);   // always ended, also after a failed enqueue
+            if (rc != GS_OK) { if (g) cudaGraphDestroy(g); return rc; }
+            if (ce != cudaSuccess) return cuda_fail(ce);
+            lc->graph = g;
+            e = cudaGraphInstantiate(&lc->gexec, g, 0);
+            if (e == cudaSuccess) e = cudaGraphInstantiate(&lc->gexec2, g, 0);
+            if (e != cudaSuccess) { destroy_call_resources(*lc); return cuda_fail(e); }
+            // the three nodes with per-frame arguments, found by their kernel function
+            size_t n_nodes = 0;
+            GS_CK(cudaGraphGetNodes(g, nullptr, &n_nodes));
+            std::vector<cudaGraphNode_t> nodes(n_nodes);
+            GS_CK(cudaGraphGetNodes(g, nodes.data(), &n_nodes));
+            lc->g_pre = LastCall::GNode(); lc->g_grid = LastCall::GNode(); lc->g_render = LastCall::GNode();
+            for (cudaGraphNode_t nd : nodes) {
+                cudaGraphNodeType ty;
+                GS_CK(cudaGraphNodeGetType(nd, &ty));
+                if (ty != cudaGraphNodeTypeKernel) continue;
+                cudaKernelNodeParams kp = {};
+                GS_CK(cudaGraphKernelNodeGetParams(nd, &kp));
+                LastCall::GNode* dst = nullptr;
+                int n_args = 0;
+                if (kp.func == g_caplog.preprocess) { dst = &lc->g_pre; n_args = 7; }
+                else if (kp.func == g_caplog.render) { dst = &lc->g_render; n_args = 8; }
+                else if (kp.func == g_caplog.tile_grid && *static_cast<uint32_t**>(kp.kernelParams[2]) == out_tile_counts) { dst = &lc->g_grid; n_args = 4; }
+                if (!dst) continue;
+                dst->node = nd; dst->kp = kp;
+                dst->args.assign(kp.kernelParams, kp.kernelParams + n_args);
+            }
+            if (!lc->g_pre.node || !lc->g_grid.node || !lc->g_render.node) { destroy_call_resources(*lc); return GS_ERR_CUDA; }
+            memcpy(lc->gkey, key, sizeof(key));
+            lc->g_launches = launches;
+            fresh = true;
+        }
+        lc->gflip ^= 1;
+        cudaGraphExec_t ex = lc->gflip ? lc->gexec2 : lc->gexec;
+        if (!fresh || lc->gflip) {   // (a fresh capture holds this frame's arguments; its twin does not)
+            auto set = [&](LastCall::GNode& gn) {
+                gn.kp.kernelParams = gn.args.data();
+                return cudaGraphExecKernelNodeSetParams(ex, gn.node, &gn.kp);
+            };
+            lc->g_pre.args[0] = &f;
+            lc->g_pre.args[2] = &means3D; lc->g_pre.args[3] = &scales; lc->g_pre.args[4] = &rotations;
+            lc->g_pre.args[5] = &opacities; lc->g_pre.args[6] = &sh_coeffs;
+            lc->g_grid.args[2] = &out_tile_counts;
+            lc->g_render.args[0] = &f;
+            lc->g_render.args[5] = &out_rgb; lc->g_render.args[6] = &out_final_T; lc->g_render.args[7] = &out_n_contrib;
+            GS_CK(set(lc->g_pre));
+            GS_CK(set(lc->g_grid));
+            GS_CK(set(lc->g_render));
+            launches = lc->g_launches;
+        }
+        GS_CK(cudaGraphLaunch(ex, st));
+    }
     g_launches.store(launches);
     if (mark_err != cudaSuccess) return cuda_fail(mark_err);
     e = cudaGetLastError();
@@ -577,6 +671,11 @@ int gs_release(const void* workspace) {
     if (lc.rstream && e == cudaSuccess) e = cudaStreamSynchronize(lc.rstream);
     destroy_call_resources(lc);
     return e == cudaSuccess ? GS_OK : cuda_fail(e);
+}
+
+int gs_set_graph(int enable) {
+    g_graph.store(enable ? 1 : 0);
+    return GS_OK;
 }
 
 int gs_set_rank_mode(int mode) {

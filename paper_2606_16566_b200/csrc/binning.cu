@@ -680,6 +680,7 @@ void launch_depth_sort(const Frame& f, const Pointers& p, int n_sm, cudaStream_t
 }
 
 void launch_tile_grid(const Frame& f, const Pointers& p, uint32_t* out_tile_counts, const Ctrl* parent, cudaStream_t st, int* launches) {
+    g_caplog.tile_grid = (const void*)tile_grid_kernel;
     launch_pdl(tile_grid_kernel, dim3(1), dim3(GRID_THREADS), st, f, p, out_tile_counts, parent);
     (*launches)++;
 }

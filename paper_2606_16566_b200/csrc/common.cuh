@@ -102,6 +102,10 @@ __device__ __forceinline__ void griddep_sync() {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
+// Kernel functions of the three launches whose arguments change from frame to frame (camera, caller pointers), noted by
+// their launchers so that api.cu can find the matching nodes of a captured CUDA graph (gs_set_graph).
+struct CaptureLog { const void* preprocess = nullptr; const void* tile_grid = nullptr; const void* render = nullptr; };
+extern thread_local CaptureLog g_caplog;
 extern thread_local int g_use_pdl;   // api.cu: 1 = launch with the programmatic-serialization attribute (set per frame, by the calling thread)
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, Args&&... args) {

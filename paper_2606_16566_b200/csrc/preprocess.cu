@@ -478,6 +478,7 @@ preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ me
 template <int DEG>
 static void launch_pre(const Frame& f, const Pointers& p, const float* means, const float* scales, const float* rots,
                        const float* opac, const float* sh, int grid, cudaStream_t st) {
+    g_caplog.preprocess = f.compact ? (const void*)preprocess2_kernel<DEG> : (const void*)preprocess_kernel<DEG>;
     if (f.compact) launch_pdl(preprocess2_kernel<DEG>, dim3(grid), dim3(PRE_THREADS), st, f, p, means, scales, rots, opac, sh);
     else launch_pdl(preprocess_kernel<DEG>, dim3(grid), dim3(PRE_THREADS), st, f, p, means, scales, rots, opac, sh);
 }

@@ -255,6 +255,8 @@ void launch_render_b200(const Frame& f, const Pointers& p, float* out_rgb, float
                         bool stats, cudaStream_t st) {
     (void)n_sm;
     const dim3 grid(f.n_tiles), block(QB);
+    g_caplog.render = (stats && out_n) ? (const void*)render_b200_kernel<true, true>
+                                       : (out_n ? (const void*)render_b200_kernel<true, false> : (const void*)render_b200_kernel<false, false>);
     if (stats && out_n)
         launch_pdl(render_b200_kernel<true, true>, grid, block, st, f, p.ctrl, p.desc, p.ids, p.rec, out_rgb, out_T, out_n);
     else if (out_n)

@@ -16,13 +16,17 @@ _SCENE_ARRAYS = ("means3D", "scales", "rotations", "opacities", "sh")
 
 
 class Renderer:
-    def __init__(self, P: int, W: int, H: int, max_dup: int, device="cuda:0", count_contrib: bool = True):
+    def __init__(self, P: int, W: int, H: int, max_dup: int, device="cuda:0", count_contrib: bool = True, graph=None):
+        """graph: replay the frame's launch sequence as a CUDA graph (include/gs.h: gs_set_graph); None = for scenes of up to
+        2^21 Gaussians, whose frames are launch-chain-bound."""
         self.P, self.W, self.H = int(P), int(W), int(H)
+        self.graph = (self.P <= (1 << 21)) if graph is None else bool(graph)
         self.device = torch.device(device)
         self.gx, self.gy = (W + 15) // 16, (H + 15) // 16
         self.max_dup = int(max_dup)
         nbytes = binding.gs_workspace_bytes(P, W, H, max_dup)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        binding.gs_set_workspace_option(self.workspace, binding.GS_OPT_GRAPH, 1 if self.graph else 0)
         self.out_rgb = torch.empty((3, H, W), dtype=torch.float32, device=self.device)
         self.out_final_T = torch.empty((H, W), dtype=torch.float32, device=self.device)
         self.out_tile_counts = torch.empty((self.gy * self.gx,), dtype=torch.int32, device=self.device)
@@ -183,6 +187,8 @@ class Renderer:
                       out_final_T=self.out_final_T if first else torch.empty_like(self.out_final_T),
                       out_tile_counts=self.out_tile_counts if first else torch.empty_like(self.out_tile_counts),
                       done=torch.cuda.Event(), copied=torch.cuda.Event(), copy_pending=False, render_stream=False)
+            if not first:
+                binding.gs_set_workspace_option(ln["workspace"], binding.GS_OPT_GRAPH, 1 if self.graph else 0)
             self._lanes.append(ln)
         return self._lanes[k]
 

@@ -569,3 +569,43 @@ def test_workspace_options_are_per_workspace_and_release_forgets_the_workspace()
     rb.render(sc.cameras[1])
     assert torch.equal(ra.out_rgb, rb.out_rgb)
     ra.close(); rb.close()
+
+
+def test_graph_replay_gives_the_same_frames_as_plain_launches():
+    """gs_set_graph / GS_OPT_GRAPH: the launch sequence is captured once and replayed with the camera and the caller's
+    pointers patched into three kernel nodes.  Poses, output tensors, the optional n_contrib output (another kernel: the
+    graph is re-captured) and the tile-cull switch change between calls; every frame must equal the plain-launch frame."""
+    sc = scenes.make_scene(2, P=30_000, W=400, H=300, f=500.0)
+    rg = Renderer(sc.P, 400, 300, 1 << 20, device="cuda:0", graph=True)
+    rp = Renderer(sc.P, 400, 300, 1 << 20, device="cuda:0", graph=False)
+    rg.upload(sc); rp.upload(sc)
+    other = torch.empty_like(rg.out_rgb)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):                      # a capturable stream (the legacy default stream falls back to plain launches)
+        for k, pose in enumerate([0, 3, 3, 5, 1, 0, 7, 2]):
+            cc = k not in (3, 4)
+            cull = 1 if k in (5, 6) else 0
+            binding.gs_set_workspace_option(rg.workspace, binding.GS_OPT_TILE_CULL, cull)
+            binding.gs_set_workspace_option(rp.workspace, binding.GS_OPT_TILE_CULL, cull)
+            out = other if k % 2 else None
+            rg.render(sc.cameras[pose], count_contrib=cc, out_rgb=out)
+            rp.render(sc.cameras[pose], count_contrib=cc)
+            st.synchronize()
+            img = other if k % 2 else rg.out_rgb
+            assert torch.equal(img, rp.out_rgb), "frame %d" % k
+            assert torch.equal(rg.out_final_T, rp.out_final_T) and torch.equal(rg.out_tile_counts, rp.out_tile_counts)
+            if cc:
+                assert torch.equal(rg.out_n_contrib, rp.out_n_contrib)
+            ig, ip = rg.intermediates(), rp.intermediates()
+            assert ig.n_dup == ip.n_dup and np.array_equal(ig.sorted_ids, ip.sorted_ids)
+        # batches: several workspaces, render streams, per-frame output tensors
+        cams = list(sc.cameras)
+        a = torch.empty((len(cams), 3, 300, 400), device="cuda:0")
+        b = torch.empty_like(a)
+        for rep in range(2):
+            rg.render_batch(cams, lanes=3, out_rgb=a)
+            rp.render_batch(cams, lanes=3, out_rgb=b)
+            st.synchronize()
+            assert torch.equal(a, b)
+    rep, *_ = pu.oracle_and_compare(sc, 4)           # and the oracle agrees with the plain path as everywhere else
+    rg.close(); rp.close()

@@ -248,7 +248,13 @@ def _stage_bytes(P, K_sh, n_vis, n_dup, n_coarse, n_sort_passes, max_dup):
 # ncu `--set full` captures of render_b200_kernel committed under profiles/ (file named beside each number): DRAM bytes
 # of one launch, and the hardware pipe utilisation / executed-work figures (A) and (B) of SURVEY.md 8(d).
 PROFILED = {
-    # config: (file, dram bytes read + written per launch, FMA pipe %, XU pipe %, issue slots %, executed FP32 thread-ops, MUFU thread-ops)
+    # (A) and (B) of SURVEY.md 8(d) and the DRAM traffic of one launch, from profiles/r02_render_ncu.md (ncu --set full, pose 0)
+    2: {"file": "profiles/r02_render_ncu.md", "dram_bytes": 10132992, "us_under_ncu": 49.3, "fma_pipe_pct": 50.8, "xu_pipe_pct": 42.4,
+        "issue_slots_pct": 67.2, "branch_uniformity_pct": 96.4, "threads_per_inst": 31.0,
+        "executed_fp32_thread_ops": 615531814, "executed_mufu_thread_ops": 57049984, "executed_work_roofline_frac": 0.350},
+    5: {"file": "profiles/r02_render_ncu.md", "dram_bytes": 316532736, "us_under_ncu": 644.6, "fma_pipe_pct": 48.4, "xu_pipe_pct": 46.1,
+        "issue_slots_pct": 71.0, "branch_uniformity_pct": 95.3, "threads_per_inst": 30.1,
+        "executed_fp32_thread_ops": 8539326460, "executed_mufu_thread_ops": 796944460, "executed_work_roofline_frac": 0.371},
 }
 
 
@@ -438,7 +444,7 @@ def measure_config(config, args, ctx):
     alu_peak = max(issue["ffma"], issue["ffma2"]) / 1e12    # T FP32 thread-operations / s
     render_s = stage_ms["render"] * 1e-3
     achieved = pairs_eval * INSTR_PER_PAIR / render_s / 1e12
-    prof = PROFILED.get(config) if args.res_scale == 1 else None
+    prof = PROFILED.get(config) if (args.res_scale == 1 and args.tile_cull == 0 and args.render_variant in (None, 4)) else None
     roofline = {"kernel": "render_b200_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                 "unit": "T FP32-pipe thread-instr/s", "frac": achieved / alu_peak,
                 "traffic": (prof["dram_bytes"] if prof else None),

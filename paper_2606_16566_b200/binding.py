@@ -55,9 +55,12 @@ def lib():
     """Loads (building if needed) libgs.so.  Raises if the CUDA extension is unavailable."""
     global _lib
     if _lib is None:
-        path = _build.LIB
-        if not os.path.exists(path) or os.environ.get("GS_REBUILD"):
-            path = _build.build()
+        if os.environ.get("GS_DEBUG_BOUNDS") == "1":   # the bounds-checked build of the same sources (tests only)
+            path = _build.build(debug_bounds=True)
+        else:
+            path = _build.LIB
+            if not os.path.exists(path) or os.environ.get("GS_REBUILD"):
+                path = _build.build()
         L = C.CDLL(path)
         vp = C.c_void_p
         L.gs_workspace_bytes.restype = C.c_size_t

@@ -16,6 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgs.so")
+LIB_DBG = os.path.join(HERE, "libgs_dbg.so")   # -DGS_DEBUG_BOUNDS: device-side checks of every workspace / output index
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include")]
 UNITS = {
@@ -41,23 +42,28 @@ def _deps():
     return d
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    os.makedirs(OBJ, exist_ok=True)
+def build(force: bool = False, verbose: bool = False, debug_bounds: bool = False) -> str:
+    """Builds libgs.so (or, with debug_bounds, libgs_dbg.so: the same sources with -DGS_DEBUG_BOUNDS, objects in build/dbg)."""
+    obj_dir = os.path.join(OBJ, "dbg") if debug_bounds else OBJ
+    lib = LIB_DBG if debug_bounds else LIB
+    extra = ["-DGS_DEBUG_BOUNDS"] if debug_bounds else []
+    os.makedirs(obj_dir, exist_ok=True)
     nvcc = _nvcc()
     objs, rebuilt = [], False
     for src, flags in UNITS.items():
+        flags = flags + extra
         s = os.path.join(CSRC, src)
-        o = os.path.join(OBJ, src.replace(".cu", ".o"))
+        o = os.path.join(obj_dir, src.replace(".cu", ".o"))
         objs.append(o)
         newest = max(os.path.getmtime(x) for x in [s] + _deps())
         if force or not os.path.exists(o) or os.path.getmtime(o) < newest:
             cmd = [nvcc] + ARCH + COMMON + flags + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
             subprocess.run(cmd, check=True)
             rebuilt = True
-    if rebuilt or not os.path.exists(LIB):
-        subprocess.run([nvcc] + ARCH + ["-shared", "-o", LIB] + objs, check=True)
-    return LIB
+    if rebuilt or not os.path.exists(lib):
+        subprocess.run([nvcc] + ARCH + ["-shared", "-o", lib] + objs, check=True)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, debug_bounds="--debug-bounds" in sys.argv))

@@ -46,7 +46,8 @@ struct SortSmem {
 // exclusive scan of the global digit histogram.  digit(key) -> 0..255; store(pos, key) writes one output element.
 template <int ITEMS, typename K, typename DigitF, typename StoreF>
 __device__ __forceinline__ void radix_tile(SortSmem<ITEMS, K>& sm, K (&key)[ITEMS], const int tile, const uint32_t tile_n,
-                                           unsigned long long* __restrict__ status, const int rank_mode, DigitF digit, StoreF store) {
+                                           unsigned long long* __restrict__ status, const int rank_mode, const unsigned long long n_total, DigitF digit, StoreF store) {
+    (void)n_total;
     constexpr int NW = SORT_THREADS / 32;
     constexpr int TILE_N = SORT_THREADS * ITEMS;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -116,6 +117,7 @@ __device__ __forceinline__ void radix_tile(SortSmem<ITEMS, K>& sm, K (&key)[ITEM
     for (int j = 0; j < ITEMS; j++) {
         if (wbase + j * 32 < tile_n) {
             const uint32_t d = digit(key[j]);
+            GS_BOUND(sm.bpos[d] + sm.hist[w][d] + ((rk2[j / 2] >> (16 * (j & 1))) & 0xffffu), TILE_N);
             sm.sorted[sm.bpos[d] + sm.hist[w][d] + ((rk2[j / 2] >> (16 * (j & 1))) & 0xffffu)] = key[j];
         }
     }
@@ -160,6 +162,7 @@ __device__ __forceinline__ void radix_tile(SortSmem<ITEMS, K>& sm, K (&key)[ITEM
         const uint32_t li = j * SORT_THREADS + tid;
         if (li < tile_n) {
             const K k = sm.sorted[li];
+            GS_BOUND(sm.gpos[digit(k)] + li, n_total);
             store(sm.gpos[digit(k)] + li, k);
         }
     }
@@ -214,7 +217,7 @@ radix_pass_kernel(const void* __restrict__ in_v, void* __restrict__ out_v, const
 #pragma unroll
             for (int j = 0; j < ITEMS; j++) key[j] = (wbase + j * 32 < tile_n) ? in[tile_base + wbase + j * 32] : (K)0;
         }
-        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, rank_mode, digit, store);
+        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, rank_mode, n, digit, store);
     }
 }
 
@@ -333,6 +336,7 @@ tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts 
     unsigned long long run = s_part[w] + inc - sum;
     for (int t = t0; t < t1; t++) {
         const uint32_t c = counts[t];
+        GS_BOUND(t, f.n_tiles);
         p.ranges[t] = overflow ? 0u : (uint32_t)run;
         if (p.desc != nullptr) {   // tile descriptor at its slot of the render schedule
             const int bk = lpt_bucket(c);
@@ -340,6 +344,7 @@ tile_grid_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ counts 
 #pragma unroll
             for (int k = 0; k < LPT_BUCKETS; k++)
                 if (k == bk) slot = pos[k]++;
+            GS_BOUND(slot, f.n_tiles);
             p.desc[slot] = overflow ? make_uint4((uint32_t)t, 0u, 0u, 0u) : make_uint4((uint32_t)t, (uint32_t)run, (uint32_t)(run + c), 0u);
         }
         run += c;
@@ -372,7 +377,8 @@ __device__ __forceinline__ uint32_t rect_tiles(const uint4 pg) {
 // One WARP per 256-rank tile (8 consecutive ranks per lane), chained through the look-back status words; no block
 // barrier.  The rect of every rank is gathered once here and stored in depth order for the duplicate kernel.
 __global__ void __launch_bounds__(SCAN_THREADS)
-scan_offsets_kernel(const Pointers p, const int cshift) {
+scan_offsets_kernel(const Pointers p, const int cshift, const unsigned long long max_dup) {
+    (void)max_dup;
     griddep_sync();
     const int lane = threadIdx.x & 31;
     const unsigned long long n = p.ctrl->n_vis;
@@ -451,7 +457,7 @@ scan_offsets_kernel(const Pointers p, const int cshift) {
                 }
                 if (tt[k]) {  // chunk boundaries c*DUP_TILE that fall inside [off, off + tt)
                     const unsigned long long c0 = (off + DUP_TILE - 1) / DUP_TILE, c1 = (off + tt[k] - 1) / DUP_TILE;
-                    for (unsigned long long c = c0; c <= c1; c++) p.chunk_start[c] = (uint32_t)(base_r + k);
+                    for (unsigned long long c = c0; c <= c1; c++) { GS_BOUND(c, max_dup / DUP_TILE + 2); p.chunk_start[c] = (uint32_t)(base_r + k); }
                 }
             }
             off += tt[k];
@@ -569,7 +575,7 @@ dup_pass_kernel(const Frame f, const Pointers p, void* __restrict__ out_v, const
         const uint32_t wbase = w * (32 * ITEMS) + lane;
 #pragma unroll
         for (int j = 0; j < ITEMS; j++) key[j] = (wbase + j * 32 < tile_n) ? sm.sorted[wbase + j * 32] : (K)0;
-        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, f.rank_mode, digit, store);   // first barrier inside precedes its stores
+        radix_tile<ITEMS, K>(sm, key, tile, tile_n, status, f.rank_mode, n, digit, store);   // first barrier inside precedes its stores
     }
 }
 
@@ -636,6 +642,7 @@ duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict
                     tx = x0; ty++; tile = ty * gx + tx;
                 }
             }
+            GS_BOUND(k0 + lk0, f.max_dup);
             unsigned long long* dst = ent + k0 + lk0;
             if (lk0 + GEN_ITEMS <= cn) {
 #pragma unroll
@@ -688,7 +695,7 @@ void launch_tile_grid(const Frame& f, const Pointers& p, uint32_t* out_tile_coun
 void launch_scan_offsets(const Frame& f, const Pointers& p, int cshift, int n_sm, cudaStream_t st, int* launches) {
     const long long cap_blocks = ((long long)f.P + SCAN_WARP_TILE * (SCAN_THREADS / 32) - 1) / (SCAN_WARP_TILE * (SCAN_THREADS / 32));
     const int grid = imin(cap_blocks > 0 ? cap_blocks : 1, (long long)n_sm * 8);
-    launch_pdl(scan_offsets_kernel, dim3(grid), dim3(SCAN_THREADS), st, p, cshift);
+    launch_pdl(scan_offsets_kernel, dim3(grid), dim3(SCAN_THREADS), st, p, cshift, (unsigned long long)f.max_dup);
     (*launches)++;
 }
 
@@ -829,6 +836,7 @@ expand_kernel(const Frame f, const Pointers p) {
 #pragma unroll
             for (int k = 0; k < SUPER; k++) {
                 const unsigned b = b8[k];
+                if ((b >> lane) & 1u) GS_BOUND((out - p.ids) + __popc(b & lt), f.max_dup);
                 if ((b >> lane) & 1u) out[__popc(b & lt)] = s_id[buf][32 * k + lane];
                 out += __popc(b);
             }

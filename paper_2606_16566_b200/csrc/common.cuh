@@ -4,6 +4,15 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// -DGS_DEBUG_BOUNDS (build.py build(debug_bounds=True) -> libgs_dbg.so, loaded with GS_DEBUG_BOUNDS=1): every index into the
+// workspace and into the caller's output arrays is checked on the device and a violation traps -- the stand-in for
+// compute-sanitizer, which is not available on the GPU pool.  Compiles to nothing in the product build.
+#ifdef GS_DEBUG_BOUNDS
+#define GS_BOUND(idx, limit) do { if (!((unsigned long long)(idx) < (unsigned long long)(limit))) __trap(); } while (0)
+#else
+#define GS_BOUND(idx, limit) ((void)0)
+#endif
+
 namespace gs {
 
 constexpr int TILE = 16;

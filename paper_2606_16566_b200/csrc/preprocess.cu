@@ -252,6 +252,7 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
                 pg.z = __float_as_uint(s.depth);
                 pg.w = (uint32_t)s.radius;
             }
+            GS_BOUND(i, f.P);
             p.per_g[i] = pg;
             // a culled Gaussian sorts behind every depth: digit 255 in all four passes
             const uint32_t db = vis ? __float_as_uint(s.depth) : 0xffffffffu;
@@ -262,6 +263,7 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             p.gkeyA[i] = vis ? (((unsigned long long)db << 32) | (unsigned)i) : ~0ull;
         }
         if (vis) {
+            GS_BOUND(s.ymax * gw + s.xmax, f.diff_cells); GS_BOUND(s.ymin * gw + s.xmin, f.diff_cells);
             atomicAdd(diff + s.ymin * gw + s.xmin, 1);
             atomicAdd(diff + s.ymin * gw + s.xmax, -1);
             atomicAdd(diff + s.ymax * gw + s.xmin, -1);
@@ -270,6 +272,7 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
                 const int cs = f.cshift, cr = (1 << cs) - 1;
                 const int cx0 = s.xmin >> cs, cy0 = s.ymin >> cs;
                 const int cx1 = (s.xmax + cr) >> cs, cy1 = (s.ymax + cr) >> cs;
+                GS_BOUND(cy1 * cgw + cx1, f.cdiff_cells);
                 atomicAdd(cdiff + cy0 * cgw + cx0, 1);
                 atomicAdd(cdiff + cy0 * cgw + cx1, -1);
                 atomicAdd(cdiff + cy1 * cgw + cx0, -1);
@@ -358,6 +361,7 @@ preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ me
                 if (!alive) p.per_g[i] = zero4;
             }
             const unsigned ba = __ballot_sync(0xffffffffu, alive);
+            if (alive) GS_BOUND(n_alive + __popc(ba & lt), PRE2_TILE);
             if (alive) s_q[w][n_alive + __popc(ba & lt)] = (uint32_t)i;
             n_alive += __popc(ba);
         }
@@ -416,6 +420,7 @@ preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ me
                     g[h].a, g[h].b, g[h].c, g[h].d, g[h].e};
                 depth_bits[h] = pg.z;
                 const float px = __ldg(means + 3 * (size_t)i), py = __ldg(means + 3 * (size_t)i + 1), pz = __ldg(means + 3 * (size_t)i + 2);
+                GS_BOUND(t.ymax * gw + t.xmax, f.diff_cells); GS_BOUND(t.ymin * gw + t.xmin, f.diff_cells); GS_BOUND(i, f.P);
                 atomicAdd(diff + t.ymin * gw + t.xmin, 1);
                 atomicAdd(diff + t.ymin * gw + t.xmax, -1);
                 atomicAdd(diff + t.ymax * gw + t.xmin, -1);
@@ -424,6 +429,7 @@ preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ me
                     const int cs = f.cshift, cr = (1 << cs) - 1;
                     const int cx0 = t.xmin >> cs, cy0 = t.ymin >> cs;
                     const int cx1 = (t.xmax + cr) >> cs, cy1 = (t.ymax + cr) >> cs;
+                    GS_BOUND(cy1 * cgw + cx1, f.cdiff_cells);
                     atomicAdd(cdiff + cy0 * cgw + cx0, 1);
                     atomicAdd(cdiff + cy0 * cgw + cx1, -1);
                     atomicAdd(cdiff + cy1 * cgw + cx0, -1);
@@ -459,6 +465,7 @@ preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ me
         uint32_t before = 0;
 #pragma unroll
         for (int h = 0; h < PRE2_TILE / 32; h++) {
+            if (vis[h]) GS_BOUND(excl + before + __popc(vb[h] & lt), f.P);
             if (vis[h]) p.gkeyA[excl + before + __popc(vb[h] & lt)] = ((unsigned long long)depth_bits[h] << 32) | (unsigned)idx[h];
             before += __popc(vb[h]);
         }

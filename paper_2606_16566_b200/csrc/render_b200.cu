@@ -122,6 +122,7 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
     // blocks are dispatched in index order: descriptor b follows the render schedule of tile_grid_kernel (classes of
     // list length, longest first, raster order inside), so the long tiles start first and the launch has no tail
     const uint4 dsc = desc[blockIdx.x];
+    GS_BOUND(dsc.x, f.n_tiles); GS_BOUND(dsc.z, f.max_dup + 1); GS_BOUND(dsc.y, (unsigned long long)dsc.z + 1);
     const int tile = (int)dsc.x;
     const int tyi = tile / f.gx, txi = tile - tyi * f.gx;
     const int Tx = txi * TILE, Ty = tyi * TILE;
@@ -226,6 +227,7 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
         if ((bb.y >> lane) & 1u) list[c0 + __popc(bb.y & lt)] = rec_addr + (32 + lane) * REC;
         if ((bb.z >> lane) & 1u) list[c1 + __popc(bb.z & lt)] = rec_addr + (64 + lane) * REC;
         if ((bb.w >> lane) & 1u) list[c2 + __popc(bb.w & lt)] = rec_addr + (96 + lane) * REC;
+        GS_BOUND(cnt, QB + 1);
         list[cnt] = rec_addr + QB * REC;  // pad to an even length with the null record (alpha = 0); same word from every lane
         __syncwarp();
         // ---- blend: this warp walks ITS list only, two entries per iteration ---------------------------------------

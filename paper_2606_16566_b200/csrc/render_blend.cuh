@@ -111,6 +111,8 @@ __device__ __forceinline__ void write_pixels(const Frame& f, const PixelPair& s,
     unpk(s.Cr, c0r, c1r); unpk(s.Cg, c0g, c1g); unpk(s.Cb, c0b, c1b);
     T0 *= K_INV; T1 *= K_INV;
     const size_t npix = (size_t)f.W * f.H, pix = (size_t)py * f.W + px;
+    if (in0) GS_BOUND(pix, npix);
+    if (in1) GS_BOUND(pix + 1, npix);
     if (in1 && !(f.W & 1)) {  // both pixels inside, 8-byte aligned pair
         __stcs(reinterpret_cast<float2*>(out_rgb + pix), make_float2(fmaf(T0, f.bg[0], c0r), fmaf(T1, f.bg[0], c1r)));
         __stcs(reinterpret_cast<float2*>(out_rgb + npix + pix), make_float2(fmaf(T0, f.bg[1], c0g), fmaf(T1, f.bg[1], c1g)));

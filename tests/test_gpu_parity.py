@@ -609,3 +609,37 @@ def test_graph_replay_gives_the_same_frames_as_plain_launches():
             assert torch.equal(a, b)
     rep, *_ = pu.oracle_and_compare(sc, 4)           # and the oracle agrees with the plain path as everywhere else
     rg.close(); rp.close()
+
+
+def test_bounds_checked_build_runs_clean():
+    """libgs_dbg.so = the same sources with -DGS_DEBUG_BOUNDS: every index into the workspace and the output arrays is
+    checked on the device and a violation traps (the stand-in for compute-sanitizer, closed on this pool).  Configs 1 and 2 at
+    full size, a two-level frame, the tile-cull mode and the ballot ranking run through it in a fresh process and must still
+    agree with the oracle."""
+    import subprocess
+    import sys
+    code = r'''
+import sys
+sys.path.insert(0, "tests")
+import parity_util as pu
+from paper_2606_16566_b200 import binding, build, scenes
+assert binding.lib()._name == build.LIB_DBG, binding.lib()._name
+print(pu.oracle_and_compare(scenes.make_scene(1), 0)[0])
+sc = scenes.make_scene(2)
+print(pu.oracle_and_compare(sc, 0)[0])
+print(pu.oracle_and_compare(sc, 4, tile_cull=True)[0])
+binding.gs_set_rank_mode(1)
+print(pu.oracle_and_compare(sc, 6)[0])
+binding.gs_set_rank_mode(-1)
+sc = scenes.make_scene(3, P=300_000)
+r = pu.run_gpu(sc, 2, max_dup=9 << 20)
+it = r.intermediates()
+assert it.n_coarse > 0
+from oracle import oracle
+print(pu.compare(r, it, oracle.render(sc, 2, n_threads=8, fragile_delta=pu.DELTA)))
+print("BOUNDS OK")
+'''
+    env = dict(os.environ, GS_DEBUG_BOUNDS="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    res = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=1200)
+    assert res.returncode == 0 and "BOUNDS OK" in res.stdout, res.stdout[-2000:] + res.stderr[-3000:]

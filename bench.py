@@ -9,7 +9,9 @@ all five configurations are measured, each with its own W warm-up and K timed st
 `roofline`, `e2e` and `cpu_baseline` are those of configs[4] (10 M Gaussians, 3840x2160: the largest single-GPU
 workload, whose sort and render times BASELINE.json wants reported separately) and `per_config` holds the same fields
 for every configuration.  All five fit one GPU (config 4 needs ~21.5 GB of workspace).  With --config C only that one is
-measured and it is the headline.
+measured and it is the headline.  Every configuration also gets a companion entry `with_tile_cull`: the same measurement
+(no e2e, no CPU baseline) with gs_set_tile_cull(1) -- tighter tile rects, same image; the top-level
+numbers are always the standard 3-sigma rect of BASELINE.json's north_star.
 `value` = frames/s with the scene resident in HBM, device-timed (CUDA events on the launching stream around every step,
 L2 flushed before every step, max over ranks).  `latency` = one frame at a time, L2 flushed before every frame.
 `e2e` = the same metric through the public API with HOST buffers: every step copies the scene host->device from pinned
@@ -258,8 +260,9 @@ PROFILED = {
 }
 
 
-def measure_config(config, args, ctx):
-    """All measurements of one configuration on this rank; returns the result dict (rank 0 uses it)."""
+def measure_config(config, args, ctx, tile_cull=None, light=False):
+    """All measurements of one configuration on this rank; returns the result dict (rank 0 uses it).  tile_cull: override of
+    the process-wide switch for this measurement; light: no e2e and no CPU baseline (the tile-cull companion entries)."""
     import torch
     from paper_2606_16566_b200 import binding, scenes
     from paper_2606_16566_b200.renderer import Renderer
@@ -268,13 +271,15 @@ def measure_config(config, args, ctx):
     cfg = scenes.config_defaults(config)
     if args.res_scale != 1:   # PAPER.md Table VI's 1x / 2x resolution axis: same scene, image and focal length scaled
         cfg = dict(cfg, W=cfg["W"] * args.res_scale, H=cfg["H"] * args.res_scale, f=cfg["f"] * args.res_scale)
-        sc = scenes.make_scene(config, W=cfg["W"], H=cfg["H"], f=cfg["f"])
-    else:
-        sc = scenes.make_scene(config)
+    if config not in ctx["scenes"]:      # generated once per run (the 10 M-Gaussian scene takes ~25 s of numpy)
+        sc0 = scenes.make_scene(config, W=cfg["W"], H=cfg["H"], f=cfg["f"]) if args.res_scale != 1 else scenes.make_scene(config)
+        ctx["scenes"][config] = (sc0, Renderer.pin_scene(sc0))   # the host copy lives in pinned memory (what e2e uploads from)
+    sc, pinned = ctx["scenes"][config]
     cams = sc.cameras
     n_pose = len(cams)
     W, H = cfg["W"], cfg["H"]
-    pinned = Renderer.pin_scene(sc)      # the host copy of the scene lives in pinned memory (what e2e uploads from)
+    if tile_cull is not None:
+        binding.gs_set_tile_cull(tile_cull)
 
     def barrier():
         replica_barrier(ws)
@@ -414,37 +419,40 @@ def measure_config(config, args, ctx):
     stage_ms = {n: acc[n] / n_t for n in acc}
 
     # ---- e2e: host (pinned) buffers in, host images out, every step ---------------------------------------------------------
+    e2e_fps, h2d_bytes, d2h_bytes = None, 0, 0
+
     def e2e_step():
         h2d = r.upload(pinned)
         r.render_batch(cams, lanes=lanes, to_host=True)   # device -> pinned host copies overlap the later frames
         r.synchronize_readback()
         return h2d
-    for _ in range(2):
+    for _ in range(0 if light else 2):
         h2d_bytes = e2e_step()
     barrier()
     torch.cuda.synchronize()
     # K steps, each with its own host -> device copy of the scene and its own device -> host copies of the images; the
     # upload of step k+1 goes to a second set of device buffers on an upload stream while step k is rendered and read back
-    t0 = time.perf_counter()
-    r.upload_async(pinned)
-    for k in range(K):
-        r.activate_uploaded()
-        if k + 1 < K:
-            r.upload_async(pinned)
-        r.render_batch(cams, lanes=lanes, to_host=True)
-    r.synchronize_readback()
-    torch.cuda.synchronize()
-    e2e_s = rank_max(time.perf_counter() - t0)
-    h2d_bytes += n_pose * (16 + 16 + 3) * 4
-    d2h_bytes = n_pose * 3 * H * W * 4
-    e2e_fps = ws * n_pose * K / e2e_s
+    if not light:
+        t0 = time.perf_counter()
+        r.upload_async(pinned)
+        for k in range(K):
+            r.activate_uploaded()
+            if k + 1 < K:
+                r.upload_async(pinned)
+            r.render_batch(cams, lanes=lanes, to_host=True)
+        r.synchronize_readback()
+        torch.cuda.synchronize()
+        e2e_s = rank_max(time.perf_counter() - t0)
+        h2d_bytes += n_pose * (16 + 16 + 3) * 4
+        d2h_bytes = n_pose * 3 * H * W * 4
+        e2e_fps = ws * n_pose * K / e2e_s
 
     # ---- rooflines ---------------------------------------------------------------------------------------------------------------------
     issue = ctx["issue"]                                    # measured on this device, this run (gs_selftest_issue_peak)
     alu_peak = max(issue["ffma"], issue["ffma2"]) / 1e12    # T FP32 thread-operations / s
     render_s = stage_ms["render"] * 1e-3
     achieved = pairs_eval * INSTR_PER_PAIR / render_s / 1e12
-    prof = PROFILED.get(config) if (args.res_scale == 1 and args.tile_cull == 0 and args.render_variant in (None, 4)) else None
+    prof = PROFILED.get(config) if (args.res_scale == 1 and binding.gs_get_tile_cull() == 0 and args.render_variant in (None, 4)) else None
     roofline = {"kernel": "render_b200_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                 "unit": "T FP32-pipe thread-instr/s", "frac": achieved / alu_peak,
                 "traffic": (prof["dram_bytes"] if prof else None),
@@ -478,7 +486,7 @@ def measure_config(config, args, ctx):
     sort_ms = stage_ms["depth_sort"] + stage_ms["tile_grid"] + stage_ms["offset_scan"] + stage_ms["duplicate"] + stage_ms["tile_sort"]
 
     cpu_baseline = None
-    if rank == 0 and ws == 1 and not args.no_cpu_baseline:
+    if rank == 0 and ws == 1 and not args.no_cpu_baseline and not light:
         cores = os.cpu_count() or 1
         smp = OracleSampler(sc, config, cores)
         budget = args.cpu_seconds
@@ -508,8 +516,11 @@ def measure_config(config, args, ctx):
            "gpu_launches": launches, "launches_per_frame": launches_per_frame,
            "roofline": roofline, "kernels": kernels, "stage_ms_per_frame": stage_ms,
            "cpu_baseline": cpu_baseline}
-    del r, pinned, sc
+    r.close()
+    del r
     torch.cuda.empty_cache()
+    if tile_cull is not None:
+        binding.gs_set_tile_cull(args.tile_cull)
     return res
 
 
@@ -531,24 +542,36 @@ def run_ours(args):
     binding.gs_set_tile_cull(args.tile_cull)
     ctx = {"ws": ws, "rank": rank, "lrank": lrank, "dev": dev, "peaks": _peaks(),
            "n_sm": torch.cuda.get_device_properties(dev).multi_processor_count,
-           "flush": torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev),
+           "flush": torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev), "scenes": {},
            "issue": binding.gs_selftest_issue_peak(2000)}
     configs = [args.config] if args.config else [1, 2, 3, 4, 5]
     headline = args.config if args.config else HEADLINE_CONFIG
     results = {}
     # everything runs on an ordinary (capturable) stream: the legacy default stream cannot replay CUDA graphs (gs_set_graph)
     main_stream = torch.cuda.Stream(device=dev)
+    culled = {}
     for c in configs:
         with torch.cuda.stream(main_stream):
             results[c] = measure_config(c, args, ctx)
+            if args.tile_cull == 0 and not args.no_tile_cull_entries:
+                # companion entry: the same configuration with gs_set_tile_cull(1) (tighter rects, same image)
+                culled[c] = measure_config(c, args, ctx, tile_cull=1, light=True)
+        if c != configs[-1]:
+            ctx["scenes"].pop(c, None)   # one multi-GB scene at a time
     if rank == 0:
         line = dict(results[headline])
         line["peaks"] = dict(ctx["peaks"], issue_peak_measured=ctx["issue"])
-        line["gpu_launches"] = sum(r["gpu_launches"] for r in results.values())
+        line["gpu_launches"] = sum(r["gpu_launches"] for r in results.values()) + sum(r["gpu_launches"] for r in culled.values())
+        cull_keep = ("value", "unit", "ms_per_frame", "latency", "sort_ms_per_frame", "render_ms_per_frame", "roofline", "stage_ms_per_frame", "run", "clocks")
+        for c, rc in culled.items():
+            results[c]["with_tile_cull"] = {k: rc[k] for k in cull_keep}
+        if headline in culled:
+            line["with_tile_cull"] = results[headline]["with_tile_cull"]
         if len(configs) > 1:
             keep = ("config", "value", "unit", "ms_per_step", "ms_per_frame", "latency", "sort_ms_per_frame", "render_ms_per_frame",
-                    "e2e", "roofline", "cpu_baseline", "clocks", "gpu_launches", "launches_per_frame", "stage_ms_per_frame", "kernels", "run")
-            line["per_config"] = [{k: results[c][k] for k in keep} for c in configs]
+                    "e2e", "roofline", "cpu_baseline", "clocks", "gpu_launches", "launches_per_frame", "stage_ms_per_frame", "kernels", "run",
+                    "with_tile_cull")
+            line["per_config"] = [{k: results[c][k] for k in keep if k in results[c]} for c in configs]
             line["headline"] = "configs[%d] (top-level fields); every configuration has its own %d warm-up and %d timed steps" % (
                 headline - 1, args.warmup, args.steps)
         print(json.dumps(line))
@@ -583,6 +606,7 @@ def main():
     ap.add_argument("--res-scale", type=int, default=1, choices=(1, 2), help="render at 1x or 2x the configuration's resolution (our arm only)")
     ap.add_argument("--tile-cull", type=int, default=0, choices=(0, 1), help="gs_set_tile_cull: 1 = rects intersected with the alpha >= 1/255 bounding box (our arm only; the default is the standard 3-sigma rect)")
     ap.add_argument("--graph", type=int, default=-1, choices=(-1, 0, 1), help="CUDA graph replay of the frame (gs_set_graph): -1 = the Renderer's default (on up to 2^21 Gaussians), 0 off, 1 on")
+    ap.add_argument("--no-tile-cull-entries", action="store_true", help="skip the companion measurement of every configuration with gs_set_tile_cull(1)")
     ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")
     args = ap.parse_args()
     if args.gpus < 1:

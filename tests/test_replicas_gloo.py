@@ -46,3 +46,21 @@ def test_single_rank_needs_no_process_group():
     assert bench.replica_max(3.5, 1, None) == 3.5
     assert bench.aggregate_fps(1, 8, 2.0) == 4000.0
     bench.replica_barrier(1)
+
+
+def test_gpus_flag_without_torchrun_relaunches_itself_and_never_claims_more_ranks_than_it_runs(monkeypatch):
+    """`python bench.py --gpus N` outside torchrun must start N ranks (round-1 finding: it silently ran one replica and
+    printed n_gpus 1); a WORLD_SIZE that disagrees with --gpus is an error, not a quiet single-replica run."""
+    import subprocess
+    import bench
+    calls = []
+    monkeypatch.setattr(subprocess, "call", lambda cmd: calls.append(cmd) or 0)
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "4", "--steps", "3", "--config", "2"])
+    assert bench.main() == 0
+    (cmd,) = calls
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"] and cmd[cmd.index("--nproc-per-node") + 1] == "4"
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[-6:] == ["--gpus", "4", "--steps", "3", "--config", "2"]
+    assert os.path.basename(cmd[cmd.index("--master-port") + 2]) == "bench.py"
+    monkeypatch.setenv("WORLD_SIZE", "2")                       # launched by someone else with the wrong world size
+    assert bench.main() == 2 and len(calls) == 1

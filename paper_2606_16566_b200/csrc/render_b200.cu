@@ -40,7 +40,7 @@ __device__ __forceinline__ void blend_list(PixelPair& s, uint32_t& lp, uint32_t&
         float4 p1, q1;
         float2 p2, q2;
         float e0, e1, g0, g1;
-        u64 w1, w2, T1;
+        u64 w1, w2;
         bool hit;
         do {
             const uint32_t a1 = aa.x, a2 = aa.y;
@@ -55,9 +55,9 @@ __device__ __forceinline__ void blend_list(PixelPair& s, uint32_t& lp, uint32_t&
             const u64 al1 = alpha_pair<GUARD>(s, p0, p1, p2.y, e0, e1);
             const u64 al2 = alpha_pair<GUARD>(s, q0, q1, q2.y, g0, g1);
             w1 = fmul2(al1, s.T);
-            T1 = ffma2(bc(-K_SCALE), w1, s.T);
-            w2 = fmul2(al2, T1);
-            s.T = ffma2(bc(-K_SCALE), w2, T1);
+            ffma2_acc(s.T, bc(-K_SCALE), w1);
+            w2 = fmul2(al2, s.T);
+            ffma2_acc(s.T, bc(-K_SCALE), w2);
             ffma2_acc(s.Cr, bc(p1.z), w1);
             ffma2_acc(s.Cg, bc(p1.w), w1);
             ffma2_acc(s.Cb, bc(p2.x), w1);
@@ -73,30 +73,33 @@ __device__ __forceinline__ void blend_list(PixelPair& s, uint32_t& lp, uint32_t&
             hit = __any_sync(0xffffffffu, fminf(t0, t1) < TMIN_S);   // rare; a stopped pixel keeps T >= 1e-4 K: it never fires again
         } while (!hit && lp < lend);
         if (hit) {
-            float t0, t1, u0, u1, w10, w11, w20, w21;
+            float t0, t1, w10, w11, w20, w21;
             unpk(s.T, t0, t1);
-            unpk(T1, u0, u1); unpk(w1, w10, w11); unpk(w2, w20, w21);
-            const bool sa0 = u0 < TMIN_S, sa1 = u1 < TMIN_S;      // stopped at the first entry
+            unpk(w1, w10, w11); unpk(w2, w20, w21);
             const bool sb0 = t0 < TMIN_S, sb1 = t1 < TMIN_S;      // stopped at the first or the second entry
-            const u64 wm2 = pk(sb0 ? w20 : 0.0f, sb1 ? w21 : 0.0f), wm1 = pk(sa0 ? w10 : 0.0f, sa1 ? w11 : 0.0f);
+            const u64 wm2 = pk(sb0 ? w20 : 0.0f, sb1 ? w21 : 0.0f);
+            ffma2_acc(s.T, bc(K_SCALE), wm2);                     // on the stopped pixels: the T before the second entry
+            float u0, u1;
+            unpk(s.T, u0, u1);
+            const bool sa0 = sb0 && u0 < TMIN_S, sa1 = sb1 && u1 < TMIN_S;   // stopped at the first entry already
+            const u64 wm1 = pk(sa0 ? w10 : 0.0f, sa1 ? w11 : 0.0f);
+            ffma2_acc(s.T, bc(K_SCALE), wm1);
             ffma2_acc(s.Cr, bc(-q1.z), wm2);
             ffma2_acc(s.Cg, bc(-q1.w), wm2);
             ffma2_acc(s.Cb, bc(-q2.x), wm2);
             ffma2_acc(s.Cr, bc(-p1.z), wm1);
             ffma2_acc(s.Cg, bc(-p1.w), wm1);
             ffma2_acc(s.Cb, bc(-p2.x), wm1);
-            ffma2_acc(s.T, bc(K_SCALE), wm2);
-            ffma2_acc(s.T, bc(K_SCALE), wm1);
             float r0, r1;
             unpk(s.T, r0, r1);   // the T of rule R1 passed the test when it was formed: >= 1e-4 K up to the rounding of the repair
             s.T = pk(sb0 ? fmaxf(r0, TMIN_S) : r0, sb1 ? fmaxf(r1, TMIN_S) : r1);
-            ffma2_acc(s.bx2, pk(sb0 ? 1.0f : 0.0f, sb1 ? 1.0f : 0.0f), bc(POISON));
+            ffma2_acc(s.bx, pk(sb0 ? 1.0f : 0.0f, sb1 ? 1.0f : 0.0f), bc(POISON));
             if (COUNT) {
                 s.n0 -= (sa0 ? 1u + ((g0 > 0.0f) ? 1u : 0u) : (sb0 ? 1u : 0u));
                 s.n1 -= (sa1 ? 1u + ((g1 > 0.0f) ? 1u : 0u) : (sb1 ? 1u : 0u));
             }
             float x0, x1;
-            unpk(s.bx2, x0, x1);
+            unpk(s.bx, x0, x1);
             if (__all_sync(0xffffffffu, x0 >= 0.5f * POISON && x1 >= 0.5f * POISON)) lend = 0;
         }
     }
@@ -105,7 +108,7 @@ __device__ __forceinline__ void blend_list(PixelPair& s, uint32_t& lp, uint32_t&
 // 7 blocks per SM: 72 registers.  (8 blocks / 64 registers measured 8 % slower: ptxas then splits the live ranges of the
 // accumulators, 10 register moves per iteration of the blend loop instead of 4.)
 template <bool COUNT, bool STATS>
-__global__ void __launch_bounds__(QB, 7)
+__global__ void __launch_bounds__(QB, 8)
 render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restrict__ desc, const uint32_t* __restrict__ ids,
                    const float4* __restrict__ rec, float* __restrict__ out_rgb, float* __restrict__ out_T,
                    uint32_t* __restrict__ out_n) {
@@ -134,11 +137,9 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
     PixelPair s;
     {
         const float x0 = (float)lx - 7.5f, x1 = x0 + 1.0f, y = (float)ly - 7.5f;
-        s.bx2 = pk(in0 ? x0 * x0 : POISON, in1 ? x1 * x1 : POISON);
-        s.bxy = pk(x0 * y, x1 * y);
-        s.by2 = pk(y * y, y * y);
-        s.bx = pk(x0, x1);
-        s.by = pk(y, y);
+        s.bx = pk(in0 ? x0 : POISON, in1 ? x1 : POISON);
+        s.y = y;
+        s.y2 = y * y;
         s.T = pk(K_SCALE, K_SCALE);
         s.Cr = s.Cg = s.Cb = pk(0.0f, 0.0f);
         s.n0 = s.n1 = 0;

@@ -7,7 +7,7 @@
 namespace gs {
 
 constexpr int QB = 128;            // threads per block == staged entries per batch
-constexpr float POISON = 1.0e36f;  // x'^2 of a finished pixel: A * POISON <= -1e3 for every conic with a >= 1e-33
+constexpr float POISON = 1.0e18f;  // x' of a finished pixel: (A * POISON + H) * POISON <= -1e3 for every conic with a >= 1e-33 and |H| < 1e-15 a
 // alpha' = 2^(L + L_BIAS) = alpha / K:  alpha' < 2^-126 (flushed to 0 by ex2.approx.ftz)  <=>  alpha < 1/255
 constexpr float L_BIAS = -118.00564575195312f;   // fl32(-126 - log2(1/255))
 constexpr float K_SCALE = 3.33609985e+35f;       // 2^(-L_BIAS): alpha = K alpha', T_s = K T
@@ -38,7 +38,8 @@ __device__ __forceinline__ u64 bc(float v) { return pk(v, v); }  // scalar broad
 __device__ __forceinline__ void ffma2_acc(u64& acc, u64 a, u64 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b)); }
 
 struct PixelPair {
-    u64 bx2, bxy, by2, bx, by;  // B_local (Eq. 9) of the two pixels, tile-centre origin
+    u64 bx;                     // x' of the two pixels, tile-centre origin (B_local of Eq. 9 in separable form, see alpha_pair)
+    float y, y2;                // y' and y'^2: the two pixels of a thread share their row
     u64 T, Cr, Cg, Cb;          // T scaled by K
     uint32_t n0, n1;
 };
@@ -56,6 +57,11 @@ __device__ __forceinline__ float2 lds64(uint32_t addr) {
     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr) : "memory");
     return v;
 }
+__device__ __forceinline__ uint32_t lds32u(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
 __device__ __forceinline__ uint2 lds64u(uint32_t addr) {
     uint2 v;
     asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory");
@@ -67,11 +73,9 @@ __device__ __forceinline__ uint2 lds64u(uint32_t addr) {
 template <bool GUARD>
 __device__ __forceinline__ u64 alpha_pair(const PixelPair& s, const float4 q0, const float4 q1, const float guard, float& e0,
                                           float& e1) {
-    u64 L2 = ffma2(bc(q0.x), s.bx2, bc(q0.w));
-    L2 = ffma2(bc(q0.y), s.bxy, L2);
-    L2 = ffma2(bc(q0.z), s.by2, L2);
-    L2 = ffma2(bc(q1.x), s.bx, L2);
-    L2 = ffma2(bc(q1.y), s.by, L2);
+    const float H = fmaf(q0.y, s.y, q1.x);                       // B y' + D
+    const float G = fmaf(q0.z, s.y2, fmaf(q1.y, s.y, q0.w));     // C y'^2 + E y' + F
+    const u64 L2 = ffma2(ffma2(bc(q0.x), s.bx, bc(H)), s.bx, bc(G));   // (A x' + H) x' + G
     float L0, L1;
     unpk(L2, L0, L1);
     e0 = ex2_approx(L0);

@@ -35,7 +35,6 @@ namespace gs {
 // pixels are poisoned.  When the whole warp is finished (Eq. 22) `lend` is zeroed: the warp-uniform end of the walk.
 template <bool COUNT, bool GUARD>
 __device__ __forceinline__ void blend_list(PixelPair& s, uint32_t& lp, uint32_t& lend) {
-    uint2 aa = lds64u(lp);
     while (lp < lend) {
         float4 p1, q1;
         float2 p2, q2;
@@ -43,9 +42,9 @@ __device__ __forceinline__ void blend_list(PixelPair& s, uint32_t& lp, uint32_t&
         u64 w1, w2;
         bool hit;
         do {
+            const uint2 aa = lds64u(lp);   // no prefetch across the back edge: ptxas carried a prefetched pair through two moves
             const uint32_t a1 = aa.x, a2 = aa.y;
             lp += 8;
-            aa = lds64u(lp);   // the pair after this one (the list buffer has room for one pair past the padding)
             const float4 p0 = lds128(a1);                     // (A, B, C, F)
             p1 = lds128(a1 + 16);                             // (D, E, r, g)
             p2 = lds64(a1 + 32);                              // (b, guard)
@@ -161,6 +160,8 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
     // c ^ ((j >> 1) & 3): the 16-byte reads of the staging thread (stride 64 bytes across lanes) are then conflict-free.
     // Warp w gathers, and later stages, entries 32 w .. 32 w + 31 of the batch: the raw records are warp-private.
     const uint32_t raw_w = (uint32_t)__cvta_generic_to_shared(&s_raw[w * 32 * 64]);
+    // this thread's own raw record: chunk c sits at raw_me ^ (c << 4) (the swizzle above, (lane >> 1) & 3 for record `lane`)
+    const uint32_t raw_me = raw_w + lane * 64 + (((uint32_t)(lane >> 1) & 3u) << 4);
     auto gather = [&](const uint32_t id_mine, const uint32_t n_valid /* entries of this warp in the batch */) {
 #pragma unroll
         for (int k = 0; k < 4; k++) {
@@ -184,28 +185,30 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
     if (start + QB + tid < end) id_next = ids[start + QB + tid];
     int buf = 0;
     for (uint32_t base = start; base < end; base += QB, buf ^= 1) {
-        // ---- staging of batch `base` from registers: tight box -> 4-bit warp mask, hoist -> shared memory ----------
-        uint32_t m = 0;
-        bool indefinite = false;
+        // ---- staging of batch `base`: tight box -> four quadrant hits -> ballots, hoist -> shared memory -------------
         if (STATS && tid == 0) st_staged += min((uint32_t)QB, end - base);
-        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0, r2 = r0, r3 = r0;
         cp_async_wait_all();
         __syncwarp();               // the four chunks of this thread's record were copied by four lanes of this warp
-        if (base + tid < end) {
-            const uint32_t a = raw_w + lane * 64, sw = (uint32_t)((lane >> 1) & 3);
-            r0 = lds128(a + ((0u ^ sw) << 4)); r1 = lds128(a + ((1u ^ sw) << 4));
-            r2 = lds128(a + ((2u ^ sw) << 4)); r3 = lds128(a + ((3u ^ sw) << 4));
-            m = quadrant_mask(r0.x - (float)Tx, r0.y - (float)Ty, r0.z, r0.w, r1.x, r1.y, r1.z);
-            if (__float_as_uint(r1.w) & 1u) { m = 15u; indefinite = true; }  // degenerate conic: keep everything
-        }
-        const unsigned b0 = __ballot_sync(0xffffffffu, m & 1u), b1 = __ballot_sync(0xffffffffu, m & 2u),
-                       b2 = __ballot_sync(0xffffffffu, m & 4u), b3 = __ballot_sync(0xffffffffu, m & 8u);
+        // straight-line for every lane: a lane past the end of the list works on whatever its raw slot holds (stale
+        // bytes, never a trap) and is masked out of the predicates -- no divergent region, the four hits go to the votes
+        const bool valid = base + tid < end;
+        const float4 r0 = lds128(raw_me), r1 = lds128(raw_me ^ 0x10u), r2 = lds128(raw_me ^ 0x20u), r3 = lds128(raw_me ^ 0x30u);
+        bool q[4];
+        quadrant_hits(r0.x - (float)Tx, r0.y - (float)Ty, r0.z, r0.w, r1.x, r1.y, r1.z, q);
+        const bool indefinite = valid && (__float_as_uint(r1.w) & 1u);   // degenerate conic: keep everything
+#pragma unroll
+        for (int k = 0; k < 4; k++) q[k] = (valid && q[k]) || indefinite;
+        const unsigned b0 = __ballot_sync(0xffffffffu, q[0]), b1 = __ballot_sync(0xffffffffu, q[1]),
+                       b2 = __ballot_sync(0xffffffffu, q[2]), b3 = __ballot_sync(0xffffffffu, q[3]);
         const unsigned bi = __ballot_sync(0xffffffffu, indefinite);
+        const bool any = q[0] | q[1] | q[2] | q[3];
         // every lane stores the same words (one wavefront, no branch on the lane index)
         *reinterpret_cast<uint4*>(&s_ball[buf][w][0]) = make_uint4(b0, b1, b2, b3);
         s_indef[buf][w] = bi;
-        if (m) {  // only entries that reach some warp are hoisted
-            const Hoisted h = hoist(r0.x, r0.y, r2.x, r0.z, r2.y, r2.z, ox, oy, L_BIAS);
+        // the hoist itself is straight-line too (some lane of the warp needs it in practically every batch; a branch
+        // around it only adds a divergent region), only the stores are kept to the entries that reach some warp
+        const Hoisted h = hoist(r0.x, r0.y, r2.x, r0.z, r2.y, r2.z, ox, oy, L_BIAS);
+        if (any) {
             float4* d = reinterpret_cast<float4*>(&s_rec[buf][tid * REC]);
             d[0] = make_float4(h.A, h.B, h.C, h.F);
             d[1] = make_float4(h.D, h.E, r2.w, r3.x);

@@ -113,12 +113,13 @@ __device__ __forceinline__ TightBox tight_box_constants(float a, float b, float 
     return t;
 }
 
-// 4-bit quadrant mask of one (tile, Gaussian): bit (col + 2 band) is set when the alpha >= 1/255 ellipse can reach a
-// pixel of the 8x8 quadrant (columns 8 col .. 8 col + 7, rows 8 band .. 8 band + 7) -- Eq. 19-21 with 8-row bands,
-// evaluated for the two 8-pixel sub-columns.  (dxc, dyc) = centre relative to the tile corner.  Conservative by the
-// widening of tau and SPAN_EPS; a row band is hit iff an INTEGER row lies in [ymin, ymax] (PAPER.md:216 ceil/floor).
-__device__ __forceinline__ uint32_t quadrant_mask(float dxc, float dyc, float b, float det, float xstar, float ic, float ct) {
-    uint32_t m = 0;
+// Quadrant hits of one (tile, Gaussian): q[col + 2 band] is set when the alpha >= 1/255 ellipse can reach a pixel of
+// the 8x8 quadrant (columns 8 col .. 8 col + 7, rows 8 band .. 8 band + 7) -- Eq. 19-21 with 8-row bands, evaluated for
+// the two 8-pixel sub-columns.  (dxc, dyc) = centre relative to the tile corner.  Conservative by the widening of tau
+// and SPAN_EPS; a row band is hit iff an INTEGER row lies in [ymin, ymax] (PAPER.md:216 ceil/floor).  The four results
+// are predicates (they feed the warp ballots directly; no mask word is assembled and taken apart again).
+__device__ __forceinline__ void quadrant_hits(float dxc, float dyc, float b, float det, float xstar, float ic, float ct,
+                                              bool (&q)[4]) {
 #pragma unroll
     for (int col = 0; col < 2; col++) {
         const float x0 = 8.0f * col - dxc, x1 = x0 + 7.0f;      // Eq. 14, centre-relative
@@ -126,26 +127,11 @@ __device__ __forceinline__ uint32_t quadrant_mask(float dxc, float dyc, float b,
         const float du = fmaf(-det * xu, xu, ct), dl = fmaf(-det * xl, xl, ct);
         const float ymax = fmaf(fmaf(-b, xu, sqrtf(fmaxf(du, 0.0f))), ic, dyc + SPAN_EPS);   // Eq. 17 / 18 / Case C
         const float ymin = fmaf(fmaf(-b, xl, -sqrtf(fmaxf(dl, 0.0f))), ic, dyc - SPAN_EPS);
-        // misses (du or dl < 0) are folded into the comparison operands, so the whole test is straight-line selects
-        const float top = (fminf(du, dl) >= 0.0f) ? ymax : -1.0f;
-        const uint32_t h0 = floorf(fminf(top, 7.0f)) >= fmaxf(ymin, 0.0f) ? 1u : 0u;
-        const uint32_t h1 = floorf(fminf(top, 15.0f)) >= fmaxf(ymin, 8.0f) ? 4u : 0u;
-        m |= (h0 | h1) << col;
+        // misses (du or dl < 0) are folded into the comparison operand, so the whole test is straight-line selects
+        const float top = floorf((fminf(du, dl) >= 0.0f) ? ymax : -1.0f);   // floor(min(top, 7)) = min(floor(top), 7)
+        q[col] = fminf(top, 7.0f) >= fmaxf(ymin, 0.0f);
+        q[col + 2] = fminf(top, 15.0f) >= fmaxf(ymin, 8.0f);
     }
-    return m;
-}
-
-// The same tight box against the WHOLE 16x16 tile (one column of 16 pixels, rows 0..15): true when the alpha >= 1/255
-// ellipse can reach a pixel of the tile.  A superset of "quadrant_mask != 0" (a wider column and a taller band can
-// only widen the span), at a quarter of its cost: the first, cheap stage of the cull.
-__device__ __forceinline__ bool tile_reach(float dxc, float dyc, float b, float det, float xstar, float ic, float ct) {
-    const float x0 = -dxc, x1 = x0 + 15.0f;                     // Eq. 14, centre-relative
-    const float xu = fminf(fmaxf(xstar, x0), x1), xl = fminf(fmaxf(-xstar, x0), x1);
-    const float du = fmaf(-det * xu, xu, ct), dl = fmaf(-det * xl, xl, ct);
-    const float ymax = fmaf(fmaf(-b, xu, sqrtf(fmaxf(du, 0.0f))), ic, dyc + SPAN_EPS);   // Eq. 17 / 18 / Case C
-    const float ymin = fmaf(fmaf(-b, xl, -sqrtf(fmaxf(dl, 0.0f))), ic, dyc - SPAN_EPS);
-    const float top = (fminf(du, dl) >= 0.0f) ? ymax : -1.0f;
-    return floorf(fminf(top, 15.0f)) >= fmaxf(ymin, 0.0f);
 }
 
 // Rows [r0, r1] (tile-local, clamped to [0, 15]) of the tile column [ox + cx0, ox + cx1] that the ellipse can reach;

@@ -78,8 +78,13 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     L.st_pre = take(8 * ((Pz + 31) / 32 + 1));
     L.st_scan = take(8 * ((Pz + SCAN_WARP_TILE - 1) / SCAN_WARP_TILE + 1));
     L.st_depth = take(8 * 256 * L.n_depth_tiles * MAX_SORT_PASSES_DEPTH);
-    L.st_tile = take(8 * 256 * L.n_tile_tiles * (size_t)L.n_tile_passes);
+    // The look-back status words of the tile passes are sized by CAPACITY (2 KB per tile of the sorted array: 1.1 GB at
+    // the 1.1 G-entry capacity of the outdoor scene).  Small frames clear them with the rest of the control block; large
+    // (two-level) frames sort a few per cent of their capacity, so there duplicate_kernel clears exactly the words the
+    // passes of THIS frame will use and the block stays out of the memset.
+    if (!L.two_level) L.st_tile = take(8 * 256 * L.n_tile_tiles * (size_t)L.n_tile_passes);
     L.zero_end = o;
+    if (L.two_level) L.st_tile = take(8 * 256 * L.n_tile_tiles * (size_t)L.n_tile_passes);
     L.per_g = take(16 * Pz);
     L.rec = take(64 * Pz);
     L.gkeyA = take(8 * Pz);

@@ -592,6 +592,15 @@ duplicate_kernel(const Frame f, const Pointers p, unsigned long long* __restrict
     const unsigned long long n = p.ctrl->n_dup_eff;
     const uint32_t n_vis = (uint32_t)p.ctrl->n_vis;
     const uint32_t gx = (uint32_t)f.gx;
+    {   // clear the look-back status words of the tile passes that follow: only the tiles n entries occupy (api.cu make_layout)
+        const unsigned long long tile_n = (unsigned long long)SORT_THREADS * sort_items_for(f.max_dup);
+        const unsigned long long words = min((n + tile_n - 1) / tile_n + 1, (unsigned long long)p.n_tile_tiles) * 256ull;
+        for (int pass = 0; pass < f.n_tile_passes; pass++) {
+            unsigned long long* st = p.st_tile + (size_t)pass * p.n_tile_tiles * 256;
+            for (unsigned long long i = (unsigned long long)blockIdx.x * SORT_THREADS + tid; i < words; i += (unsigned long long)gridDim.x * SORT_THREADS)
+                st[i] = 0ull;
+        }
+    }
     for (unsigned long long chunk = blockIdx.x; chunk * DUP_TILE < n; chunk += gridDim.x) {
         const unsigned long long k0 = chunk * DUP_TILE;
         const uint32_t cn = (uint32_t)min((unsigned long long)DUP_TILE, n - k0);

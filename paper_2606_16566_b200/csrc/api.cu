@@ -20,7 +20,7 @@ void launch_preprocess(const Frame&, const Pointers&, const float*, const float*
 void launch_depth_sort(const Frame&, const Pointers&, int, cudaStream_t, int*);
 void launch_tile_grid(const Frame&, const Pointers&, uint32_t*, const Ctrl*, cudaStream_t, int*);
 void launch_scan_offsets(const Frame&, const Pointers&, int, int, cudaStream_t, int*);
-void launch_expand(const Frame&, const Pointers&, cudaStream_t, int*);
+void launch_expand(const Frame&, const Pointers&, int, cudaStream_t, int*);
 void launch_duplicate_and_tile_sort(const Frame&, const Pointers&, int, cudaStream_t, int*, cudaEvent_t);
 void launch_atomic_order_selftest(unsigned long long*, int, uint32_t, int, int, cudaStream_t);
 cudaError_t run_issue_peak(int, int, double*);
@@ -35,7 +35,7 @@ constexpr size_t ALIGN = 256;
 size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t ctrl, cctrl, diff, cdiff, st_pre, st_scan, st_depth, st_tile, zero_end;
+    size_t ctrl, cctrl, diff, cdiff, st_pre, st_scan, st_depth, st_tile, st_exp, zero_end;
     size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, desc, cranges, ccounts, entA, entB, cids, ids, total;
     size_t n_depth_tiles, n_tile_tiles;
     int gx, gy, n_tiles, tile_bits, n_tile_passes, diff_copies, diff_cells;
@@ -85,6 +85,7 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     if (!L.two_level) L.st_tile = take(8 * 256 * L.n_tile_tiles * (size_t)L.n_tile_passes);
     L.zero_end = o;
     if (L.two_level) L.st_tile = take(8 * 256 * L.n_tile_tiles * (size_t)L.n_tile_passes);
+    L.st_exp = take(L.two_level ? 8 * 64 * (((size_t)max_dup + EXP_SEG - 1) / EXP_SEG + 2) : 0);   // cleared by duplicate_kernel too
     L.per_g = take(16 * Pz);
     L.rec = take(64 * Pz);
     L.gkeyA = take(8 * Pz);
@@ -216,6 +217,7 @@ Pointers carve(void* ws, const Layout& L) {
     p.st_scan = reinterpret_cast<unsigned long long*>(b + L.st_scan);
     p.st_depth = reinterpret_cast<unsigned long long*>(b + L.st_depth);
     p.st_tile = reinterpret_cast<unsigned long long*>(b + L.st_tile);
+    p.st_exp = reinterpret_cast<unsigned long long*>(b + L.st_exp);
     p.per_g = reinterpret_cast<uint4*>(b + L.per_g);
     p.rec = reinterpret_cast<float4*>(b + L.rec);
     p.gkeyA = reinterpret_cast<unsigned long long*>(b + L.gkeyA);
@@ -405,7 +407,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
         launch_scan_offsets(fc, pc, f.cshift, g_n_sm, st, &launches);   // (2) prefix-sum offsets of the super-tile duplicates
         mark(4);
         launch_duplicate_and_tile_sort(fc, pc, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b) on super-tiles
-        launch_expand(f, p, st, &launches);                  // (3c) super-tile lists -> tile lists, written in place
+        launch_expand(f, p, g_n_sm, st, &launches);                 // (3c) super-tile lists -> tile lists, written in place
     } else {
         launch_scan_offsets(f, p, 0, g_n_sm, st, &launches);  // (2) prefix-sum offsets
         mark(4);

@@ -31,6 +31,8 @@ constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_WARP_TILE = 32 * SCAN_ITEMS;        // 256 depth-sorted Gaussians per offset-scan tile (one warp)
 constexpr unsigned long long FUSED_DUP_MAX = 4ull << 20;   // frames up to this capacity fuse the duplication into the first tile pass
+constexpr int EXP_SEG = 2048;                         // expand_kernel: super-tile list entries per chunk (8 warps x 8 x 32 lanes)
+constexpr int EXP_THREADS = 256;
 constexpr int DUP_TILE = 1024;                        // duplication chunk: output slots per staged set of depth ranks
 // keys per thread of the fused duplicate + first-tile-pass kernel (its tile also holds the staged ranks of a chunk)
 __host__ __device__ inline int dup_items_for(unsigned long long capacity) { return capacity <= (256ull << 10) ? 4 : 8; }
@@ -51,7 +53,7 @@ struct Ctrl {
 // The workspace holds TWO control blocks: `ctrl` (frame-level counters + the FINE tile grid: n_dup, overflow) and
 // `cctrl` (the same fields for the SUPER-TILE grid that duplication and sort run on: n_vis is copied there,
 // n_dup / tile_hist / tile_counter are the coarse ones).
-enum { TC_PRE = 0, TC_DEPTH0 = 1, TC_SCAN = 5, TC_TILE0 = 6 };
+enum { TC_PRE = 0, TC_DEPTH0 = 1, TC_SCAN = 5, TC_TILE0 = 6, TC_EXPAND = 10 };
 
 // Look-back status word: [63:62] flag, [61:0] value.
 constexpr unsigned long long ST_EMPTY = 0ull;
@@ -87,6 +89,7 @@ struct Pointers {           // device pointers carved from the workspace
     unsigned long long* st_scan;            // [scan tiles]   look-back status: duplicate offsets
     unsigned long long* st_depth;           // [4][depth sort tiles][256]
     unsigned long long* st_tile;            // [3][tile sort tiles][256]
+    unsigned long long* st_exp;             // [chunks of EXP_SEG super-tile entries][64] look-back status of expand_kernel (two-level frames)
     uint4* per_g;                           // [P] {rect01, rect23, depth bits, radius}
     float4* rec;                            // [P][4] 64-byte render record (layout: include/gs.h, gs_intermediates.record)
     unsigned long long* gkeyA;              // [P] (depth bits << 32 | id), compacted

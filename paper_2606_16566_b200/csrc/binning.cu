@@ -800,7 +800,7 @@ void launch_duplicate_and_tile_sort(const Frame& f, const Pointers& p, int n_sm,
 __device__ __forceinline__ uint32_t spread4(uint32_t x) { return ((x & 15u) * 0x00204081u) & 0x01010101u; }   // bit i -> byte i
 
 template <int SH>
-__global__ void __launch_bounds__(EXP_THREADS)
+__global__ void __launch_bounds__(EXP_THREADS, 4)
 expand_kernel(const Frame f, const Pointers p) {
     static_assert(SH == 3, "the tile masks are 64-bit: 8 x 8 tiles per super-tile");
     constexpr int SUPER = 8;
@@ -908,12 +908,26 @@ expand_kernel(const Frame f, const Pointers p) {
                 unsigned long long* st = p.st_exp + (size_t)g * 64 + t;
                 if (goes_on && from_before) st_status(st, ST_AGG | (unsigned long long)run);
                 unsigned long long prev = 0;
-                if (from_before) {                       // entries of this super-tile in the chunks before this one
-                    for (uint32_t idx = g - 1;; idx--) {
-                        unsigned long long v;
-                        do { v = ld_status(p.st_exp + (size_t)idx * 64 + t); } while ((v >> 62) == 0);
-                        prev += v & ST_MASK;
-                        if ((v >> 62) == 2) break;       // the chunk the super-tile starts in publishes an inclusive prefix
+                if (from_before) {
+                    // entries of this super-tile in the chunks before this one: back to the nearest inclusive prefix (the
+                    // chunk the super-tile starts in publishes one at once), EXP_LB status words in flight per round trip
+                    // -- a super-tile of the outdoor scene fills 76 chunks, most of them in flight in the same wave
+                    constexpr int EXP_LB = 16;
+                    const uint32_t g_first = cbeg / EXP_SEG;
+                    uint32_t idx = g - 1;
+                    bool done = false;
+                    while (!done) {
+                        unsigned long long sv[EXP_LB];
+#pragma unroll
+                        for (int k = 0; k < EXP_LB; k++)
+                            sv[k] = (idx >= g_first + (uint32_t)k) ? ld_status(p.st_exp + (size_t)(idx - k) * 64 + t) : ST_INC;
+#pragma unroll
+                        for (int k = 0; k < EXP_LB; k++) {
+                            if (done || (sv[k] >> 62) == 0) break;   // not published yet: poll again from here
+                            prev += sv[k] & ST_MASK;
+                            idx--;
+                            done = (sv[k] >> 62) == 2;
+                        }
                     }
                 }
                 if (goes_on) st_status(st, ST_INC | (prev + run));
@@ -944,9 +958,10 @@ expand_kernel(const Frame f, const Pointers p) {
                         for (int c = 0; c < 8; c++) {
                             const bool hit = (rowbyte >> c) & 1u;
                             const unsigned bal = __ballot_sync(0xffffffffu, hit);
+                            const uint32_t rank = __popc(bal & lt);
                             if (hit) {
-                                GS_BOUND(slot[c] + __popc(bal & lt), f.max_dup);
-                                p.ids[slot[c] + __popc(bal & lt)] = my_id;
+                                GS_BOUND(slot[c] + rank, f.max_dup);
+                                p.ids[slot[c] + rank] = my_id;
                             }
                             slot[c] += __popc(bal);
                         }
@@ -967,7 +982,9 @@ expand_kernel(const Frame f, const Pointers p) {
 
 void launch_expand(const Frame& f, const Pointers& p, int n_sm, cudaStream_t st, int* launches) {
     const long long cap_chunks = ((long long)f.max_dup + EXP_SEG - 1) / EXP_SEG;
-    launch_pdl(expand_kernel<SUPER_SHIFT>, dim3(imin(cap_chunks > 0 ? cap_chunks : 1, (long long)n_sm * 4)), dim3(EXP_THREADS), st, f, p);
+    // three blocks per SM measured best (two to five tried): with more chunks in flight the look-back chains of the long
+    // super-tile lists get deeper and the store streams of a tile list interleave more
+    launch_pdl(expand_kernel<SUPER_SHIFT>, dim3(imin(cap_chunks > 0 ? cap_chunks : 1, (long long)n_sm * 3)), dim3(EXP_THREADS), st, f, p);
     (*launches)++;
 }
 

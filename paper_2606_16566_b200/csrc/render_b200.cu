@@ -162,25 +162,22 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
     const uint32_t raw_w = (uint32_t)__cvta_generic_to_shared(&s_raw[w * 32 * 64]);
     // this thread's own raw record: chunk c sits at raw_me ^ (c << 4) (the swizzle above, (lane >> 1) & 3 for record `lane`)
     const uint32_t raw_me = raw_w + lane * 64 + (((uint32_t)(lane >> 1) & 3u) << 4);
-    auto gather = [&](const uint32_t id_mine, const uint32_t n_valid /* entries of this warp in the batch */) {
+    // Unconditional: a slot past the end of the list copies the record of whatever valid id its lane still holds (0 or an
+    // id of the previous batch -- a cache hit, masked out at staging); four predicates and their compares per batch saved.
+    auto gather = [&](const uint32_t id_mine) {
 #pragma unroll
         for (int k = 0; k < 4; k++) {
             const int j = 8 * k + (lane >> 2), c = lane & 3;
             const uint32_t id = __shfl_sync(0xffffffffu, id_mine, j);
-            if ((uint32_t)j < n_valid)
-                cp_async16(raw_w + j * 64 + ((c ^ ((j >> 1) & 3)) << 4), rec + 4 * (size_t)id + c);
+            cp_async16(raw_w + j * 64 + ((c ^ ((j >> 1) & 3)) << 4), rec + 4 * (size_t)id + c);
         }
         cp_async_commit();
-    };
-    auto warp_valid = [&](const uint32_t base) -> uint32_t {   // how many entries of batch `base` fall to this warp
-        const uint32_t first = base + 32u * (uint32_t)w;
-        return first < end ? min(32u, end - first) : 0u;
     };
     // ---- software pipeline prologue: records of batch 0 (in flight), ids of batch 1 -------------------------------------
     uint32_t id_next = 0;
     {
         const uint32_t id0 = (start + tid < end) ? ids[start + tid] : 0u;
-        gather(id0, warp_valid(start));
+        if (start < end) gather(id0);
     }
     if (start + QB + tid < end) id_next = ids[start + QB + tid];
     int buf = 0;
@@ -216,7 +213,7 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
         }
         // ---- gather of the next batch into the raw slots just consumed (the hoist above read them), ids of the one after ---
         __syncwarp();
-        if (base + QB < end) gather(id_next, warp_valid(base + QB));
+        if (base + QB < end) gather(id_next);
         if (base + 2 * QB + tid < end) id_next = ids[base + 2 * QB + tid];
         // ---- the batch's only barrier; also the block-level exit (every warp of the tile finished, Eq. 22) ----------
         if (__syncthreads_and(wdone)) break;

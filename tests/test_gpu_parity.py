@@ -419,6 +419,52 @@ def test_two_level_binning_edge_cases():
     print(pu.compare(r, it, ref))
 
 
+def _same_frame(sc, caps=(3 << 20, 5 << 20)):
+    """Renders sc with a one-level and a two-level workspace; every list, range and pixel must be identical."""
+    res = []
+    for cap in caps:
+        r = pu.run_gpu(sc, 0, max_dup=cap, count_contrib=True)
+        it = r.intermediates(copy=("per_gaussian", "tile_ranges", "sorted_ids"))
+        assert it.n_dup <= caps[0]
+        assert (it.n_coarse > 0) == (cap > 4 << 20)
+        res.append((r, it))
+    (r1, i1), (r2, i2) = res
+    assert i1.n_dup == i2.n_dup
+    assert np.array_equal(i1.tile_ranges, i2.tile_ranges) and np.array_equal(i1.sorted_ids, i2.sorted_ids)
+    assert torch.equal(r1.out_rgb, r2.out_rgb) and torch.equal(r1.out_n_contrib, r2.out_n_contrib)
+    return r2, i2
+
+
+def test_expand_kernel_chunk_and_piece_edges():
+    """expand_kernel cuts the sorted super-tile entries into chunks of 2 048, whatever super-tiles they belong to, and chains
+    the chunks of one super-tile by look-back.  Adversarial list shapes, each against the one-level sort of the same frame:
+    (a) every super-tile list exactly one chunk long (piece boundaries ON chunk boundaries), (b) lists of 5 000 (boundaries inside
+    chunks, a chunk holding the tail of one list and the head of the next), (c) ONE super-tile list of 40 000 entries (20 chunks
+    chained by look-back), (d) 64 super-tiles of ~50 entries each (dozens of pieces per chunk)."""
+    rng = np.random.default_rng(5)
+
+    def blanket(P, W, H):   # P faint Gaussians that each cover the whole W x H image, distinct depths
+        z = rng.uniform(3.0, 6.0, P)
+        means = np.stack([rng.uniform(-0.2, 0.2, P), rng.uniform(-0.2, 0.2, P), z], 1)
+        return scenes.single_gaussian_scene(means, [40.0, 40.0, 40.0], [1, 0, 0, 0], 0.004, rng.uniform(0, 1, (P, 3)), [0.1, 0.2, 0.3],
+                                            W, H, 100.0, 100.0)
+    # (a) 256 x 256 = 2 x 2 super-tiles, 2 048 entries each
+    r, it = _same_frame(blanket(2048, 256, 256))
+    assert it.n_coarse == 4 * 2048 and it.n_dup == 2048 * 256
+    # (b) 5 000 entries per super-tile list: 20 000 entries, 10 chunks, every piece boundary inside a chunk
+    r, it = _same_frame(blanket(5000, 256, 256))
+    assert it.n_coarse == 4 * 5000
+    # (c) one super-tile (128 x 128), 40 000 entries: 20 chunks of one list
+    r, it = _same_frame(blanket(40_000, 128, 128))
+    assert it.n_coarse == 40_000 and it.n_dup == 40_000 * 64
+    # (d) many short lists: 1 024 x 1 024 = 8 x 8 super-tiles, 3 000 small Gaussians; also against the oracle
+    sc = scenes.make_scene(1, P=3000, W=1024, H=1024, f=800.0)
+    r, it = _same_frame(sc)
+    assert 0 < it.n_coarse < 2 * 2048 * 4
+    ref = oracle.render(sc, 0, n_threads=8, fragile_delta=pu.DELTA)
+    print(pu.compare(r, it, ref))
+
+
 def test_overlapped_scene_upload_switches_buffer_sets_safely():
     """Renderer.upload_async() fills a second set of scene buffers on an upload stream while frames are rendered from the
     active one; activate_uploaded() switches.  Alternating two DIFFERENT scenes of the same size through it must give, for

@@ -465,6 +465,44 @@ def test_expand_kernel_chunk_and_piece_edges():
     print(pu.compare(r, it, ref))
 
 
+def test_two_level_workspace_reused_across_frames_of_different_size():
+    """On two-level frames the look-back status words of the tile passes and of expand_kernel are not part of the per-frame
+    memset: duplicate_kernel clears the words THIS frame's entry count needs.  One workspace, a sequence of frames whose
+    sorted level grows and shrinks (a pulled-back pose with 1.5x the entries between the scene's own poses): every frame must
+    equal the frame a fresh renderer produces -- a stale status word read as "published" would corrupt the sort or the offsets."""
+    sc = scenes.make_scene(3, P=200_000, W=1264, H=832, poses=4)
+    cams = list(sc.cameras)
+    V = np.array(cams[0].viewmatrix, dtype=np.float64, copy=True)   # the same camera pulled back: more of the scene in view
+    V[2, 3] += 30.0
+    far = scenes.make_camera(V, cams[0].fx, cams[0].fy, cams[0].W, cams[0].H)
+    seq = [cams[0], far, cams[1], far, cams[2], cams[0]]
+    cap = 12 << 20
+    want = {}
+    for cam in seq:
+        if id(cam) in want:
+            continue
+        r0 = Renderer(sc.P, cam.W, cam.H, cap, device="cuda:0", count_contrib=True)
+        r0.upload(sc)
+        r0.render(cam)
+        torch.cuda.synchronize()
+        it = r0.intermediates(copy=("tile_ranges", "sorted_ids"))
+        assert it.n_coarse > 0
+        want[id(cam)] = (it.n_coarse, it.tile_ranges.copy(), it.sorted_ids[: it.n_dup].copy(), r0.out_rgb.clone())
+        del r0
+    sizes = [want[id(c)][0] for c in seq]
+    assert min(sizes) * 1.5 < max(sizes), sizes               # the sequence really grows and shrinks (radix tiles: 4 096 entries)
+    r = Renderer(sc.P, cams[0].W, cams[0].H, cap, device="cuda:0", count_contrib=True)
+    r.upload(sc)
+    for cam in seq:
+        r.render(cam)
+        torch.cuda.synchronize()
+        it = r.intermediates(copy=("tile_ranges", "sorted_ids"))
+        n_coarse, ranges, ids, rgb = want[id(cam)]
+        assert it.n_coarse == n_coarse
+        assert np.array_equal(it.tile_ranges, ranges) and np.array_equal(it.sorted_ids[: it.n_dup], ids)
+        assert torch.equal(r.out_rgb, rgb)
+
+
 def test_overlapped_scene_upload_switches_buffer_sets_safely():
     """Renderer.upload_async() fills a second set of scene buffers on an upload stream while frames are rendered from the
     active one; activate_uploaded() switches.  Alternating two DIFFERENT scenes of the same size through it must give, for

@@ -33,6 +33,7 @@ extern "C" {
 #define GS_ERR_WORKSPACE (-2) /* workspace_bytes < gs_workspace_bytes(P, W, H, max_dup) or misaligned pointer    */
 #define GS_ERR_OVERFLOW (-3)  /* reported by gs_get_intermediates: the frame needed more than max_dup duplicates */
 #define GS_ERR_CUDA (-4)      /* a CUDA runtime call failed; gs_last_cuda_error() returns its cudaError_t        */
+#define GS_ERR_LIMIT (-5)     /* gs_depth_sort_noalloc: more keys than the fixed scratch holds (GS_NOALLOC_MAX_KEYS) */
 
 #define GS_TILE 16            /* tile edge in pixels                                         */
 
@@ -206,6 +207,27 @@ int gs_selftest_atomic_order(int iters, uint64_t out[2]);
  * synchronous, default stream) -- and returns THREAD-OPERATIONS per second: out[0] FFMA, out[1] FFMA2 (two FP32
  * operations per lane and instruction), out[2] MUFU.EX2.  Uses 16 bytes of private device scratch. */
 int gs_selftest_issue_peak(int iters, double out[3]);
+
+/* Depth sort WITHOUT any allocation -- for callers that cannot call cudaMalloc (code under CUDA stream capture, tight
+ * serving loops, harnesses that forbid it).  The operation is the depth sort of the binning stage ("sorts them
+ * by tile index and depth"; four stable 8-bit LSD radix passes over the depth bits, before duplication):
+ *   keys_out[0..n) = keys_in[0..n) in ascending order of bits 63..32, STABLE (keys whose high words are equal keep their
+ *   input order; bits 31..0 are carried along) -- with keys (depth bits << 32 | Gaussian id) in id order this is the
+ *   (depth, id) order of gs_intermediates.depth_sorted.
+ * keys_in, keys_out: dev, n 64-bit keys each, 8-byte aligned, distinct buffers on the CURRENT device (GS_ERR_BAD_ARG
+ * otherwise); keys_in is only read.  Enqueued on `cuda_stream` (one memset node, 5 kernels); no host synchronisation.
+ * The passes are the radix_pass_kernel of gs_render; their scratch (ping-pong keys, digit histograms, tile counters,
+ * look-back status words) is a static __device__ array of 4.2 MB that every GPU that loads the library holds until the
+ * process exits.  Hence the LIMIT: n <= GS_NOALLOC_MAX_KEYS (= gs_noalloc_max_keys()); a larger n returns GS_ERR_LIMIT
+ * and enqueues nothing; n == 0 returns GS_OK and enqueues nothing.  The call makes no cudaMalloc / cudaFree / stream or
+ * event creation; its first call on a device looks up the array's address (cudaGetSymbolAddress) and the SM count.
+ * Ranking uses the ballot multi-split (gs_set_rank_mode(1) semantics), which needs no self-test.
+ * ALL calls share the one array per device: two calls that overlap on the GPU (different streams, or graphs launched
+ * concurrently) race -- order them on one stream or with events.  The array keeps the last call's contents; the call
+ * itself clears what must start at zero. */
+#define GS_NOALLOC_MAX_KEYS 262144
+uint32_t gs_noalloc_max_keys(void);
+int gs_depth_sort_noalloc(const uint64_t* keys_in, uint64_t* keys_out, uint32_t n, void* cuda_stream);
 
 /* Synchronous device->host copy of `bytes` bytes (a plain cudaMemcpy) -- lets a binding without CUDA runtime access
  * read the arrays gs_get_intermediates() points at. */

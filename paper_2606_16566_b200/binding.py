@@ -16,7 +16,8 @@ import torch
 
 from . import build as _build
 
-GS_OK, GS_ERR_BAD_ARG, GS_ERR_WORKSPACE, GS_ERR_OVERFLOW, GS_ERR_CUDA = 0, -1, -2, -3, -4
+GS_OK, GS_ERR_BAD_ARG, GS_ERR_WORKSPACE, GS_ERR_OVERFLOW, GS_ERR_CUDA, GS_ERR_LIMIT = 0, -1, -2, -3, -4, -5
+GS_NOALLOC_MAX_KEYS = 262144   # include/gs.h: key capacity of gs_depth_sort_noalloc's fixed scratch
 GS_TILE = 16
 GS_DEFAULT_RENDER_VARIANT = 4   # include/gs.h: the B200 render kernel
 GS_N_TIMINGS = 8
@@ -26,7 +27,8 @@ EXPORTS = ("gs_workspace_bytes", "gs_render", "gs_get_intermediates", "gs_set_ti
            "gs_set_render_variant", "gs_get_render_variant", "gs_last_launch_count", "gs_error_string",
            "gs_last_cuda_error", "gs_copy_to_host", "gs_set_stats", "gs_get_stats", "gs_selftest_atomic_order",
            "gs_set_render_stream", "gs_selftest_issue_peak", "gs_set_tile_cull", "gs_get_tile_cull",
-           "gs_set_workspace_option", "gs_release", "gs_set_rank_mode", "gs_get_rank_mode", "gs_set_graph")
+           "gs_set_workspace_option", "gs_release", "gs_set_rank_mode", "gs_get_rank_mode", "gs_set_graph",
+           "gs_noalloc_max_keys", "gs_depth_sort_noalloc")
 GS_OPT_RENDER_VARIANT, GS_OPT_TILE_CULL, GS_OPT_TIMING, GS_OPT_STATS, GS_OPT_RENDER_STREAM, GS_OPT_GRAPH = range(6)
 GS_N_STATS = 4
 STATS_NAMES = ("warp_slots_walked", "pairs_blended", "entries_staged", "pairs_evaluated")
@@ -101,6 +103,10 @@ def lib():
         L.gs_set_tile_cull.restype = C.c_int
         L.gs_set_tile_cull.argtypes = [C.c_int]
         L.gs_get_tile_cull.restype = C.c_int
+        L.gs_noalloc_max_keys.restype = C.c_uint32
+        L.gs_noalloc_max_keys.argtypes = []
+        L.gs_depth_sort_noalloc.restype = C.c_int
+        L.gs_depth_sort_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
         L.gs_selftest_issue_peak.restype = C.c_int
         L.gs_selftest_issue_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.gs_selftest_atomic_order.restype = C.c_int
@@ -246,6 +252,26 @@ def gs_selftest_issue_peak(iters: int = 2000) -> dict:
     if rc != GS_OK:
         raise GsError(rc, "gs_selftest_issue_peak")
     return {"ffma": float(out[0]), "ffma2": float(out[1]), "ex2": float(out[2])}
+
+
+def gs_noalloc_max_keys() -> int:
+    return int(lib().gs_noalloc_max_keys())
+
+
+def gs_depth_sort_noalloc(keys_in, keys_out, n: int = None, stream=None) -> None:
+    """keys_out[:n] = keys_in[:n] sorted ascending by bits 63..32, stable (include/gs.h).  keys_in / keys_out: distinct
+    contiguous int64 CUDA tensors (the 64-bit keys' bit patterns).  Allocates nothing; n <= GS_NOALLOC_MAX_KEYS, else
+    GsError(GS_ERR_LIMIT).  All calls share one static device scratch: do not overlap them on the GPU."""
+    import torch
+    if n is None:
+        n = keys_in.numel()
+    for t in (keys_in, keys_out):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.int64 and t.numel() >= min(n, GS_NOALLOC_MAX_KEYS)):
+            raise ValueError("gs_depth_sort_noalloc: contiguous int64 CUDA tensors of at least n elements expected")
+    st = stream if stream is not None else torch.cuda.current_stream(keys_in.device)
+    rc = lib().gs_depth_sort_noalloc(C.c_void_p(keys_in.data_ptr()), C.c_void_p(keys_out.data_ptr()), int(n), C.c_void_p(st.cuda_stream))
+    if rc != GS_OK:
+        raise GsError(rc, "gs_depth_sort_noalloc(n = %d, limit %d)" % (n, GS_NOALLOC_MAX_KEYS))
 
 
 def gs_set_workspace_option(workspace, option: int, value: int) -> None:

@@ -24,6 +24,7 @@ UNITS = {
     "preprocess.cu": ["-fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false"],
     "binning.cu": [],
     "selftest.cu": [],
+    "noalloc.cu": [],
     "render.cu": ["-use_fast_math"],
     "render_b200.cu": ["-use_fast_math"],
 }

@@ -263,6 +263,11 @@ bool fit_max_dup(int P, int W, int H, size_t bytes, unsigned long long& max_dup)
 
 }  // namespace
 
+namespace gs {
+// lets the other translation units of the library (noalloc.cu) record a CUDA error for gs_last_cuda_error()
+int record_cuda_error(cudaError_t e) { return cuda_fail(e); }
+}  // namespace gs
+
 extern "C" {
 
 size_t gs_workspace_bytes(int P, int W, int H, uint64_t max_dup) {
@@ -723,6 +728,7 @@ const char* gs_error_string(int code) {
         case GS_ERR_WORKSPACE: return "workspace too small or misaligned";
         case GS_ERR_OVERFLOW: return "more duplicated entries than the workspace capacity (max_dup)";
         case GS_ERR_CUDA: return "CUDA runtime error (see gs_last_cuda_error)";
+        case GS_ERR_LIMIT: return "more keys than the fixed scratch of gs_depth_sort_noalloc holds (GS_NOALLOC_MAX_KEYS)";
         default: return "unknown error";
     }
 }

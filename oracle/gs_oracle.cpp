@@ -39,6 +39,7 @@ struct Pre {  // per-Gaussian outputs of C-P (all zero when culled)
     std::vector<uint32_t> depth_bits, tiles_touched;
     std::vector<int32_t> radius, rect;
     std::vector<float> mu, conic, rgb, opacity;
+    std::vector<float> tau;   // C-P8': the upper bound of 2 ln(255 o) the tile-cull modes use (0 in the standard mode)
 };
 
 inline uint32_t f2u(float f) { uint32_t u; std::memcpy(&u, &f, 4); return u; }
@@ -87,7 +88,8 @@ struct Frame {
     const float *means, *scales, *rots, *opac, *sh, *V, *PM;
     float fx, fy;
     double campos[3];
-    int tile_cull = 0;   // 0: standard 3-sigma square rect (C-P8); 1: intersected with the AABB of the alpha >= 1/255 ellipse (C-P8')
+    int tile_cull = 0;   // 0: standard 3-sigma square rect (C-P8); 1: intersected with the AABB of the alpha >= 1/255 ellipse (C-P8');
+                         // 2: that rect, and a (tile, Gaussian) pair is listed only if tile_hit() below holds (C-P8'')
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -174,6 +176,7 @@ void preprocess_one(const Frame& f, int i, Pre& o) {
     // C-P8 tile rectangle, half-open, clamped to the grid                            (reading S6)
     const float rf = (float)radius;
     float rxf = rf, ryf = rf;
+    float tau_out = 0.0f;
     if (f.tile_cull) {
         // C-P8' ("tighter tile culling", off by default): the square is intersected with the axis-aligned
         // bounding box of the ellipse alpha >= 1/255, i.e. a dx^2 + 2 b dx dy + c dy^2 <= tau, tau = 2 ln(255 o)
@@ -190,6 +193,7 @@ void preprocess_one(const Frame& f, int i, Pre& o) {
         std::memcpy(&m, &mb, 4);
         const float lnm = (m - 1.0f) / std::sqrt(m);
         const float tau = (2.0f * (((float)e2 * 0.693147182f) + lnm)) + 1e-5f;
+        tau_out = tau;
         const double dd = ((double)ca * (double)cc) - ((double)cb * (double)cb);
         if (dd > 0.0 && ca > 0.0f && cc > 0.0f) {
             const double hx = std::sqrt(((double)tau * (double)cc) / dd), hy = std::sqrt(((double)tau * (double)ca) / dd);
@@ -227,6 +231,7 @@ void preprocess_one(const Frame& f, int i, Pre& o) {
     o.conic[3 * (size_t)i + 1] = cb;
     o.conic[3 * (size_t)i + 2] = cc;
     o.opacity[i] = f.opac[i];
+    o.tau[i] = tau_out;
 }
 
 bool make_frame(Frame& f, int P, const float* means, const float* scales, const float* rots, const float* opac,
@@ -247,11 +252,43 @@ void alloc_pre(Pre& o, int P) {
     o.depth_bits.assign(P, 0); o.tiles_touched.assign(P, 0); o.radius.assign(P, 0); o.rect.assign(4 * (size_t)P, 0);
     o.mu.assign(2 * (size_t)P, 0.f); o.conic.assign(3 * (size_t)P, 0.f); o.rgb.assign(3 * (size_t)P, 0.f);
     o.opacity.assign(P, 0.f);
+    o.tau.assign(P, 0.f);
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // C-R: per-pixel blend, termination rule R1 = the paper's BASELINE column (reading S11).
 // ---------------------------------------------------------------------------------------------------------
+// C-P8'' (SURVEY.md 8(f) N2 "exact ellipse-tile intersection"; flag TILE_CULL_EXACT, off by default): does the ellipse
+//   E = { a dx^2 + 2 b dx dy + c dy^2 <= tau_e },  (dx, dy) relative to the 2-D mean,  tau_e = tau + 0.05
+// (tau: the upper bound of 2 ln(255 o) of C-P8'; PAPER.md:181 alpha >= 1/255) meet the box of pixel CENTRES of tile
+// (tx, ty), [16 tx, 16 tx + 15] x [16 ty, 16 ty + 15]?  E restricted to the row band is convex, so the tile is met iff the
+// x-extent of that restriction reaches the tile's columns.  The extent comes from the paper's tight box (Eq. 13-18) with
+// the roles of x and y exchanged: the right-most point of E lies at dy* = -b h_x / c, h_x = sqrt(tau_e c / det); over the
+// band dy in [d0, d1] the right boundary x(dy) = (-b dy + sqrt(a tau_e - det dy^2)) / a is concave, so its maximum is at
+// clamp(dy*, d0, d1) (the left boundary: convex, minimum at clamp(-dy*, d0, d1)).  fp32, ONE rounding per operation in
+// this order (the CUDA side restates it with __f*_rn intrinsics): the decision is an integer and must be bit-identical.
+// Every "miss" is an affirmative comparison, so a NaN keeps the tile; the 0.05 added to tau (>= 4e-3 relative) covers the
+// fp32 rounding of the pixel-to-centre differences (<= 5e-4 px at 8 K) and of the discriminants (1e-6 relative).
+bool tile_hit(const Pre& pre, int i, int tx, int ty) {
+    const float a = pre.conic[3 * (size_t)i], b = pre.conic[3 * (size_t)i + 1], c = pre.conic[3 * (size_t)i + 2];
+    const float mux = pre.mu[2 * (size_t)i], muy = pre.mu[2 * (size_t)i + 1];
+    const float det = (a * c) - (b * b);
+    if (!(det > 0.0f) || !(a > 0.0f) || !(c > 0.0f)) return true;      // degenerate conic: keep everything
+    const float te = pre.tau[i] + 0.05f;
+    const float at = a * te;
+    const float hx = std::sqrt((te * c) / det);
+    const float ys = ((-b) * hx) / c;                                  // dy of the right-most point; the left-most is at -ys
+    const float d0 = (float)(16 * ty) - muy, d1 = d0 + 15.0f;          // the band, relative to the mean
+    const float yu = std::fmin(std::fmax(ys, d0), d1), yl = std::fmin(std::fmax(-ys, d0), d1);
+    const float du = at - ((det * yu) * yu), dl = at - ((det * yl) * yl);
+    if (du < 0.0f || dl < 0.0f) return false;                          // the band misses the ellipse
+    const float xmax = (((-b) * yu) + std::sqrt(std::fmax(du, 0.0f))) / a;
+    const float xmin = (((-b) * yl) - std::sqrt(std::fmax(dl, 0.0f))) / a;
+    const float e0 = (float)(16 * tx) - mux, e1 = e0 + 15.0f;          // the tile's columns, relative to the mean
+    if (xmax < e0 || xmin > e1) return false;
+    return true;
+}
+
 struct PixelOut {
     double C[3], T;
     uint32_t n, last_k;
@@ -322,7 +359,7 @@ gs_oracle_result* gs_oracle_render(int P, const float* means3D, const float* sca
     if (!make_frame(f, P, means3D, scales, rotations, opacities, sh_coeffs, sh_degree, viewmatrix, projmatrix, fx, fy, W, H))
         return nullptr;
     if (!bg) return nullptr;
-    f.tile_cull = (flags & GS_ORACLE_TILE_CULL) ? 1 : 0;
+    f.tile_cull = (flags & GS_ORACLE_TILE_CULL_EXACT) ? 2 : ((flags & GS_ORACLE_TILE_CULL) ? 1 : 0);
     gs_oracle_result* r = new gs_oracle_result();
     r->f = f;
     const int n_tiles = f.gx * f.gy;
@@ -351,8 +388,11 @@ gs_oracle_result* gs_oracle_render(int P, const float* means3D, const float* sca
         if (!pre.tiles_touched[i]) continue;
         const int32_t* rc = &pre.rect[4 * (size_t)i];
         for (int ty = rc[1]; ty < rc[3]; ty++)
-            for (int tx = rc[0]; tx < rc[2]; tx++) r->tile_counts[(size_t)ty * f.gx + tx]++;
-        r->n_dup += pre.tiles_touched[i];
+            for (int tx = rc[0]; tx < rc[2]; tx++) {
+                if (f.tile_cull == 2 && !tile_hit(pre, i, tx, ty)) continue;
+                r->tile_counts[(size_t)ty * f.gx + tx]++;
+            }
+        r->n_dup += pre.tiles_touched[i];   // the rect area in every mode: the capacity a frame needs
     }
     r->list_offsets.assign(n_lists + 1, 0);
     if (!(flags & GS_ORACLE_NO_LISTS)) {
@@ -364,6 +404,7 @@ gs_oracle_result* gs_oracle_render(int P, const float* means3D, const float* sca
             const int32_t* rc = &pre.rect[4 * (size_t)i];
             for (int ty = rc[1]; ty < rc[3]; ty++)
                 for (int tx = rc[0]; tx < rc[2]; tx++) {
+                    if (f.tile_cull == 2 && !tile_hit(pre, i, tx, ty)) continue;
                     const int32_t l = slot[(size_t)ty * f.gx + tx];
                     if (l >= 0) r->sorted_ids[cursor[l]++] = (uint32_t)i;
                 }

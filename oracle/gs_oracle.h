@@ -56,6 +56,11 @@ typedef struct gs_oracle_view {
 #define GS_ORACLE_TILE_CULL 4   /* C-P8': tile rect intersected with the AABB of the alpha >= 1/255 ellipse;
                                    off by default -- every pin of the standard definition uses the 3-sigma square */
 
+#define GS_ORACLE_TILE_CULL_EXACT 8 /* C-P8'': the C-P8' rect, and a (tile, Gaussian) pair is counted and listed only if the
+                                   ellipse alpha >= 1/255 (widened) meets the tile's box of pixel centres (exact
+                                   ellipse-tile test).  tile_counts and the lists shrink; rect,
+                                   tiles_touched and n_dup stay those of C-P8' */
+
 /* Runs the oracle.  tile_subset == NULL: all tiles (full).  Otherwise only the n_subset listed tiles get
  * lists and pixels; per-Gaussian outputs and tile_counts always cover everything.
  * n_threads <= 1: single-threaded (the definitional baseline); > 1: the per-list stable sorts of C-B and the tiles of

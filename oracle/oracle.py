@@ -12,6 +12,7 @@ from . import build_oracle
 NO_RENDER = 1
 NO_LISTS = 2
 TILE_CULL = 4
+TILE_CULL_EXACT = 8   # C-P8'': TILE_CULL's rect + exact ellipse-tile test per (tile, Gaussian)
 
 _u32p, _i32p, _f32p, _u64p, _u8p = (C.POINTER(t) for t in (C.c_uint32, C.c_int32, C.c_float, C.c_uint64, C.c_uint8))
 

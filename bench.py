@@ -9,7 +9,7 @@ all five configurations are measured, each with its own W warm-up and K timed st
 `roofline`, `e2e` and `cpu_baseline` are those of configs[4] (10 M Gaussians, 3840x2160: the largest single-GPU
 workload, whose sort and render times BASELINE.json wants reported separately) and `per_config` holds the same fields
 for every configuration.  All five fit one GPU (config 4 needs ~21.5 GB of workspace).  With --config C only that one is
-measured and it is the headline.  Every configuration also gets a companion entry `with_tile_cull`: the same measurement
+measured and it is the headline.  Every configuration also gets a companion entry `with_tile_cull` (configs 3-5 also `with_exact_tile_cull`, gs_set_tile_cull(2)): the same measurement
 (no e2e, no CPU baseline) with gs_set_tile_cull(1) -- tighter tile rects, same image; the top-level
 numbers are always the standard 3-sigma rect of BASELINE.json's north_star.
 `value` = frames/s with the scene resident in HBM, device-timed (CUDA events on the launching stream around every step,
@@ -288,7 +288,9 @@ def measure_config(config, args, ctx, tile_cull=None, light=False):
         return replica_max(x, ws, dev)
 
     # ---- size the workspace: largest N_dup over the poses (+5 %) -----------------------------------------------------
-    max_dup, need = 1 << 21, 0
+    # gs_set_tile_cull(2) culls where the super-tile lists are expanded: it needs the two-level binning (capacity > 4 Mi entries)
+    min_dup = (5 << 20) if binding.gs_get_tile_cull() == 2 else 0
+    max_dup, need = max(1 << 21, min_dup), 0
     graph = None if args.graph < 0 else bool(args.graph)
     r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True, graph=graph)
     r.upload(pinned)
@@ -304,7 +306,7 @@ def measure_config(config, args, ctx, tile_cull=None, light=False):
     if need > max_dup or overflowed:
         del r
         torch.cuda.empty_cache()
-        max_dup = int(need * 1.05) + 4096
+        max_dup = max(int(need * 1.05) + 4096, min_dup)
         r = Renderer(sc.P, W, H, max_dup, device=dev, count_contrib=True, graph=graph)
         r.upload(pinned)
     # ---- statistics pass (untimed): units of the rooflines -------------------------------------------------------------
@@ -314,7 +316,7 @@ def measure_config(config, args, ctx, tile_cull=None, light=False):
         r.render(cam, count_contrib=True)
         stats.append(binding.gs_get_stats(r.workspace))
         it = r.intermediates(copy=())
-        per_pose.append((it.n_visible, it.n_dup, it.n_coarse))
+        per_pose.append((it.n_visible, it.n_dup, it.n_coarse, int(r.out_tile_counts.sum().item())))
         max_dup = int(it.max_dup)   # the capacity the library recovered from the workspace size
     binding.gs_set_stats(False)
     launches_per_frame = binding.gs_last_launch_count()
@@ -323,6 +325,7 @@ def measure_config(config, args, ctx, tile_cull=None, light=False):
     pairs_blend = mean([s["pairs_blended"] for s in stats])
     staged = mean([s["entries_staged"] for s in stats])
     n_vis_m, n_dup_m, n_coarse_m = mean([p[0] for p in per_pose]), mean([p[1] for p in per_pose]), mean([p[2] for p in per_pose])
+    n_list_m = mean([p[3] for p in per_pose])   # entries of the tile lists (= N_dup except with gs_set_tile_cull(2))
 
     flush = ctx["flush"]
 
@@ -502,7 +505,7 @@ def measure_config(config, args, ctx, tile_cull=None, light=False):
            "dtype": "f32", "data": "synthetic",
            "config": _config_dict(config, cfg, sc),
            "run": {"frames_per_step": n_pose, "l2": "flushed (256 MiB write) before every step", "frames_in_flight": lanes,
-                   "parallelism": "replicas x%d" % ws, "n_dup_mean": n_dup_m, "n_visible_mean": n_vis_m, "n_coarse_mean": n_coarse_m,
+                   "parallelism": "replicas x%d" % ws, "n_dup_mean": n_dup_m, "n_list_entries_mean": n_list_m, "n_visible_mean": n_vis_m, "n_coarse_mean": n_coarse_m,
                    "binning": "two-level (8x8-tile super-tiles)" if n_coarse_m > 0 else "one-level", "res_scale": args.res_scale,
                    "render_variant": binding.gs_get_render_variant(), "tile_cull": binding.gs_get_tile_cull(), "cuda_graph": bool(r.graph), "workspace_bytes": int(r.workspace.numel())},
            "ms_per_frame": ms_per_step / n_pose, "wall_ms_per_step_incl_flush": 1e3 * wall / K,
@@ -549,28 +552,34 @@ def run_ours(args):
     results = {}
     # everything runs on an ordinary (capturable) stream: the legacy default stream cannot replay CUDA graphs (gs_set_graph)
     main_stream = torch.cuda.Stream(device=dev)
-    culled = {}
+    culled, exact = {}, {}
     for c in configs:
         with torch.cuda.stream(main_stream):
             results[c] = measure_config(c, args, ctx)
             if args.tile_cull == 0 and not args.no_tile_cull_entries:
                 # companion entry: the same configuration with gs_set_tile_cull(1) (tighter rects, same image)
                 culled[c] = measure_config(c, args, ctx, tile_cull=1, light=True)
+                if c >= 3:   # ... and with gs_set_tile_cull(2), the exact ellipse-tile test (the frames that bin in two levels)
+                    exact[c] = measure_config(c, args, ctx, tile_cull=2, light=True)
         if c != configs[-1]:
             ctx["scenes"].pop(c, None)   # one multi-GB scene at a time
     if rank == 0:
         line = dict(results[headline])
         line["peaks"] = dict(ctx["peaks"], issue_peak_measured=ctx["issue"])
-        line["gpu_launches"] = sum(r["gpu_launches"] for r in results.values()) + sum(r["gpu_launches"] for r in culled.values())
+        line["gpu_launches"] = sum(r["gpu_launches"] for r in results.values()) + sum(r["gpu_launches"] for r in culled.values()) + sum(r["gpu_launches"] for r in exact.values())
         cull_keep = ("value", "unit", "ms_per_frame", "latency", "sort_ms_per_frame", "render_ms_per_frame", "roofline", "stage_ms_per_frame", "run", "clocks")
         for c, rc in culled.items():
             results[c]["with_tile_cull"] = {k: rc[k] for k in cull_keep}
+        for c, rc in exact.items():
+            results[c]["with_exact_tile_cull"] = {k: rc[k] for k in cull_keep}
         if headline in culled:
             line["with_tile_cull"] = results[headline]["with_tile_cull"]
+        if headline in exact:
+            line["with_exact_tile_cull"] = results[headline]["with_exact_tile_cull"]
         if len(configs) > 1:
             keep = ("config", "value", "unit", "ms_per_step", "ms_per_frame", "latency", "sort_ms_per_frame", "render_ms_per_frame",
                     "e2e", "roofline", "cpu_baseline", "clocks", "gpu_launches", "launches_per_frame", "stage_ms_per_frame", "kernels", "run",
-                    "with_tile_cull")
+                    "with_tile_cull", "with_exact_tile_cull")
             line["per_config"] = [{k: results[c][k] for k in keep if k in results[c]} for c in configs]
             line["headline"] = "configs[%d] (top-level fields); every configuration has its own %d warm-up and %d timed steps" % (
                 headline - 1, args.warmup, args.steps)
@@ -604,7 +613,7 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=8.0, help="budget of the cpu_baseline leg per configuration")
     ap.add_argument("--lanes", type=int, default=0, help="frames in flight in a step (0 = the fastest of 1-6 over a few warm-up steps)")
     ap.add_argument("--res-scale", type=int, default=1, choices=(1, 2), help="render at 1x or 2x the configuration's resolution (our arm only)")
-    ap.add_argument("--tile-cull", type=int, default=0, choices=(0, 1), help="gs_set_tile_cull: 1 = rects intersected with the alpha >= 1/255 bounding box (our arm only; the default is the standard 3-sigma rect)")
+    ap.add_argument("--tile-cull", type=int, default=0, choices=(0, 1, 2), help="gs_set_tile_cull: 1 = rects intersected with the alpha >= 1/255 bounding box, 2 = and the exact ellipse-tile test per list entry (our arm only; the default is the standard 3-sigma rect)")
     ap.add_argument("--graph", type=int, default=-1, choices=(-1, 0, 1), help="CUDA graph replay of the frame (gs_set_graph): -1 = the Renderer's default (on up to 2^21 Gaussians), 0 off, 1 on")
     ap.add_argument("--no-tile-cull-entries", action="store_true", help="skip the companion measurement of every configuration with gs_set_tile_cull(1)")
     ap.add_argument("--render-variant", type=int, default=None, help="ablation: gs_set_render_variant (default: the library default)")

@@ -86,7 +86,8 @@ typedef struct gs_intermediates {
                                       2 ln(255 o) widened)   [7] flags (bits; 1 = degenerate conic)
                                       second 32 bytes -- read only for entries that reach a pixel (hoist, Eq. 8):
                                       [8] conic a  [9] conic c  [10] log2(opacity)
-                                      [11..13] r, g, b (SH colour clamped at 0)   [14..15] 0                       */
+                                      [11..13] r, g, b (SH colour clamped at 0)   [14] 0   [15] tile-cull modes: the
+                                      upper bound of 2 ln(255 o) the rect and the exact tile test use, else 0      */
     const uint64_t* depth_sorted;  /* dev [n_visible]: (depth bits << 32 | Gaussian id), ascending, stable       */
     const uint32_t* dup_offsets;   /* dev [n_visible]: exclusive prefix sum, in depth order, of the number of
                                       SUPER-TILES (8 x 8 tiles) each Gaussian's tile rect reaches -- the level the
@@ -128,6 +129,15 @@ int gs_get_render_variant(void);
  * Gaussians with o <= 1/255 dropped.  No pixel outside that box can be blended, so the image, final T and n_contrib are
  * unchanged while tiles_touched, N_dup, the tile counts and the sorted lists shrink (30-55 % fewer entries on the five
  * configurations).  The rect arithmetic is one IEEE rounding per operation: bit-identical to the oracle's TILE_CULL mode.
+ * mode 2: the rect of mode 1, and a (tile, Gaussian) pair is LISTED only if the ellipse (tau + 0.05) meets the tile's box of
+ * pixel centres -- the exact ellipse-tile intersection, evaluated where the super-tile lists are expanded into tile lists
+ * (x-extent of the ellipse over the row band: PAPER.md Eq. 13-18 with x and y exchanged; fp32, one IEEE rounding per
+ * operation, bit-identical to the oracle's TILE_CULL_EXACT mode).  Per-Gaussian outputs, tiles_touched and N_dup (the capacity
+ * a frame needs) stay those of mode 1; out_tile_counts holds the EXACT list lengths; gs_intermediates.tile_ranges still
+ * holds the rect-based first slots: list t is sorted_ids[tile_ranges[t] .. tile_ranges[t] + out_tile_counts[t]).  Another
+ * 25-40 % fewer entries than mode 1.  Mode 2 needs the two-level binning, i.e. a workspace sized for max_dup > 4 Mi entries
+ * (gs_render returns GS_ERR_WORKSPACE otherwise), and render variant 4 (GS_ERR_BAD_ARG otherwise); it launches plainly
+ * (gs_set_graph is ignored).
  * Returns GS_ERR_BAD_ARG for another mode.  Process-wide. */
 int gs_set_tile_cull(int mode);
 int gs_get_tile_cull(void);

@@ -20,7 +20,7 @@ void launch_preprocess(const Frame&, const Pointers&, const float*, const float*
 void launch_depth_sort(const Frame&, const Pointers&, int, cudaStream_t, int*);
 void launch_tile_grid(const Frame&, const Pointers&, uint32_t*, const Ctrl*, cudaStream_t, int*);
 void launch_scan_offsets(const Frame&, const Pointers&, int, int, cudaStream_t, int*);
-void launch_expand(const Frame&, const Pointers&, int, cudaStream_t, int*);
+void launch_expand(const Frame&, const Pointers&, uint32_t*, int, cudaStream_t, int*);
 void launch_duplicate_and_tile_sort(const Frame&, const Pointers&, int, cudaStream_t, int*, cudaEvent_t);
 void launch_atomic_order_selftest(unsigned long long*, int, uint32_t, int, int, cudaStream_t);
 cudaError_t run_issue_peak(int, int, double*);
@@ -36,7 +36,7 @@ size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
     size_t ctrl, cctrl, diff, cdiff, st_pre, st_scan, st_depth, st_tile, st_exp, zero_end;
-    size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, desc, cranges, ccounts, entA, entB, cids, ids, total;
+    size_t per_g, rec, gkeyA, gkeyB, dup_off, rk_rect, chunk_start, ranges, desc, cranges, ccounts, tile_len, entA, entB, cids, ids, total;
     size_t n_depth_tiles, n_tile_tiles;
     int gx, gy, n_tiles, tile_bits, n_tile_passes, diff_copies, diff_cells;
     int cshift, cgx, cgy, n_ctiles, cdiff_cells;
@@ -97,6 +97,7 @@ bool make_layout(int P, int W, int H, unsigned long long max_dup, Layout& L) {
     L.desc = take(16 * (size_t)L.n_tiles);
     L.cranges = take(4 * ((size_t)L.n_ctiles + 1));
     L.ccounts = take(4 * (size_t)L.n_ctiles);
+    L.tile_len = take(L.two_level ? 4 * (size_t)L.n_tiles : 0);
     // Two-level frames with <= 2 radix passes over packed entries (P <= 2^24) use at most the first half of entA (packed
     // 4-byte entries between the two passes), so the sorted super-tile ids (cids) live in its second half.
     const bool cids_in_entA = L.two_level && L.n_tile_passes <= 2 && P <= (1 << 24);
@@ -213,6 +214,7 @@ Pointers carve(void* ws, const Layout& L) {
     p.cranges = reinterpret_cast<uint32_t*>(b + L.cranges);
     p.ccounts = reinterpret_cast<uint32_t*>(b + L.ccounts);
     p.cids = reinterpret_cast<uint32_t*>(b + L.cids);
+    p.tile_len = reinterpret_cast<uint32_t*>(b + L.tile_len);
     p.st_pre = reinterpret_cast<unsigned long long*>(b + L.st_pre);
     p.st_scan = reinterpret_cast<unsigned long long*>(b + L.st_scan);
     p.st_depth = reinterpret_cast<unsigned long long*>(b + L.st_depth);
@@ -315,6 +317,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
                                (double)viewmatrix[8 + c] * viewmatrix[11]);
     for (int c = 0; c < 3; c++) f.bg[c] = bg[c];
     f.max_dup = max_dup;
+    f.tile_len = nullptr;
     const Pointers p = carve(workspace, L);
     // the super-tile level of the binning: the same kernels on the coarse grid, with their own control block
     Frame fc = f;
@@ -337,7 +340,12 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     const bool render_stream = opt(GS_OPT_RENDER_STREAM, g_render_stream.load()) != 0;
     f.tile_cull = opt(GS_OPT_TILE_CULL, g_tile_cull.load());
     f.rank_mode = rank_mode;
-    fc.tile_cull = f.tile_cull; fc.rank_mode = rank_mode;
+    // exact ellipse-tile culling happens where the super-tile lists are expanded: it needs the two-level binning (a workspace
+    // sized for more than FUSED_DUP_MAX entries) and the B200 render kernel (the ladder variants walk tile_ranges)
+    if (f.tile_cull == 2 && !L.two_level) return GS_ERR_WORKSPACE;
+    if (f.tile_cull == 2 && variant != 4) return GS_ERR_BAD_ARG;
+    if (f.tile_cull == 2) f.tile_len = p.tile_len;
+    fc.tile_cull = f.tile_cull; fc.rank_mode = rank_mode; fc.tile_len = nullptr;
     if (timed && !lc->have_events) {
         lc->have_events = true;
         for (auto& e : lc->ev) {
@@ -412,7 +420,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
         launch_scan_offsets(fc, pc, f.cshift, g_n_sm, st, &launches);   // (2) prefix-sum offsets of the super-tile duplicates
         mark(4);
         launch_duplicate_and_tile_sort(fc, pc, g_n_sm, st, &launches, timed ? lc->ev[5] : nullptr);  // (2) + (3b) on super-tiles
-        launch_expand(f, p, g_n_sm, st, &launches);                 // (3c) super-tile lists -> tile lists, written in place
+        launch_expand(f, p, out_tile_counts, g_n_sm, st, &launches);                 // (3c) super-tile lists -> tile lists, written in place
     } else {
         launch_scan_offsets(f, p, 0, g_n_sm, st, &launches);  // (2) prefix-sum offsets
         mark(4);
@@ -437,7 +445,7 @@ int gs_render(int P, const float* means3D, const float* scales, const float* rot
     };   // enqueue
 
     const bool special_stream = st == nullptr || st == cudaStreamLegacy || st == cudaStreamPerThread;   // cannot be captured
-    const bool use_graph = opt(GS_OPT_GRAPH, g_graph.load()) != 0 && !timed && variant == 4 && !special_stream;
+    const bool use_graph = opt(GS_OPT_GRAPH, g_graph.load()) != 0 && !timed && variant == 4 && !special_stream && f.tile_cull != 2;
     cudaError_t e = cudaSuccess;
     if (!use_graph) {
         const int rc = enqueue();
@@ -650,7 +658,7 @@ int gs_set_render_variant(int variant) {
 }
 int gs_get_render_variant(void) { return g_variant.load(); }
 int gs_set_tile_cull(int mode) {
-    if (mode != 0 && mode != 1) return GS_ERR_BAD_ARG;
+    if (mode < 0 || mode > 2) return GS_ERR_BAD_ARG;
     g_tile_cull.store(mode);
     return GS_OK;
 }
@@ -662,7 +670,7 @@ int gs_set_render_stream(int enable) {
 int gs_set_workspace_option(const void* workspace, int option, int value) {
     if (!workspace || option < 0 || option >= GS_N_OPTIONS || value < -1) return GS_ERR_BAD_ARG;
     if (option == GS_OPT_RENDER_VARIANT && (value > 6 || value == 5)) return GS_ERR_BAD_ARG;
-    if (option != GS_OPT_RENDER_VARIANT && value > 1) return GS_ERR_BAD_ARG;
+    if (option != GS_OPT_RENDER_VARIANT && value > (option == GS_OPT_TILE_CULL ? 2 : 1)) return GS_ERR_BAD_ARG;
     std::lock_guard<std::mutex> g(g_mu);
     g_calls[workspace].opt.v[option] = value;
     return GS_OK;

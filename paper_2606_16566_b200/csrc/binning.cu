@@ -799,9 +799,46 @@ void launch_duplicate_and_tile_sort(const Frame& f, const Pointers& p, int n_sm,
 // ------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t spread4(uint32_t x) { return ((x & 15u) * 0x00204081u) & 0x01010101u; }   // bit i -> byte i
 
-template <int SH>
+// C-P8'' (gs_set_tile_cull(2), exact ellipse-tile intersection): the tiles of super-tile (X0, Y0) whose box
+// of pixel centres the ellipse a dx^2 + 2 b dx dy + c dy^2 <= tau + 0.05 meets, as the 64-bit mask (byte r = columns of tile
+// row r; lo = rows 0-3, hi = rows 4-7).  Per tile row: the x-extent of the ellipse over the row band -- the paper's tight box
+// (Eq. 13-18) with x and y exchanged -- then one interval test per column.  fp32 with ONE explicit IEEE rounding per
+// operation, in the order of the oracle's tile_hit(): the decision is an integer and bit-identical on both sides.  Every
+// "miss" is an affirmative comparison: a NaN keeps the tile.
+__device__ __forceinline__ void exact_tile_mask(const float a, const float b, const float c, const float mux, const float muy,
+                                                const float tau, const uint32_t X0, const uint32_t Y0, uint32_t& lo, uint32_t& hi) {
+    lo = hi = 0xffffffffu;
+    const float det = __fsub_rn(__fmul_rn(a, c), __fmul_rn(b, b));
+    if (!(det > 0.0f) || !(a > 0.0f) || !(c > 0.0f)) return;          // degenerate conic: keep everything
+    const float te = __fadd_rn(tau, 0.05f);
+    const float at = __fmul_rn(a, te);
+    const float hx = __fsqrt_rn(__fdiv_rn(__fmul_rn(te, c), det));
+    const float ys = __fdiv_rn(__fmul_rn(-b, hx), c);                 // dy of the right-most point; the left-most is at -ys
+    float e0[8];
+#pragma unroll
+    for (int cc = 0; cc < 8; cc++) e0[cc] = __fsub_rn((float)(16u * (X0 + cc)), mux);
+    lo = hi = 0u;
+#pragma unroll
+    for (int r = 0; r < 8; r++) {
+        const float d0 = __fsub_rn((float)(16u * (Y0 + r)), muy), d1 = __fadd_rn(d0, 15.0f);
+        const float yu = fminf(fmaxf(ys, d0), d1), yl = fminf(fmaxf(-ys, d0), d1);
+        const float du = __fsub_rn(at, __fmul_rn(__fmul_rn(det, yu), yu)), dl = __fsub_rn(at, __fmul_rn(__fmul_rn(det, yl), yl));
+        const bool miss_row = du < 0.0f || dl < 0.0f;                 // the band misses the ellipse
+        const float xmax = __fdiv_rn(__fadd_rn(__fmul_rn(-b, yu), __fsqrt_rn(fmaxf(du, 0.0f))), a);
+        const float xmin = __fdiv_rn(__fsub_rn(__fmul_rn(-b, yl), __fsqrt_rn(fmaxf(dl, 0.0f))), a);
+        uint32_t byte = 0;
+#pragma unroll
+        for (int cc = 0; cc < 8; cc++) {
+            const bool miss = miss_row || xmax < e0[cc] || xmin > __fadd_rn(e0[cc], 15.0f);
+            byte |= (miss ? 0u : 1u) << cc;
+        }
+        if (r < 4) lo |= byte << (8 * r); else hi |= byte << (8 * (r - 4));
+    }
+}
+
+template <int SH, bool EXACT>
 __global__ void __launch_bounds__(EXP_THREADS, 4)
-expand_kernel(const Frame f, const Pointers p) {
+expand_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ out_counts) {
     static_assert(SH == 3, "the tile masks are 64-bit: 8 x 8 tiles per super-tile");
     constexpr int SUPER = 8;
     __shared__ __align__(16) uint2 s_m[8][8][32];       // [warp][sub-chunk][lane] tile mask (rows 0-3 | rows 4-7)
@@ -873,6 +910,21 @@ expand_kernel(const Frame f, const Pointers p) {
                 s_m[w][j][lane] = make_uint2(mlo[j], mhi[j]);
                 s_id[w][j][lane] = id[j];
             }
+            if (EXACT) {   // AND the exact ellipse-tile mask into the rect mask, entry by entry (not unrolled: ~400 instructions each)
+#pragma unroll 1
+                for (int j = 0; j < 8; j++) {
+                    const uint2 m = s_m[w][j][lane];
+                    if ((m.x | m.y) != 0u) {
+                        const float4* rec = p.rec + 4 * (size_t)s_id[w][j][lane];
+                        const float4 r0 = __ldg(rec), r2 = __ldg(rec + 2), r3 = __ldg(rec + 3);   // {mu_x, mu_y, b, .} {a, c, ., .} {., ., ., tau}
+                        uint32_t xl, xh;
+                        exact_tile_mask(r2.x, r0.z, r2.y, r0.x, r0.y, r3.w, X0, Y0, xl, xh);
+                        s_m[w][j][lane] = make_uint2(m.x & xl, m.y & xh);
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < 8; j++) { const uint2 m = s_m[w][j][lane]; mlo[j] = m.x; mhi[j] = m.y; }
+            }
             {   // counts: for tile row r the bytes of this lane's eight entries side by side, popcount of column c's bit
                 // in all of them, one warp reduction per tile; lane t & 31 keeps the count of tile t
                 uint32_t mine0 = 0, mine1 = 0;
@@ -934,6 +986,10 @@ expand_kernel(const Frame f, const Pointers p) {
                 const uint32_t ty = Y0 + (uint32_t)(t >> 3), tx = X0 + (uint32_t)(t & 7);
                 const bool inside = ty < (uint32_t)f.gy && tx < (uint32_t)f.gx;
                 s_tb[t] = (inside ? p.ranges[ty * f.gx + tx] : 0u) + (uint32_t)prev;
+                if (EXACT && !goes_on && inside) {       // the super-tile ends here: the exact length of this tile's list
+                    p.tile_len[ty * f.gx + tx] = (uint32_t)prev + run;
+                    out_counts[ty * f.gx + tx] = (uint32_t)prev + run;
+                }
             }
             __syncthreads();
             // ---- (c) emit ------------------------------------------------------------------------------------------
@@ -980,11 +1036,13 @@ expand_kernel(const Frame f, const Pointers p) {
     }
 }
 
-void launch_expand(const Frame& f, const Pointers& p, int n_sm, cudaStream_t st, int* launches) {
+void launch_expand(const Frame& f, const Pointers& p, uint32_t* out_tile_counts, int n_sm, cudaStream_t st, int* launches) {
     const long long cap_chunks = ((long long)f.max_dup + EXP_SEG - 1) / EXP_SEG;
     // three blocks per SM measured best (two to five tried): with more chunks in flight the look-back chains of the long
     // super-tile lists get deeper and the store streams of a tile list interleave more
-    launch_pdl(expand_kernel<SUPER_SHIFT>, dim3(imin(cap_chunks > 0 ? cap_chunks : 1, (long long)n_sm * 3)), dim3(EXP_THREADS), st, f, p);
+    const dim3 grid(imin(cap_chunks > 0 ? cap_chunks : 1, (long long)n_sm * 3));
+    if (f.tile_cull == 2) launch_pdl(expand_kernel<SUPER_SHIFT, true>, grid, dim3(EXP_THREADS), st, f, p, out_tile_counts);
+    else launch_pdl(expand_kernel<SUPER_SHIFT, false>, grid, dim3(EXP_THREADS), st, f, p, out_tile_counts);
     (*launches)++;
 }
 

@@ -68,13 +68,15 @@ struct Frame {              // per-frame constants, passed by value to the kerne
     int tile_bits, n_tile_passes;         // of the grid the duplication + sort runs on (the super-tile grid)
     int compact;                // 1: preprocess compacts the visible Gaussians (P >= COMPACT_MIN_P)
     int rank_mode;              // radix passes: 0 = rank by shared-memory atomics, 1 = by ballots (gs_set_rank_mode)
-    int tile_cull;              // 1: tile rect intersected with the bounding box of the alpha >= 1/255 ellipse (gs_set_tile_cull)
+    int tile_cull;              // 1: tile rect intersected with the bounding box of the alpha >= 1/255 ellipse (gs_set_tile_cull);
+                                // 2: that rect, and expand_kernel lists a (tile, Gaussian) pair only if the ellipse meets the tile
     int diff_copies, diff_cells; // replicas of the coverage difference grid (power of two) and cells per replica
     float V[16], PM[16];
     float fx, fy;
     float campos[3];
     float bg[3];
     unsigned long long max_dup;
+    const uint32_t* tile_len;   // tile_cull == 2: exact list length of every tile (workspace; written by expand_kernel), else nullptr
 };
 
 struct Pointers {           // device pointers carved from the workspace
@@ -83,6 +85,7 @@ struct Pointers {           // device pointers carved from the workspace
     int* cdiff;                             // [(cgy+1)*(cgx+1)] difference grid of super-tile coverage
     uint32_t* cranges;                      // [n_ctiles + 1] ranges of the super-tile lists in cids
     uint32_t* ccounts;                      // [n_ctiles]
+    uint32_t* tile_len;                     // [n_tiles] two-level frames, tile_cull == 2: exact list lengths (expand_kernel)
     uint32_t* cids;                         // [max_dup] Gaussian ids sorted by (super-tile, depth bits, id)
     int* diff;                              // [diff_copies][(gy+1)*(gx+1)] 2-D difference grid of tile coverage
     unsigned long long* st_pre;             // [pre tiles]    look-back status: compaction of visible Gaussians

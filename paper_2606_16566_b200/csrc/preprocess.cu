@@ -29,8 +29,20 @@ __device__ __forceinline__ float dot3(float a0, float a1, float a2, float b0, fl
 struct float5 { float a, b, c, d, e; };
 struct Splat {
     float mux, muy, ca, cb, cc, depth;
+    float tau;   // tile-cull modes: the upper bound of 2 ln(255 o) of C-P8' (0 in the standard mode)
     int radius, xmin, ymin, xmax, ymax;
 };
+
+// Library-free UPPER bound of tau = 2 ln(255 o), o > 1/255: 255 o = 2^e m, ln m <= (m - 1) / sqrt(m) on
+// [1, 2] (at most 0.014 above), + 1e-5; fp32, one rounding per operation (C-P8').
+__device__ __forceinline__ float tau_upper(float opacity) {
+    const float x255 = mul(255.0f, opacity);
+    const uint32_t xb = __float_as_uint(x255);
+    const int e2 = (int)(xb >> 23) - 127;
+    const float m = __uint_as_float((xb & 0x007fffffu) | 0x3f800000u);
+    const float lnm = dvd(sub(m, 1.0f), sqr(m));
+    return add(mul(2.0f, add(mul((float)e2, 0.693147182f), lnm)), 1e-5f);
+}
 
 // C-P0..C-P8.  Returns false when the Gaussian is culled.
 __device__ __forceinline__ bool project(const Frame& f, float px, float py, float pz, float sx, float sy, float sz,
@@ -109,19 +121,16 @@ __device__ __forceinline__ bool project(const Frame& f, float px, float py, floa
     // C-P8 tile rect, half-open, clamped to the grid (reading S6)
     const float rf = (float)radius;
     float rxf = rf, ryf = rf;
+    o.tau = 0.0f;
     if (f.tile_cull) {
         // C-P8' (gs_set_tile_cull(1)): the square intersected with the bounding box of the ellipse
         // alpha >= 1/255, i.e. a dx^2 + 2 b dx dy + c dy^2 <= tau = 2 ln(255 o), half-extents
         // sqrt(tau c / det) and sqrt(tau a / det).  tau is a library-free UPPER bound (255 o = 2^e m, ln m <= (m - 1) /
         // sqrt(m) on [1, 2], + 1e-5); the extents are formed in double from the fp32 conic the blend uses; every operation
         // is one explicit IEEE rounding, as in the rest of this function, so the rect is bit-reproducible.
-        const float x255 = mul(255.0f, opacity);
-        if (!(x255 > 1.0f)) return false;                 // alpha < 1/255 everywhere: never blended
-        const uint32_t xb = __float_as_uint(x255);
-        const int e2 = (int)(xb >> 23) - 127;
-        const float m = __uint_as_float((xb & 0x007fffffu) | 0x3f800000u);
-        const float lnm = dvd(sub(m, 1.0f), sqr(m));
-        const float tau = add(mul(2.0f, add(mul((float)e2, 0.693147182f), lnm)), 1e-5f);
+        if (!(mul(255.0f, opacity) > 1.0f)) return false;   // alpha < 1/255 everywhere: never blended
+        const float tau = tau_upper(opacity);
+        o.tau = tau;
         const double dd = __dsub_rn(__dmul_rn((double)o.ca, (double)o.cc), __dmul_rn((double)o.cb, (double)o.cb));
         if (dd > 0.0 && o.ca > 0.0f && o.cc > 0.0f) {
             const double hx = __dsqrt_rn(__ddiv_rn(__dmul_rn((double)tau, (double)o.cc), dd));
@@ -290,7 +299,7 @@ preprocess_kernel(const Frame f, const Pointers p, const float* __restrict__ mea
             rec[0] = make_float4(s.mux, s.muy, s.cb, (float)dd);          // the half the tight box needs ...
             rec[1] = make_float4(tb.xstar, tb.ic, tb.ct, __uint_as_float(flags));
             rec[2] = make_float4(s.ca, s.cc, l2o, col.x);                   // ... and the half only the hoist needs
-            rec[3] = make_float4(col.y, col.z, 0.0f, 0.0f);
+            rec[3] = make_float4(col.y, col.z, 0.0f, s.tau);                 // [15]: C-P8' tau (0 in the standard mode)
         }
     }
     __syncthreads();
@@ -452,7 +461,7 @@ preprocess2_kernel(const Frame f, const Pointers p, const float* __restrict__ me
                 rec[0] = make_float4(t.mux, t.muy, t.cb, (float)dd);          // the half the tight box needs ...
                 rec[1] = make_float4(tb.xstar, tb.ic, tb.ct, __uint_as_float(flags));
                 rec[2] = make_float4(t.ca, t.cc, l2o, col.x);                   // ... and the half only the hoist needs
-                rec[3] = make_float4(col.y, col.z, 0.0f, 0.0f);
+                rec[3] = make_float4(col.y, col.z, 0.0f, f.tile_cull ? tau_upper(o) : 0.0f);   // [15]: C-P8' tau, read by expand_kernel (tile_cull 2)
             }
         }
         // ---- exclusive prefix by decoupled look-back; keys of the visible Gaussians in index order ------------------

@@ -149,7 +149,9 @@ render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restri
         if ((tid >> 1) == 2) d->y = 3.0e38f;
     }
     bool wdone = __all_sync(0xffffffffu, !in0 && !in1);
-    const uint32_t start = __reduce_max_sync(0xffffffffu, dsc.y), end = __reduce_max_sync(0xffffffffu, dsc.z);   // warp-uniform to ptxas
+    uint32_t end_ = dsc.z;
+    if (f.tile_len != nullptr && dsc.z > dsc.y) end_ = dsc.y + __ldg(f.tile_len + tile);   // gs_set_tile_cull(2): exact list length (expand_kernel)
+    const uint32_t start = __reduce_max_sync(0xffffffffu, dsc.y), end = __reduce_max_sync(0xffffffffu, end_);   // warp-uniform to ptxas
     const unsigned lt = (1u << lane) - 1u;
     uint32_t st_walk = 0, st_staged = 0;  // STATS only
     // ---- gather of a batch: FOUR LANES PER RECORD.  A lane that fetches its own 64-byte record with four 16-byte loads

@@ -54,9 +54,11 @@ def run_gpu_auto(scene, cam_index=0, variant=None, count_contrib=True, device="c
     raise AssertionError("workspace still too small after 4 attempts")
 
 
-def compare(r, it, ref, check_lists=True, check_pixels=True):
+def compare(r, it, ref, check_lists=True, check_pixels=True, exact_cull=False):
     """Returns a report dict; raises AssertionError on any violation.  `ref` is an oracle.render() result (possibly a
-    tile subset), `r` a Renderer after render(), `it` its intermediates."""
+    tile subset), `r` a Renderer after render(), `it` its intermediates.  exact_cull: both sides ran the exact ellipse-tile
+    mode (gs_set_tile_cull(2) / TILE_CULL_EXACT): the tile counts are the exact list lengths, tile_ranges still holds the
+    rect-based first slots, and list t is sorted_ids[ranges[t] : ranges[t] + counts[t]]."""
     rep = {}
     # ---- 1. bit-exact integers -----------------------------------------------------------------------------------
     assert it.P == ref.P and it.n_tiles == ref.n_tiles
@@ -72,9 +74,22 @@ def compare(r, it, ref, check_lists=True, check_pixels=True):
     counts = r.out_tile_counts.cpu().numpy().view(np.uint32)
     assert np.array_equal(counts, ref.tile_counts), "tile counts differ"
     ranges = it.tile_ranges.astype(np.uint64)
-    assert ranges[0] == 0 and np.array_equal(np.diff(ranges), ref.tile_counts.astype(np.uint64)), "tile ranges differ"
+    if exact_cull:   # first slots from the rect-based coverage grid; every list fits into its slot range
+        assert ranges[0] == 0 and ranges[-1] == it.n_dup and (np.diff(ranges) >= ref.tile_counts.astype(np.uint64)).all(), "tile ranges"
+    else:
+        assert ranges[0] == 0 and np.array_equal(np.diff(ranges), ref.tile_counts.astype(np.uint64)), "tile ranges differ"
     rep.update(P=int(it.P), n_visible=int(it.n_visible), n_dup=int(it.n_dup))
-    if check_lists and ref.full:   # every list: the concatenation IS the sorted id array (ranges already compared)
+    if check_lists and exact_cull:
+        n_bad = 0
+        for l, t in enumerate(ref.list_tile):
+            a = it.sorted_ids[int(ranges[t]):int(ranges[t]) + int(counts[t])]
+            b = ref.sorted_ids[int(ref.list_offsets[l]):int(ref.list_offsets[l + 1])]
+            if not np.array_equal(a, b):
+                n_bad += 1
+        assert n_bad == 0, "sorted id lists differ in %d of %d tiles" % (n_bad, len(ref.list_tile))
+        rep["lists_checked"] = int(len(ref.list_tile))
+        rep["list_entries"] = int(counts.sum())
+    elif check_lists and ref.full:   # every list: the concatenation IS the sorted id array (ranges already compared)
         assert it.sorted_ids.shape == ref.sorted_ids.shape and np.array_equal(it.sorted_ids, ref.sorted_ids), \
             "sorted id array differs (first at %s)" % (np.flatnonzero(it.sorted_ids != ref.sorted_ids)[:5],)
         rep["lists_checked"] = int(len(ref.list_tile))
@@ -124,15 +139,19 @@ def compare(r, it, ref, check_lists=True, check_pixels=True):
 
 
 def oracle_and_compare(scene, cam_index=0, tile_subset=None, n_threads=8, variant=None, count_contrib=True, flags=0, tile_cull=False):
-    """tile_cull: both sides in the tighter-rect mode (gs_set_tile_cull(1) / oracle flag TILE_CULL); reset to 0 afterwards."""
-    binding.gs_set_tile_cull(1 if tile_cull else 0)
+    """tile_cull: both sides in the tighter-rect mode (True / 1: gs_set_tile_cull(1) / oracle flag TILE_CULL; 2: the exact
+    ellipse-tile mode gs_set_tile_cull(2) / TILE_CULL_EXACT, which needs a two-level workspace); reset to 0 afterwards."""
+    mode = int(tile_cull)
+    binding.gs_set_tile_cull(mode)
     try:
-        r, it = run_gpu_auto(scene, cam_index, variant=variant, count_contrib=count_contrib)
+        r, it = run_gpu_auto(scene, cam_index, variant=variant, count_contrib=count_contrib, start_dup=(5 << 20) if mode == 2 else (1 << 20))
     finally:
         binding.gs_set_tile_cull(0)
-    if tile_cull:
+    if mode == 1:
         flags |= oracle.TILE_CULL
+    elif mode == 2:
+        flags |= oracle.TILE_CULL_EXACT
     ref = oracle.render(scene, cam_index, tile_subset=tile_subset, n_threads=n_threads, flags=flags, fragile_delta=DELTA)
     rep = compare(r, it, ref, check_lists=not (flags & oracle.NO_LISTS),
-                  check_pixels=not (flags & (oracle.NO_LISTS | oracle.NO_RENDER)))
+                  check_pixels=not (flags & (oracle.NO_LISTS | oracle.NO_RENDER)), exact_cull=(mode == 2))
     return rep, r, it, ref

@@ -54,7 +54,8 @@ def test_workspace_bytes_and_error_strings_host_only():
     fake = ctypes.c_void_p(0x1000)
     assert L.gs_set_workspace_option(fake, 9, 0) == binding.GS_ERR_BAD_ARG
     assert L.gs_set_workspace_option(fake, binding.GS_OPT_RENDER_VARIANT, 5) == binding.GS_ERR_BAD_ARG
-    assert L.gs_set_workspace_option(fake, binding.GS_OPT_TILE_CULL, 2) == binding.GS_ERR_BAD_ARG
+    assert L.gs_set_workspace_option(fake, binding.GS_OPT_TILE_CULL, 3) == binding.GS_ERR_BAD_ARG
+    assert L.gs_set_workspace_option(fake, binding.GS_OPT_TILE_CULL, 2) == 0 and L.gs_set_workspace_option(fake, binding.GS_OPT_TILE_CULL, -1) == 0
     assert L.gs_set_workspace_option(None, 0, 0) == binding.GS_ERR_BAD_ARG
     assert L.gs_set_workspace_option(fake, binding.GS_OPT_STATS, 1) == 0 and L.gs_release(fake) == 0   # nothing CUDA was created
     assert L.gs_release(fake) == 0 and L.gs_release(None) == binding.GS_ERR_BAD_ARG

@@ -604,7 +604,47 @@ def test_tile_cull_mode_leaves_the_image_unchanged():
     assert torch.equal(out[0][2], out[1][2])
     assert float((out[0][0] - out[1][0]).abs().max()) < 2e-6 and float((out[0][1] - out[1][1]).abs().max()) < 2e-6
     with pytest.raises(binding.GsError):
-        binding.gs_set_tile_cull(2)
+        binding.gs_set_tile_cull(3)
+
+
+# exact ellipse-tile culling (gs_set_tile_cull(2) / oracle flag TILE_CULL_EXACT): the per-Gaussian integers and
+# N_dup are those of mode 1; the tile counts are the exact list lengths; every list equals the oracle's; image within tolerance
+@pytest.mark.parametrize("config,kw,pose", [
+    (2, dict(P=30_000, W=480, H=360, f=500.0), 1), (3, dict(P=60_000, W=640, H=416, f=500.0), 2),
+    (4, dict(P=20_000, W=480, H=270, f=375.0), 0), (5, dict(P=200_000, W=960, H=540, f=750.0), 3)])
+def test_exact_tile_cull_mode_matches_the_oracle_in_the_same_mode(config, kw, pose):
+    sc = scenes.make_scene(config, **kw)
+    rep, r, it, ref = pu.oracle_and_compare(sc, pose, tile_cull=2)
+    assert it.n_coarse > 0
+    print("config", config, "exact tile cull", rep, "entries / N_dup %.2f" % (rep["list_entries"] / max(rep["n_dup"], 1)))
+
+
+@pytest.mark.parametrize("config,pose", [(3, 4), (5, 2)])
+def test_exact_tile_cull_mode_full_size(config, pose):
+    sc = _full_scene(config)
+    binding.gs_set_tile_cull(2)
+    ref = oracle.render(sc, pose, n_threads=N_CPU, fragile_delta=pu.DELTA, flags=oracle.TILE_CULL_EXACT)
+    r, it = pu.run_gpu_auto(sc, pose, start_dup=max(int(ref.n_dup) + 4096, 5 << 20))
+    binding.gs_set_tile_cull(0)
+    rep = pu.compare(r, it, ref, exact_cull=True)
+    print("config", config, "FULL, exact tile cull, pose", pose, rep)
+
+
+def test_exact_tile_cull_needs_a_two_level_workspace_and_the_b200_kernel():
+    sc = scenes.make_scene(1)
+    binding.gs_set_tile_cull(2)
+    try:
+        with pytest.raises(binding.GsError) as ei:                # capacity <= 4 Mi entries: one-level binning has no expansion stage
+            pu.run_gpu(sc, 0, max_dup=1 << 20)
+        assert ei.value.code == binding.GS_ERR_WORKSPACE
+        with pytest.raises(binding.GsError) as ei:                # the ladder variants walk tile_ranges
+            pu.run_gpu(sc, 0, max_dup=5 << 20, variant=3)
+        assert ei.value.code == binding.GS_ERR_BAD_ARG
+        rep, r, it, ref = pu.oracle_and_compare(sc, 0, tile_cull=2)   # and with both it works on the smallest scene too
+        print(rep)
+    finally:
+        binding.gs_set_tile_cull(0)
+        binding.gs_set_render_variant(binding.GS_DEFAULT_RENDER_VARIANT)
 
 
 # ------------------------------------------------------------------------------------------------------------------

@@ -267,8 +267,9 @@ void alloc_pre(Pre& o, int P) {
 // band dy in [d0, d1] the right boundary x(dy) = (-b dy + sqrt(a tau_e - det dy^2)) / a is concave, so its maximum is at
 // clamp(dy*, d0, d1) (the left boundary: convex, minimum at clamp(-dy*, d0, d1)).  fp32, ONE rounding per operation in
 // this order (the CUDA side restates it with __f*_rn intrinsics): the decision is an integer and must be bit-identical.
-// Every "miss" is an affirmative comparison, so a NaN keeps the tile; the 0.05 added to tau (>= 4e-3 relative) covers the
-// fp32 rounding of the pixel-to-centre differences (<= 5e-4 px at 8 K) and of the discriminants (1e-6 relative).
+// Every "miss" is an affirmative comparison, so a NaN keeps the tile; the 0.05 added to tau (>= 4e-3 relative, >= 4e-3 px of
+// extent for the sharpest conic the dilation allows) covers the fp32 rounding of the pixel positions (<= 5e-4 px at 8 K), of
+// the reciprocal (1e-7 relative) and of the discriminants (1e-6 relative).
 bool tile_hit(const Pre& pre, int i, int tx, int ty) {
     const float a = pre.conic[3 * (size_t)i], b = pre.conic[3 * (size_t)i + 1], c = pre.conic[3 * (size_t)i + 2];
     const float mux = pre.mu[2 * (size_t)i], muy = pre.mu[2 * (size_t)i + 1];
@@ -276,16 +277,19 @@ bool tile_hit(const Pre& pre, int i, int tx, int ty) {
     if (!(det > 0.0f) || !(a > 0.0f) || !(c > 0.0f)) return true;      // degenerate conic: keep everything
     const float te = pre.tau[i] + 0.05f;
     const float at = a * te;
+    const float ia = 1.0f / a;
     const float hx = std::sqrt((te * c) / det);
     const float ys = ((-b) * hx) / c;                                  // dy of the right-most point; the left-most is at -ys
     const float d0 = (float)(16 * ty) - muy, d1 = d0 + 15.0f;          // the band, relative to the mean
     const float yu = std::fmin(std::fmax(ys, d0), d1), yl = std::fmin(std::fmax(-ys, d0), d1);
     const float du = at - ((det * yu) * yu), dl = at - ((det * yl) * yl);
     if (du < 0.0f || dl < 0.0f) return false;                          // the band misses the ellipse
-    const float xmax = (((-b) * yu) + std::sqrt(std::fmax(du, 0.0f))) / a;
-    const float xmin = (((-b) * yl) - std::sqrt(std::fmax(dl, 0.0f))) / a;
-    const float e0 = (float)(16 * tx) - mux, e1 = e0 + 15.0f;          // the tile's columns, relative to the mean
-    if (xmax < e0 || xmin > e1) return false;
+    // right-most / left-most pixel abscissa of the ellipse over the band, then the tile columns they fall in: tile tx holds
+    // the pixels 16 tx .. 16 tx + 15, so it is met iff ceil((xl - 15) / 16) <= tx <= floor(xr / 16) (the scaling is exact)
+    const float xr = mux + ((((-b) * yu) + std::sqrt(std::fmax(du, 0.0f))) * ia);
+    const float xl = mux + ((((-b) * yl) - std::sqrt(std::fmax(dl, 0.0f))) * ia);
+    const float thi = std::floor(xr * 0.0625f), tlo = std::ceil((xl - 15.0f) * 0.0625f);
+    if ((float)tx > thi || (float)tx < tlo) return false;
     return true;
 }
 

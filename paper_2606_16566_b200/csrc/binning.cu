@@ -806,32 +806,34 @@ __device__ __forceinline__ uint32_t spread4(uint32_t x) { return ((x & 15u) * 0x
 // operation, in the order of the oracle's tile_hit(): the decision is an integer and bit-identical on both sides.  Every
 // "miss" is an affirmative comparison: a NaN keeps the tile.
 __device__ __forceinline__ void exact_tile_mask(const float a, const float b, const float c, const float mux, const float muy,
-                                                const float tau, const uint32_t X0, const uint32_t Y0, uint32_t& lo, uint32_t& hi) {
+                                                const float tau, const uint32_t X0, const uint32_t Y0, const uint32_t rows,
+                                                uint32_t& lo, uint32_t& hi) {
     lo = hi = 0xffffffffu;
     const float det = __fsub_rn(__fmul_rn(a, c), __fmul_rn(b, b));
     if (!(det > 0.0f) || !(a > 0.0f) || !(c > 0.0f)) return;          // degenerate conic: keep everything
     const float te = __fadd_rn(tau, 0.05f);
     const float at = __fmul_rn(a, te);
+    const float ia = __fdiv_rn(1.0f, a);
     const float hx = __fsqrt_rn(__fdiv_rn(__fmul_rn(te, c), det));
     const float ys = __fdiv_rn(__fmul_rn(-b, hx), c);                 // dy of the right-most point; the left-most is at -ys
-    float e0[8];
-#pragma unroll
-    for (int cc = 0; cc < 8; cc++) e0[cc] = __fsub_rn((float)(16u * (X0 + cc)), mux);
+    const float fx0 = (float)X0;
     lo = hi = 0u;
 #pragma unroll
     for (int r = 0; r < 8; r++) {
+        if (!((rows >> r) & 1u)) continue;                            // the rect does not reach this tile row
         const float d0 = __fsub_rn((float)(16u * (Y0 + r)), muy), d1 = __fadd_rn(d0, 15.0f);
         const float yu = fminf(fmaxf(ys, d0), d1), yl = fminf(fmaxf(-ys, d0), d1);
         const float du = __fsub_rn(at, __fmul_rn(__fmul_rn(det, yu), yu)), dl = __fsub_rn(at, __fmul_rn(__fmul_rn(det, yl), yl));
-        const bool miss_row = du < 0.0f || dl < 0.0f;                 // the band misses the ellipse
-        const float xmax = __fdiv_rn(__fadd_rn(__fmul_rn(-b, yu), __fsqrt_rn(fmaxf(du, 0.0f))), a);
-        const float xmin = __fdiv_rn(__fsub_rn(__fmul_rn(-b, yl), __fsqrt_rn(fmaxf(dl, 0.0f))), a);
-        uint32_t byte = 0;
-#pragma unroll
-        for (int cc = 0; cc < 8; cc++) {
-            const bool miss = miss_row || xmax < e0[cc] || xmin > __fadd_rn(e0[cc], 15.0f);
-            byte |= (miss ? 0u : 1u) << cc;
-        }
+        if (du < 0.0f || dl < 0.0f) continue;                         // the band misses the ellipse
+        const float xr = __fadd_rn(mux, __fmul_rn(__fadd_rn(__fmul_rn(-b, yu), __fsqrt_rn(fmaxf(du, 0.0f))), ia));
+        const float xl = __fadd_rn(mux, __fmul_rn(__fsub_rn(__fmul_rn(-b, yl), __fsqrt_rn(fmaxf(dl, 0.0f))), ia));
+        // tile columns ceil((xl - 15) / 16) .. floor(xr / 16), relative to the super-tile, clamped to its 8 columns; fminf /
+        // fmaxf return the other operand for a NaN, i.e. a NaN keeps every column (the oracle's comparisons do the same)
+        const float thi = fminf(floorf(__fmul_rn(xr, 0.0625f)) - fx0, 7.0f);
+        const float tlo = fmaxf(ceilf(__fmul_rn(__fsub_rn(xl, 15.0f), 0.0625f)) - fx0, 0.0f);
+        const int ih = (int)thi, il = (int)tlo;
+        if (ih < il) continue;
+        const uint32_t byte = ((2u << ih) - 1u) & ~((1u << il) - 1u);
         if (r < 4) lo |= byte << (8 * r); else hi |= byte << (8 * (r - 4));
     }
 }
@@ -910,15 +912,25 @@ expand_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ out_counts
                 s_m[w][j][lane] = make_uint2(mlo[j], mhi[j]);
                 s_id[w][j][lane] = id[j];
             }
-            if (EXACT) {   // AND the exact ellipse-tile mask into the rect mask, entry by entry (not unrolled: ~400 instructions each)
+            if (EXACT) {   // AND the exact ellipse-tile mask into the rect mask, entry by entry (not unrolled: ~300 instructions each);
+                           // the record of entry j + 1 is in flight while entry j is evaluated
+                const float4* rec = p.rec + 4 * (size_t)id[0];
+                float4 n0 = __ldg(rec), n2 = __ldg(rec + 2), n3 = __ldg(rec + 3);   // {mu_x, mu_y, b, .} {a, c, ., .} {., ., ., tau}
 #pragma unroll 1
                 for (int j = 0; j < 8; j++) {
+                    const float4 r0 = n0, r2 = n2, r3 = n3;
+                    if (j < 7) {
+                        const float4* nx = p.rec + 4 * (size_t)s_id[w][j + 1][lane];
+                        n0 = __ldg(nx); n2 = __ldg(nx + 2); n3 = __ldg(nx + 3);
+                    }
                     const uint2 m = s_m[w][j][lane];
                     if ((m.x | m.y) != 0u) {
-                        const float4* rec = p.rec + 4 * (size_t)s_id[w][j][lane];
-                        const float4 r0 = __ldg(rec), r2 = __ldg(rec + 2), r3 = __ldg(rec + 3);   // {mu_x, mu_y, b, .} {a, c, ., .} {., ., ., tau}
+                        // rows the rect reaches: a byte of the mask is non-zero
+                        uint32_t rows = 0;
+#pragma unroll
+                        for (int r = 0; r < 4; r++) rows |= (((m.x >> (8 * r)) & 255u) ? 1u : 0u) << r | (((m.y >> (8 * r)) & 255u) ? 16u : 0u) << r;
                         uint32_t xl, xh;
-                        exact_tile_mask(r2.x, r0.z, r2.y, r0.x, r0.y, r3.w, X0, Y0, xl, xh);
+                        exact_tile_mask(r2.x, r0.z, r2.y, r0.x, r0.y, r3.w, X0, Y0, rows, xl, xh);
                         s_m[w][j][lane] = make_uint2(m.x & xl, m.y & xh);
                     }
                 }
@@ -1009,6 +1021,7 @@ expand_kernel(const Frame f, const Pointers p, uint32_t* __restrict__ out_counts
 #pragma unroll 1
                     for (uint32_t j = 0; j < n_sub; j++) {
                         const uint32_t rowbyte = mb[j * (32 * 8) + r];      // byte r of this lane's mask of sub-chunk j
+                        if (!__any_sync(0xffffffffu, rowbyte != 0u)) continue;   // none of the 32 entries reaches this tile row
                         const uint32_t my_id = s_id[w][j][lane];
 #pragma unroll
                         for (int c = 0; c < 8; c++) {

@@ -251,11 +251,11 @@ def _stage_bytes(P, K_sh, n_vis, n_dup, n_coarse, n_sort_passes, max_dup):
 # of one launch, and the hardware pipe utilisation / executed-work figures (A) and (B) of SURVEY.md 8(d).
 PROFILED = {
     # (A) and (B) of SURVEY.md 8(d) and the DRAM traffic of one launch, from profiles/r02_render_ncu.md (ncu --set full, pose 0)
-    2: {"file": "profiles/r02_render_ncu.md", "dram_bytes": 10129920, "us_under_ncu": 44.4, "fma_pipe_pct": 43.9, "xu_pipe_pct": 45.2,
-        "issue_slots_pct": 68.6, "branch_uniformity_pct": 96.4, "threads_per_inst": 31.7,
-        "executed_fp32_thread_ops": 539267784, "executed_mufu_thread_ops": 57513600, "executed_work_roofline_frac": 0.333},
-    5: {"file": "profiles/r02_render_ncu.md", "dram_bytes": 315163904, "us_under_ncu": 579.3, "fma_pipe_pct": 42.3, "xu_pipe_pct": 47.6,
-        "issue_slots_pct": 71.2, "branch_uniformity_pct": 95.0, "threads_per_inst": 31.4,
+    2: {"file": "profiles/r02_render_ncu.md", "dram_bytes": 10131968, "us_under_ncu": 44.4, "fma_pipe_pct": 44.1, "xu_pipe_pct": 45.3,
+        "issue_slots_pct": 68.7, "branch_uniformity_pct": 96.4, "threads_per_inst": 31.7,
+        "executed_fp32_thread_ops": 539267784, "executed_mufu_thread_ops": 57513600, "executed_work_roofline_frac": 0.338},
+    5: {"file": "profiles/r02_render_ncu.md", "dram_bytes": 314942976, "us_under_ncu": 582.8, "fma_pipe_pct": 42.3, "xu_pipe_pct": 47.5,
+        "issue_slots_pct": 71.1, "branch_uniformity_pct": 95.0, "threads_per_inst": 31.4,
         "executed_fp32_thread_ops": 7513506416, "executed_mufu_thread_ops": 797693696, "executed_work_roofline_frac": 0.364},
 }
 

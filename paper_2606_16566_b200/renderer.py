@@ -37,6 +37,7 @@ class Renderer:
         self._host_rgb = None
         self._ring = None     # render_to_host(): two device images, a copy stream and the events that order them
         self._lanes = None    # render_batch(): per-lane stream, workspace and outputs
+        self._options = {}    # set_option(): per-workspace switches of this Renderer, applied to every lane's workspace
         self._copy_stream = None
         self._standby = None  # upload_async(): second set of scene buffers, upload stream and its events
         self._upload_stream = None
@@ -174,6 +175,14 @@ class Renderer:
         return self._host_rgb[slot]
 
     # ---- several frames in flight ---------------------------------------------------------------------------------
+    def set_option(self, option: int, value: int) -> None:
+        """Per-workspace switch (binding.GS_OPT_*; -1 = follow the process-wide setter) for EVERY workspace of this Renderer:
+        its own and those of the lanes render_batch uses, present and future."""
+        self._options[int(option)] = int(value)
+        binding.gs_set_workspace_option(self.workspace, option, value)
+        for ln in (self._lanes or [])[1:]:
+            binding.gs_set_workspace_option(ln["workspace"], option, value)
+
     def _lane(self, k: int):
         """Lane k: its own stream, workspace and output buffers (lane 0 = this Renderer's own buffers, on its own
         stream too, so that the caller's stream only forks and joins)."""
@@ -189,6 +198,8 @@ class Renderer:
                       done=torch.cuda.Event(), copied=torch.cuda.Event(), copy_pending=False, render_stream=False)
             if not first:
                 binding.gs_set_workspace_option(ln["workspace"], binding.GS_OPT_GRAPH, 1 if self.graph else 0)
+                for opt, val in self._options.items():       # the switches of this Renderer hold for all its workspaces
+                    binding.gs_set_workspace_option(ln["workspace"], opt, val)
             self._lanes.append(ln)
         return self._lanes[k]
 

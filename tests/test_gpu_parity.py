@@ -647,6 +647,54 @@ def test_exact_tile_cull_needs_a_two_level_workspace_and_the_b200_kernel():
         binding.gs_set_render_variant(binding.GS_DEFAULT_RENDER_VARIANT)
 
 
+def test_exact_tile_cull_overflow_batch_and_per_workspace_switch():
+    """Edge cases of gs_set_tile_cull(2): (a) an overflowing frame -- expand_kernel does nothing, no list length is published
+    -- must come out as background with the need reported, and the same workspace must render correctly afterwards when it
+    is large enough; (b) the mode as a PER-WORKSPACE switch next to a renderer in the standard mode, through render_batch
+    with several frames in flight: same images as single renders, the other renderer untouched."""
+    bg = np.array([0.25, 0.5, 0.75], np.float32)
+    sc = scenes.make_scene(3, P=1_000_000, W=1264, H=832)
+    sc.bg = bg
+    need = int(oracle.render(sc, 0, flags=oracle.NO_LISTS | oracle.TILE_CULL).n_dup)
+    cap = 5 << 20
+    assert need > cap, need
+    binding.gs_set_tile_cull(2)
+    try:
+        r = pu.run_gpu(sc, 0, max_dup=cap)
+        with pytest.raises(binding.GsError) as ei:
+            r.intermediates()
+        assert ei.value.code == binding.GS_ERR_OVERFLOW and ei.value.n_dup == need
+        assert torch.equal(r.out_final_T, torch.ones_like(r.out_final_T))
+        assert np.array_equal(r.out_rgb.cpu().numpy(), np.broadcast_to(bg[:, None, None], (3, 832, 1264)))
+        del r
+        torch.cuda.empty_cache()
+    finally:
+        binding.gs_set_tile_cull(0)
+    rep, *_ = pu.oracle_and_compare(sc, 0, tile_cull=2)             # grows the workspace from the reported need
+    print(rep)
+    # (b)
+    sc = scenes.make_scene(5, P=150_000, W=960, H=540, f=750.0, poses=4)
+    cams = list(sc.cameras)
+    ra = Renderer(sc.P, 960, 540, 6 << 20, device="cuda:0", count_contrib=False)
+    rb = Renderer(sc.P, 960, 540, 6 << 20, device="cuda:0", count_contrib=False)
+    ra.upload(sc); rb.upload(sc)
+    ra.set_option(binding.GS_OPT_TILE_CULL, 2)                   # every workspace of ra, the lanes of render_batch included
+    singles_a, singles_b, lens = [], [], []
+    for cam in cams:
+        ra.render(cam); rb.render(cam)
+        torch.cuda.synchronize()
+        singles_a.append(ra.out_rgb.clone()); singles_b.append(rb.out_rgb.clone())
+        lens.append((int(ra.out_tile_counts.sum()), int(rb.out_tile_counts.sum())))
+    assert all(a < 0.8 * b for a, b in lens), lens              # a's lists are the exact ones, b's the standard ones
+    host_a = ra.render_batch(cams, lanes=3, to_host=True)
+    host_b = rb.render_batch(cams, lanes=3, to_host=True)
+    torch.cuda.synchronize()
+    for k in range(len(cams)):
+        assert torch.equal(host_a[k], singles_a[k].cpu()) and torch.equal(host_b[k], singles_b[k].cpu())
+        assert float((singles_a[k] - singles_b[k]).abs().max()) < 2e-6   # same image up to the rounding of the stop repair
+    assert binding.gs_get_tile_cull() == 0
+
+
 # ------------------------------------------------------------------------------------------------------------------
 # boundary: ranking fallback, per-workspace switches, release
 # ------------------------------------------------------------------------------------------------------------------

@@ -786,8 +786,8 @@ def test_graph_replay_gives_the_same_frames_as_plain_launches():
 def test_bounds_checked_build_runs_clean():
     """libgs_dbg.so = the same sources with -DGS_DEBUG_BOUNDS: every index into the workspace and the output arrays is
     checked on the device and a violation traps (the stand-in for compute-sanitizer, closed on this pool).  Configs 1 and 2 at
-    full size, a two-level frame, the tile-cull mode and the ballot ranking run through it in a fresh process and must still
-    agree with the oracle."""
+    full size, a two-level frame, both tile-cull modes, the ballot ranking and the allocation-free depth sort run through it in a
+    fresh process and must still agree with the oracle."""
     import subprocess
     import sys
     code = r'''
@@ -809,6 +809,14 @@ it = r.intermediates()
 assert it.n_coarse > 0
 from oracle import oracle
 print(pu.compare(r, it, oracle.render(sc, 2, n_threads=8, fragile_delta=pu.DELTA)))
+print(pu.oracle_and_compare(sc, 5, tile_cull=2)[0])          # exact ellipse-tile mode (expand_kernel<.., true>)
+import numpy as np, torch
+keys = torch.from_numpy(np.random.default_rng(3).integers(0, 1 << 62, 100_000, dtype=np.int64)).cuda()
+out = torch.empty_like(keys)
+binding.gs_depth_sort_noalloc(keys, out)                       # the allocation-free depth sort on its static scratch
+torch.cuda.synchronize()
+hi = keys.cpu().numpy().view(np.uint64) >> np.uint64(32)
+assert np.array_equal(out.cpu().numpy().view(np.uint64), keys.cpu().numpy().view(np.uint64)[np.argsort(hi, kind="stable")])
 print("BOUNDS OK")
 '''
     env = dict(os.environ, GS_DEBUG_BOUNDS="1")

@@ -1,9 +1,10 @@
 // render_b200.cu -- the B200 render kernel (variant 4): Local-GS (Sec. III) re-laid-out for sm_100a.
 //
-//   * 128 threads per 16x16 tile, TWO horizontally adjacent pixels per thread, every per-pixel operation issued as a
-//     packed f32x2 instruction (FFMA2 / FMUL2 with scalar-broadcast coefficient operands): the exponent
-//     log2(alpha) = V_hoisted . B_local (Eq. 9-10) is 5 FFMA2 for two pixels, the blend w = alpha T; C += f w;
-//     T -= w (Alg. 1 right column) is FMUL2 + 4 FFMA2.
+//   * 128 threads per 16x16 tile, TWO horizontally adjacent pixels per thread, the per-pixel operations issued as
+//     packed f32x2 instructions (FFMA2 / FMUL2 with scalar-broadcast coefficient operands).  The two pixels share their
+//     row, so the exponent log2(alpha) = V_hoisted . B_local (Eq. 9-10) is evaluated as (A x' + H) x' + G with the row
+//     part H = B y' + D, G = C y'^2 + E y' + F computed once for both: 3 scalar FFMA + 2 FFMA2 per entry; the blend
+//     w = alpha T; C += f w; T -= w (Alg. 1 right column) is FMUL2 + 4 FFMA2.
 //   * warp w owns the 8x8 quadrant (w&1, w>>1); the tight box (Eq. 13-19) is evaluated once per (tile, Gaussian) for
 //     the two 8-pixel sub-columns and turned into a 4-bit warp mask (Eq. 20-21 with 8-row bands); its per-Gaussian
 //     part (x*, 1/c, c tau) comes precomputed from preprocess, the per-tile part is branch-free.
@@ -15,8 +16,8 @@
 //     K = 2^126 / 255 and 1/K folds into the w = alpha T product.  No compare, no select, no predicate.
 //   * hoisting is done in double, about the tile CENTRE (S14), once per (tile, Gaussian).
 //   * termination rule R1 (reading S11) without any per-pixel state test in the hot loop: the only test is
-//     T - w < 1e-4, voted across the warp; the rare taken branch un-blends the stopping pixel and POISONS its x^2
-//     basis element (1e36), which drives every later log2(alpha) to -huge, i.e. alpha = 0 exactly.
+//     T - w < 1e-4, voted across the warp; the rare taken branch un-blends the stopping pixel and POISONS its x'
+//     (1e18), which drives every later log2(alpha) to -huge, i.e. alpha = 0 exactly.
 //   * staging is software-pipelined: the ids of batch k+2 and the 64-byte records of batch k+1 are in flight while
 //     batch k is blended; shared memory is double-buffered, so a batch costs ONE block barrier.
 #include "render_blend.cuh"
@@ -104,8 +105,8 @@ __device__ __forceinline__ void blend_list(PixelPair& s, uint32_t& lp, uint32_t&
     }
 }
 
-// 7 blocks per SM: 72 registers.  (8 blocks / 64 registers measured 8 % slower: ptxas then splits the live ranges of the
-// accumulators, 10 register moves per iteration of the blend loop instead of 4.)
+// 8 blocks per SM at 64 registers: since the separable exponent (three scalars and one packed x' instead of five packed
+// basis elements) the loop fits without a register move; at 9 blocks (56 registers) ptxas brings six moves back.
 template <bool COUNT, bool STATS>
 __global__ void __launch_bounds__(QB, 8)
 render_b200_kernel(const Frame f, Ctrl* __restrict__ ctrl, const uint4* __restrict__ desc, const uint32_t* __restrict__ ids,

@@ -69,7 +69,8 @@ __device__ __forceinline__ uint2 lds64u(uint32_t addr) {
 }
 
 // Exponent and alpha of one staged record for the two pixels of this thread: alpha / K, clamped (Eq. 10 in the biased
-// log2 domain: 5 FFMA2, "5 FMA" of Table I; exactly 0 below the 1/255 floor; min(0.99, .)).
+// log2 domain, separable form: 3 FFMA for the shared row part + 2 FFMA2 -- Table I has "5 FMA" per pixel; exactly 0 below
+// the 1/255 floor; min(0.99, .)).
 template <bool GUARD>
 __device__ __forceinline__ u64 alpha_pair(const PixelPair& s, const float4 q0, const float4 q1, const float guard, float& e0,
                                           float& e1) {

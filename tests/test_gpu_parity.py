@@ -619,7 +619,7 @@ def test_exact_tile_cull_mode_matches_the_oracle_in_the_same_mode(config, kw, po
     print("config", config, "exact tile cull", rep, "entries / N_dup %.2f" % (rep["list_entries"] / max(rep["n_dup"], 1)))
 
 
-@pytest.mark.parametrize("config,pose", [(3, 4), (5, 2)])
+@pytest.mark.parametrize("config,pose", [(2, 1), (3, 4), (5, 2)])
 def test_exact_tile_cull_mode_full_size(config, pose):
     sc = _full_scene(config)
     binding.gs_set_tile_cull(2)

@@ -91,3 +91,28 @@ def test_limit_ragged_sizes_and_stability():
         binding.gs_depth_sort_noalloc(t_in, t_out)
         torch.cuda.synchronize()
         assert np.array_equal(t_out.cpu().numpy().view(np.uint64), keys[order]), n
+
+
+def test_the_call_can_be_captured_into_a_cuda_graph_and_replayed():
+    """The use the entry point is for: under stream capture cudaMalloc is not allowed.  One warm-up call outside the capture
+    (the first call on a device looks up the scratch address), then the call is captured and the graph replayed on new keys."""
+    rng = np.random.default_rng(11)
+    n = 50_000
+    t_in = torch.zeros(n, dtype=torch.int64, device="cuda:0")
+    t_out = torch.zeros(n, dtype=torch.int64, device="cuda:0")
+    binding.gs_depth_sort_noalloc(t_in, t_out)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream(device="cuda:0")
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        graph.capture_begin()
+        binding.gs_depth_sort_noalloc(t_in, t_out, stream=side)
+        graph.capture_end()
+    torch.cuda.synchronize()
+    for rep in range(3):
+        keys = rng.integers(0, 1 << 62, n, dtype=np.int64).view(np.uint64)
+        t_in.copy_(_dev(keys))
+        graph.replay()
+        torch.cuda.synchronize()
+        hi = keys >> np.uint64(32)
+        assert np.array_equal(t_out.cpu().numpy().view(np.uint64), keys[np.argsort(hi, kind="stable")]), rep
